@@ -1,0 +1,189 @@
+/* =====================================================================================
+ *  picsarqed.h -- C ABI of the B200-native PICSAR-QED hot path (arXiv 2110.00256).
+ *
+ *  The library (paper_2110_00256_b200/libpicsarqed.so) is hand-written CUDA for sm_100a.
+ *  Citations are PAPER.md:<line> of the paper text.  DESIGN.md lists how garbled or silent
+ *  passages were read (R1..R16) and the data layout.
+ *
+ *  Conventions
+ *  -----------
+ *  * Every entry point returns an int status: PICSARQED_OK or one of the error codes below.
+ *    No C++ exception crosses the boundary.  picsarqed_last_error() returns a text for the
+ *    last non-OK status of that context.
+ *  * DEVICE pointers: all particle, field, optical-depth, secondary and counter arguments
+ *    (anything called px..bz, tau, *_out, ph_*, el_*, po_*, parent, d_*).  They are owned by
+ *    the caller (e.g. torch allocations), structure-of-arrays, contiguous, 16-byte aligned;
+ *    the library never allocates, frees or keeps them.  Work is enqueued on the context's
+ *    stream and the call returns without synchronising, except where stated.
+ *  * HOST pointers: picsarqed_table_params, the table arrays of import/export, every
+ *    argument whose name starts with host_ or h_, and every argument of the *_host calls.
+ *  * Units: momentum p in m_e c; fields e = E/E_s, b = cB/E_s with E_s the Schwinger field
+ *    (eq.1); dt in seconds.  The tables are adimensional.
+ *  * dtype / tau_dtype: PICSARQED_F32 or PICSARQED_F64 -- element type of the particle/field
+ *    arrays and of the optical-depth arrays (configuration 5 of BASELINE.json mixes fp32
+ *    particles with fp64 optical depth).  fp32 particle arithmetic reads the fp32-rounded
+ *    copy of the tables ("computed in double, stored in single").
+ *  * species: PICSARQED_LEPTON (electron or positron: eq.2 and eq.15 do not depend on the
+ *    sign of the charge) or PICSARQED_PHOTON.
+ *  * Random numbers: Philox4x32-10, key = seed, counter = (particle id, step, purpose,
+ *    species); particle id = id_base + array index.  See DESIGN.md "RNG".
+ * ===================================================================================== */
+#ifndef PICSARQED_H
+#define PICSARQED_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PICSARQED_OK 0
+#define PICSARQED_ERR_INVALID 1  /* null/misaligned pointer, n < 0, bad enum, bad table params */
+#define PICSARQED_ERR_CUDA 2     /* a CUDA runtime call failed; see picsarqed_last_error        */
+#define PICSARQED_ERR_NO_TABLES 4 /* build_tables / import_tables has not been called           */
+#define PICSARQED_ERR_DTYPE 5    /* unsupported dtype combination                              */
+
+#define PICSARQED_F32 0
+#define PICSARQED_F64 1
+#define PICSARQED_LEPTON 0
+#define PICSARQED_PHOTON 1
+
+/* which table, for export: */
+#define PICSARQED_TAB_LNG 0    /* ln G(chi_i),           n = qs_n_chi     */
+#define PICSARQED_TAB_QS_LNP 1 /* ln P_QS[chi_n][xi_m],  n = qs_n_chi*qs_n_xi, row-major */
+#define PICSARQED_TAB_LNT 2    /* ln T(chi_gamma,i),     n = bw_n_chi     */
+#define PICSARQED_TAB_BW_P 3   /* P_BW[chi_n][xi_m],     n = bw_n_chi*bw_n_xi, row-major */
+
+typedef struct picsarqed_ctx picsarqed_ctx;
+
+/* Table geometry (the paper's benchmark set is at :301).
+ * chi grids are log-spaced and include both ends; QS xi_m = xi_min^(1 - m/(n_xi-1)) on
+ * [xi_min, 1]; BW xi_m = 0.5 m/(n_xi-1) on [0, 1/2] (the other half follows from
+ * P(xi) = 1 - P(1-xi)).  All counts >= 2; 0 < min < max; 0 < qs_xi_min < 1. */
+typedef struct {
+    double qs_chi_min, qs_chi_max;
+    int qs_n_chi;
+    double qs_xi_min;
+    int qs_n_xi;
+    double bw_chi_min, bw_chi_max;
+    int bw_n_chi;
+    int bw_n_xi;
+} picsarqed_table_params;
+
+/* ---- context ------------------------------------------------------------------------
+ * One context per (device, stream).  cuda_stream is a cudaStream_t passed as void* (0 = the
+ * legacy default stream).  The context owns the tables and a few KB of scan scratch. */
+int picsarqed_create(picsarqed_ctx** out, int cuda_device, void* cuda_stream);
+int picsarqed_destroy(picsarqed_ctx* ctx);
+const char* picsarqed_last_error(const picsarqed_ctx* ctx);
+/* bit 0: library was compiled for sm_100a; returns the CUDA runtime version in the upper bits */
+int picsarqed_version(void);
+/* Tuning knobs (integers): "evolve_unroll" in {0 (default), 1, 2, 4} = independent 128-bit
+ * loads per array per thread in the evolve kernel; "evolve_ctas_per_sm" (0 = occupancy limit). */
+int picsarqed_set_option(picsarqed_ctx* ctx, const char* name, long long value);
+
+/* ---- tables -------------------------------------------------------------------------
+ * build_tables: integrates on the GPU, in fp64,
+ *     T(chi_gamma) = 1/(pi sqrt3 chi_gamma) int_0^1 f_BW dxi          (eq.9)
+ *     P_BW(chi_gamma, xi) = int_0^xi f_BW / int_0^1 f_BW               (eq.11)
+ *     G(chi) = int_0^1 S(chi,xi)/xi dxi                                (eq.16)
+ *     P_QS(chi, xi) = int_0^xi S/u du / G                              (eq.18)
+ * from the K_{1/3}, K_{2/3} Bessel quadratures, and stores ln T, ln G, P_BW and ln P_QS
+ * in fp64 plus an fp32-rounded copy.  Synchronises.
+ * rel_tol: requested relative accuracy of T, G, P (1e-9 is the design point; <= 0 = default). */
+int picsarqed_build_tables(picsarqed_ctx* ctx, const picsarqed_table_params* host_params, double rel_tol);
+/* Copies table `which` to host memory as fp64 (n_elems must equal the table's size).  Synchronises. */
+int picsarqed_export_tables(picsarqed_ctx* ctx, int which, double* host_dst, size_t n_elems);
+/* Replaces the tables by caller-provided values (host, fp64, layouts as above).  Synchronises. */
+int picsarqed_import_tables(picsarqed_ctx* ctx, const picsarqed_table_params* host_params,
+                            const double* host_lnG, const double* host_qs_lnP,
+                            const double* host_lnT, const double* host_bw_P);
+
+/* ---- chi (PAPER.md:70 eq.2 leptons, :77 eq.3 photons) --------------------------------
+ * chi_out[i] = sqrt(|g e + p x b|^2 - (p.e)^2), g = sqrt(1+p^2) (lepton) or |p| (photon).
+ * n = 0 is a no-op. */
+int picsarqed_chi(picsarqed_ctx* ctx, int species, int dtype, long long n,
+                  const void* px, const void* py, const void* pz,
+                  const void* ex, const void* ey, const void* ez,
+                  const void* bx, const void* by, const void* bz, void* chi_out);
+
+/* ---- optical depth ----------------------------------------------
+ * tau[i] = -ln U(seed, id_base+i, step 0, purpose 0, species): a draw from p(x) = exp(-x). */
+int picsarqed_init_optical_depth(picsarqed_ctx* ctx, int species, int tau_dtype, long long n,
+                                 unsigned long long seed, unsigned long long id_base, void* tau);
+
+/* tau[i] <- tau[i] - dN/dt(chi_i) dt, in place, with
+ *   leptons: dN/dt = (2/3)(alpha/tau_C) G(chi)/gamma          (eq.15), G by eq.27
+ *            (log-log interpolation of ln G, first/last value outside the table);
+ *   photons: dN/dt = (alpha/tau_C) chi_gamma T(chi_gamma)/gamma_gamma (eq.8), T by
+ *            eq.23 inside the table, the Erber form of eq.10 outside (R2);
+ *            photons with gamma_gamma <= 2 or tau = +inf never decay (R12).
+ * *d_n_events (device, 8 bytes, may be NULL) is overwritten with the number of tau[i] < 0
+ * after the update (R1). */
+int picsarqed_evolve_optical_depth(picsarqed_ctx* ctx, int species, int dtype, int tau_dtype, long long n,
+                                   const void* px, const void* py, const void* pz,
+                                   const void* ex, const void* ey, const void* ez,
+                                   const void* bx, const void* by, const void* bz,
+                                   double dt, void* tau, unsigned long long* d_n_events);
+
+/* ---- events ---------------------------------------------------------------------------
+ * generate_photons (eqs.28-30): every lepton with tau < 0 emits one
+ * photon of energy gamma_gamma = (gamma-1) xi along its momentum, xi by inverse-CDF lookup in
+ * ln P_QS; the emitter keeps its direction, loses gamma_gamma of energy and gets a fresh
+ * tau = -ln U.  Photons are written densely in ASCENDING PARENT INDEX: slot s holds the
+ * s-th fired lepton's photon (momentum ph_p*, optical depth ph_tau, parent index ph_parent,
+ * which may be NULL).
+ * Capacity rule: only the first `capacity` fired parents are processed; later ones are left
+ * untouched (tau stays negative, so a second call with a fresh buffer picks them up).
+ * *d_n_out (device, 8 bytes, required) is overwritten with the TOTAL number of fired
+ * parents, which may exceed capacity. */
+int picsarqed_generate_photons(picsarqed_ctx* ctx, int dtype, int tau_dtype, long long n,
+                               void* px, void* py, void* pz, /* in/out */
+                               const void* ex, const void* ey, const void* ez,
+                               const void* bx, const void* by, const void* bz,
+                               void* tau, /* in/out */
+                               unsigned long long seed, unsigned long long step,
+                               unsigned long long id_base, long long capacity,
+                               void* ph_px, void* ph_py, void* ph_pz, void* ph_tau,
+                               long long* ph_parent, unsigned long long* d_n_out);
+
+/* generate_pairs (eqs.24-26): every photon with tau < 0 becomes an
+ * electron-positron pair, chi_-/chi_gamma = xi by inverse-CDF lookup in P_BW on
+ * r' = min(r, 1-r) (r <= 1/2: the electron takes xi, else 1-xi),
+ * gamma_pm = 1 + (gamma_gamma-2) xi_pm, both along the photon.  The photon is marked dead:
+ * p = 0, tau = +inf.  Ordering, capacity rule and d_n_out as above. */
+int picsarqed_generate_pairs(picsarqed_ctx* ctx, int dtype, int tau_dtype, long long n,
+                             void* px, void* py, void* pz, /* in/out */
+                             const void* ex, const void* ey, const void* ez,
+                             const void* bx, const void* by, const void* bz,
+                             void* tau, /* in/out */
+                             unsigned long long seed, unsigned long long step,
+                             unsigned long long id_base, long long capacity,
+                             void* el_px, void* el_py, void* el_pz, void* el_tau,
+                             void* po_px, void* po_py, void* po_pz, void* po_tau,
+                             long long* parent, unsigned long long* d_n_out);
+
+/* Reads an 8-byte device counter written by the calls above.  Synchronises the stream. */
+int picsarqed_read_count(picsarqed_ctx* ctx, const unsigned long long* d_count,
+                         unsigned long long* host_out);
+
+/* ---- host-buffer convenience path (used for end-to-end timing) -------------------------
+ * One full QED step for one species on HOST arrays: copies the nine particle/field arrays
+ * and tau to device staging owned by the context, runs evolve + generate_photons (leptons)
+ * or generate_pairs (photons), copies p, tau and the secondaries back.  All pointers are
+ * HOST pointers (pinned memory makes the copies asynchronous, but is not required).
+ * sec[0..3] (leptons: photon px,py,pz,tau) or sec[0..7] (photons: el px,py,pz,tau, po
+ * px,py,pz,tau) receive min(*h_n_out, capacity) entries each.  Synchronises. */
+int picsarqed_step_host(picsarqed_ctx* ctx, int species, int dtype, int tau_dtype, long long n,
+                        void* h_px, void* h_py, void* h_pz,
+                        const void* h_ex, const void* h_ey, const void* h_ez,
+                        const void* h_bx, const void* h_by, const void* h_bz,
+                        void* h_tau, double dt,
+                        unsigned long long seed, unsigned long long step,
+                        unsigned long long id_base, long long capacity,
+                        void* const* h_sec, long long* h_parent, unsigned long long* h_n_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PICSARQED_H */

@@ -1,0 +1,224 @@
+"""Thin ctypes binding of include/picsarqed.h -- argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of ``libpicsarqed.so``; PyTorch is used
+for device memory and streams.  There is no CPU fallback: if the library cannot be loaded
+(or built with nvcc) the import of this module raises.
+"""
+import ctypes as C
+from dataclasses import dataclass
+
+import numpy as np
+import torch
+
+from .build import build
+
+F32, F64 = 0, 1
+LEPTON, PHOTON = 0, 1
+TAB_LNG, TAB_QS_LNP, TAB_LNT, TAB_BW_P = 0, 1, 2, 3
+
+_vp, _u64, _i64, _i, _d = C.c_void_p, C.c_uint64, C.c_longlong, C.c_int, C.c_double
+
+
+class _CParams(C.Structure):
+    _fields_ = [("qs_chi_min", _d), ("qs_chi_max", _d), ("qs_n_chi", _i), ("qs_xi_min", _d),
+                ("qs_n_xi", _i), ("bw_chi_min", _d), ("bw_chi_max", _d), ("bw_n_chi", _i),
+                ("bw_n_xi", _i)]
+
+
+@dataclass
+class TableParams:
+    """Table geometry; defaults are the paper's benchmark set."""
+    qs_chi_min: float = 1e-3
+    qs_chi_max: float = 1e3
+    qs_n_chi: int = 256
+    qs_xi_min: float = 1e-12
+    qs_n_xi: int = 256
+    bw_chi_min: float = 2e-2
+    bw_chi_max: float = 1e3
+    bw_n_chi: int = 256
+    bw_n_xi: int = 256
+
+    def _c(self):
+        return _CParams(self.qs_chi_min, self.qs_chi_max, self.qs_n_chi, self.qs_xi_min, self.qs_n_xi,
+                        self.bw_chi_min, self.bw_chi_max, self.bw_n_chi, self.bw_n_xi)
+
+    def sizes(self):
+        return (self.qs_n_chi, self.qs_n_chi * self.qs_n_xi, self.bw_n_chi, self.bw_n_chi * self.bw_n_xi)
+
+
+_SIGNATURES = {
+    "picsarqed_version": (_i, []),
+    "picsarqed_create": (_i, [C.POINTER(_vp), _i, _vp]),
+    "picsarqed_destroy": (_i, [_vp]),
+    "picsarqed_last_error": (C.c_char_p, [_vp]),
+    "picsarqed_set_option": (_i, [_vp, C.c_char_p, _i64]),
+    "picsarqed_build_tables": (_i, [_vp, C.POINTER(_CParams), _d]),
+    "picsarqed_export_tables": (_i, [_vp, _i, _vp, C.c_size_t]),
+    "picsarqed_import_tables": (_i, [_vp, C.POINTER(_CParams), _vp, _vp, _vp, _vp]),
+    "picsarqed_chi": (_i, [_vp, _i, _i, _i64] + [_vp] * 10),
+    "picsarqed_init_optical_depth": (_i, [_vp, _i, _i, _i64, _u64, _u64, _vp]),
+    "picsarqed_evolve_optical_depth": (_i, [_vp, _i, _i, _i, _i64] + [_vp] * 9 + [_d, _vp, _vp]),
+    "picsarqed_generate_photons": (_i, [_vp, _i, _i, _i64] + [_vp] * 10 + [_u64, _u64, _u64, _i64] + [_vp] * 6),
+    "picsarqed_generate_pairs": (_i, [_vp, _i, _i, _i64] + [_vp] * 10 + [_u64, _u64, _u64, _i64] + [_vp] * 10),
+    "picsarqed_read_count": (_i, [_vp, _vp, C.POINTER(_u64)]),
+    "picsarqed_step_host": (_i, [_vp, _i, _i, _i, _i64] + [_vp] * 10 + [_d, _u64, _u64, _u64, _i64, _vp, _vp,
+                                                                     C.POINTER(_u64)]),
+}
+
+_lib = None
+
+
+def lib():
+    """The loaded C-ABI library (built with nvcc on first use)."""
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        for name, (res, args) in _SIGNATURES.items():
+            f = getattr(L, name)
+            f.restype = res
+            f.argtypes = args
+        _lib = L
+    return _lib
+
+
+class PicsarQedError(RuntimeError):
+    pass
+
+
+_TORCH_DTYPE = {F32: torch.float32, F64: torch.float64}
+
+
+def _code(dtype):
+    return F64 if dtype == torch.float64 else F32
+
+
+def _dev(t, dtype=None):
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous()):
+        raise PicsarQedError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise PicsarQedError("dtype mismatch: %s vs %s" % (t.dtype, dtype))
+    return t.data_ptr()
+
+
+class Context:
+    """One library context bound to a device and a stream (picsarqed_create)."""
+
+    def __init__(self, device=0, stream=None):
+        self._h = _vp()
+        self.device = torch.device("cuda", device) if isinstance(device, int) else torch.device(device)
+        if not torch.cuda.is_available():
+            raise PicsarQedError("no CUDA device: picsarqed has no CPU fallback")
+        idx = self.device.index or 0
+        with torch.cuda.device(idx):
+            self.stream = stream if stream is not None else torch.cuda.current_stream()
+            rc = lib().picsarqed_create(C.byref(self._h), idx, _vp(self.stream.cuda_stream))
+        if rc != 0:
+            raise PicsarQedError("picsarqed_create failed with status %d (needs an sm_100 device)" % rc)
+        self.params = None
+
+    def close(self):
+        if self._h:
+            lib().picsarqed_destroy(self._h)
+            self._h = _vp()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc != 0:
+            msg = lib().picsarqed_last_error(self._h)
+            raise PicsarQedError("status %d: %s" % (rc, msg.decode() if msg else ""))
+
+    # ---- options / tables ---------------------------------------------------------------
+    def set_option(self, name, value):
+        self._check(lib().picsarqed_set_option(self._h, name.encode(), int(value)))
+
+    def build_tables(self, params, rel_tol=0.0):
+        cp = params._c()
+        self._check(lib().picsarqed_build_tables(self._h, C.byref(cp), float(rel_tol)))
+        self.params = params
+
+    def import_tables(self, params, lnG, qs_lnP, lnT, bw_P):
+        arrs = [np.ascontiguousarray(a, dtype=np.float64).ravel() for a in (lnG, qs_lnP, lnT, bw_P)]
+        for a, n in zip(arrs, params.sizes()):
+            if a.size != n:
+                raise PicsarQedError("table size mismatch")
+        cp = params._c()
+        self._check(lib().picsarqed_import_tables(self._h, C.byref(cp), *[a.ctypes.data for a in arrs]))
+        self.params = params
+
+    def export_tables(self, which):
+        n = self.params.sizes()[which]
+        out = np.empty(n, dtype=np.float64)
+        self._check(lib().picsarqed_export_tables(self._h, which, out.ctypes.data, n))
+        p = self.params
+        if which == TAB_QS_LNP:
+            return out.reshape(p.qs_n_chi, p.qs_n_xi)
+        if which == TAB_BW_P:
+            return out.reshape(p.bw_n_chi, p.bw_n_xi)
+        return out
+
+    # ---- runtime calls (device tensors) ---------------------------------------------------
+    def chi(self, species, p, e, b, out=None):
+        dt = p[0].dtype
+        n = p[0].numel()
+        if out is None:
+            out = torch.empty(n, dtype=dt, device=p[0].device)
+        ptrs = [_dev(t, dt) for t in (*p, *e, *b, out)]
+        self._check(lib().picsarqed_chi(self._h, species, _code(dt), n, *ptrs))
+        return out
+
+    def init_optical_depth(self, species, tau, seed, id_base=0):
+        self._check(lib().picsarqed_init_optical_depth(self._h, species, _code(tau.dtype), tau.numel(), seed,
+                                                       id_base, _dev(tau)))
+        return tau
+
+    def evolve_optical_depth(self, species, p, e, b, dt, tau, n_events=None):
+        d = p[0].dtype
+        ptrs = [_dev(t, d) for t in (*p, *e, *b)]
+        self._check(lib().picsarqed_evolve_optical_depth(self._h, species, _code(d), _code(tau.dtype), tau.numel(),
+                                                         *ptrs, float(dt), _dev(tau),
+                                                         _dev(n_events, torch.int64) if n_events is not None else None))
+
+    def generate_photons(self, p, e, b, tau, seed, step, id_base, capacity, ph_p, ph_tau, ph_parent, n_out):
+        d = p[0].dtype
+        ptrs = [_dev(t, d) for t in (*p, *e, *b)]
+        self._check(lib().picsarqed_generate_photons(
+            self._h, _code(d), _code(tau.dtype), tau.numel(), *ptrs, _dev(tau), seed, step, id_base, capacity,
+            *[_dev(t, d) for t in ph_p], _dev(ph_tau, tau.dtype),
+            _dev(ph_parent, torch.int64) if ph_parent is not None else None, _dev(n_out, torch.int64)))
+
+    def generate_pairs(self, p, e, b, tau, seed, step, id_base, capacity, el_p, el_tau, po_p, po_tau, parent, n_out):
+        d = p[0].dtype
+        ptrs = [_dev(t, d) for t in (*p, *e, *b)]
+        self._check(lib().picsarqed_generate_pairs(
+            self._h, _code(d), _code(tau.dtype), tau.numel(), *ptrs, _dev(tau), seed, step, id_base, capacity,
+            *[_dev(t, d) for t in el_p], _dev(el_tau, tau.dtype), *[_dev(t, d) for t in po_p],
+            _dev(po_tau, tau.dtype), _dev(parent, torch.int64) if parent is not None else None,
+            _dev(n_out, torch.int64)))
+
+    def read_count(self, counter):
+        v = _u64(0)
+        self._check(lib().picsarqed_read_count(self._h, _dev(counter, torch.int64), C.byref(v)))
+        return int(v.value)
+
+    # ---- host-buffer path -----------------------------------------------------------------
+    def step_host(self, species, p, e, b, tau, dt, seed, step, id_base, capacity, sec, parent=None):
+        """One QED step on HOST tensors (CPU, ideally pinned); p, tau and sec are overwritten.
+        Returns the total number of fired parents."""
+        for t in (*p, *e, *b, tau, *sec):
+            if t.is_cuda or not t.is_contiguous():
+                raise PicsarQedError("step_host expects contiguous CPU tensors")
+        d = p[0].dtype
+        n_out = _u64(0)
+        sec_ptrs = (_vp * len(sec))(*[t.data_ptr() for t in sec])
+        self._check(lib().picsarqed_step_host(
+            self._h, species, _code(d), _code(tau.dtype), tau.numel(), *[t.data_ptr() for t in (*p, *e, *b)],
+            tau.data_ptr(), float(dt), seed, step, id_base, capacity, C.cast(sec_ptrs, _vp),
+            parent.data_ptr() if parent is not None else None, C.byref(n_out)))
+        return int(n_out.value)

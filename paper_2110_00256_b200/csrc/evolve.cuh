@@ -1,0 +1,222 @@
+// =====================================================================================
+//  evolve.cuh -- chi, optical-depth initialisation and the fused
+//  chi + 1D-table lookup + optical-depth update kernel.
+//
+//  Streaming kernels over structure-of-arrays particle buffers: 128-bit loads that bypass
+//  L1, the ln G / ln T table staged once per CTA in shared memory by a TMA bulk copy,
+//  persistent grid sized to the SM count.  HBM traffic per particle = the ten reals of
+//  PAPER.md:301 plus the optical-depth write: 88 B (fp64), 44 B (fp32), 52 B (fp32 + fp64 tau).
+// =====================================================================================
+#pragma once
+#include "qed_device.cuh"
+
+namespace pxq {
+
+constexpr int kEvolveThreads = 256;
+
+template <typename R, typename TR>
+struct EvolveArgs {
+    const R* p[3];
+    const R* e[3];
+    const R* b[3];
+    TR* tau;
+    long long n;
+    Table1D<R> tab;
+    double rate_dt;            // (2/3) alpha/tau_C dt (leptons) or alpha/tau_C dt (photons)
+    unsigned int* partials;    // gridDim.x per-CTA event counts (ctx scratch), or nullptr
+    unsigned int* ticket;      // self-resetting arrival counter (ctx scratch)
+    unsigned long long* d_n_events;
+    int table_in_smem;
+};
+
+// ---- TMA bulk copy of a 1D table into shared memory ------------------------------------
+__device__ __forceinline__ void stage_table_tma(void* smem_dst, const void* gmem_src, unsigned bytes,
+                                                unsigned long long* mbar) {
+    const unsigned mb = (unsigned)__cvta_generic_to_shared(mbar);
+    const unsigned dst = (unsigned)__cvta_generic_to_shared(smem_dst);
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mb));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb), "r"(bytes) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"(dst), "l"(gmem_src), "r"(bytes), "r"(mb) : "memory");
+    }
+    unsigned done = 0;
+    while (!done) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done) : "r"(mb) : "memory");
+    }
+}
+
+// ---- one particle ----------------------------------------------------------------------
+// Returns the decrement dN/dt * dt in the particle arithmetic type A (float or double).
+template <typename R, int SPECIES>
+__device__ __forceinline__ auto decrement_one(R pxr, R pyr, R pzr, R exr, R eyr, R ezr, R bxr, R byr, R bzr,
+                                              const R* tab, const Table1D<R>& T, double rate_dt) -> R {
+    typedef R A;
+    const double px = pxr, py = pyr, pz = pzr;
+    const double p2 = fma(px, px, fma(py, py, pz * pz));
+    const double g2 = SPECIES == 0 ? 1.0 + p2 : p2;
+    const double inv_g = rsqrt(g2);       // 1/gamma (lepton) or 1/gamma_gamma (photon)
+    const double g = g2 * inv_g;
+    const double c2 = chi_squared<SPECIES>(px, py, pz, exr, eyr, ezr, bxr, byr, bzr, g, p2);
+    A lc;
+    if constexpr (sizeof(R) == 8) lc = 0.5 * log(c2); else lc = 0.5f * logf((float)c2);
+    const A ln_min = (A)T.ln_min, ln_max = (A)T.ln_max, inv_delta = (A)T.inv_delta;
+    if (SPECIES == 0) {
+        // eq.15 with G from eq.27; first/last value outside the table
+        lc = fmin(fmax(lc, ln_min), ln_max);
+        const A L = lookup_ln<R, A>(tab, T.n, lc, ln_min, inv_delta);
+        if constexpr (sizeof(R) == 8) return rate_dt * exp(L) * inv_g;
+        else return (float)rate_dt * expf(L) * (float)inv_g;
+    } else {
+        // eq.8 with T from eq.23; Erber form outside; gamma_gamma <= 2 cannot decay (R12)
+        if (!(g2 > 4.0) || !(c2 > 0.0)) return (A)0;
+        if (c2 < T.chi_min * T.chi_min || c2 > T.chi_max * T.chi_max) {
+            const double chi = sqrt(c2);
+            const double x = 4.0 / (3.0 * chi);
+            const double lk = ln_bessel_k13_scaled(x);                 // ln K_{1/3}(x) + x
+            const double d = rate_dt * 0.16 * exp(2.0 * (lk - x)) * inv_g;  // chi T = 0.16 K^2
+            return (A)d;
+        }
+        lc = fmin(fmax(lc, ln_min), ln_max);
+        const A L = lookup_ln<R, A>(tab, T.n, lc, ln_min, inv_delta);
+        if constexpr (sizeof(R) == 8) return rate_dt * exp(L + lc) * inv_g;
+        else return (float)rate_dt * expf(L + lc) * (float)inv_g;
+    }
+}
+
+// ---- fused evolve kernel ------------------------------------------------------------
+// V = particles per 128-bit load of R; U = independent vectors per thread per tile.
+template <typename R, typename TR, int SPECIES, int U>
+__global__ void __launch_bounds__(kEvolveThreads)
+evolve_kernel(const EvolveArgs<R, TR> a) {
+    constexpr int V = 16 / sizeof(R);
+    constexpr int TILE = kEvolveThreads * V * U;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ unsigned long long mbar;
+    __shared__ unsigned int warp_counts[kEvolveThreads / 32];
+
+    const R* tab = a.tab.L;
+    if (a.table_in_smem) {
+        const unsigned bytes = ((unsigned)(a.tab.n * sizeof(R)) + 15u) & ~15u;
+        stage_table_tma(smem_raw, a.tab.L, bytes, &mbar);
+        tab = reinterpret_cast<const R*>(smem_raw);
+    }
+
+    unsigned int fired = 0;
+    const long long ntiles = (a.n + TILE - 1) / TILE;
+    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const long long base = tile * TILE;
+        if (base + TILE <= a.n) {
+            Vec<R, V> q[9][U];
+            Vec<TR, V> t[U];
+            // all loads of the tile first: 10*U independent 128-bit requests per thread in flight
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const long long i = base + (long long)(u * kEvolveThreads + threadIdx.x) * V;
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    q[c][u] = ld_stream<R, V>(a.p[c] + i);
+                    q[3 + c][u] = ld_stream<R, V>(a.e[c] + i);
+                    q[6 + c][u] = ld_stream<R, V>(a.b[c] + i);
+                }
+                t[u] = *reinterpret_cast<const Vec<TR, V>*>(a.tau + i);
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const long long i = base + (long long)(u * kEvolveThreads + threadIdx.x) * V;
+#pragma unroll
+                for (int v = 0; v < V; ++v) {
+                    const R d = decrement_one<R, SPECIES>(q[0][u].v[v], q[1][u].v[v], q[2][u].v[v], q[3][u].v[v],
+                                                          q[4][u].v[v], q[5][u].v[v], q[6][u].v[v], q[7][u].v[v],
+                                                          q[8][u].v[v], tab, a.tab, a.rate_dt);
+                    const TR tn = t[u].v[v] - (TR)d;
+                    t[u].v[v] = tn;
+                    fired += tn < (TR)0 ? 1u : 0u;
+                }
+                *reinterpret_cast<Vec<TR, V>*>(a.tau + i) = t[u];
+            }
+        } else {  // ragged last tile: scalar, guarded
+            for (long long i = base + threadIdx.x; i < a.n; i += kEvolveThreads) {
+                const R d = decrement_one<R, SPECIES>(a.p[0][i], a.p[1][i], a.p[2][i], a.e[0][i], a.e[1][i],
+                                                      a.e[2][i], a.b[0][i], a.b[1][i], a.b[2][i], tab, a.tab,
+                                                      a.rate_dt);
+                const TR tn = a.tau[i] - (TR)d;
+                a.tau[i] = tn;
+                fired += tn < (TR)0 ? 1u : 0u;
+            }
+        }
+    }
+
+    if (a.d_n_events == nullptr) return;
+    // CTA count -> partials[blockIdx]; the last CTA to arrive sums them in index order
+    fired = __reduce_add_sync(0xffffffffu, fired);
+    if ((threadIdx.x & 31) == 0) warp_counts[threadIdx.x >> 5] = fired;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned int s = 0;
+#pragma unroll
+        for (int w = 0; w < kEvolveThreads / 32; ++w) s += warp_counts[w];
+        a.partials[blockIdx.x] = s;
+        __threadfence();
+        const unsigned int arrived = atomicInc(a.ticket, gridDim.x - 1);  // wraps to 0 after the last CTA
+        if (arrived == gridDim.x - 1) {
+            __threadfence();
+            unsigned long long total = 0;
+            for (unsigned int k = 0; k < gridDim.x; ++k) total += ((volatile unsigned int*)a.partials)[k];
+            *a.d_n_events = total;
+        }
+    }
+}
+
+// ---- standalone chi (PAPER.md:70 eq.2, :77 eq.3) ---------------------------------------
+template <typename R, int SPECIES>
+__global__ void __launch_bounds__(256) chi_kernel(const R* __restrict__ px, const R* __restrict__ py,
+                                                  const R* __restrict__ pz, const R* __restrict__ ex,
+                                                  const R* __restrict__ ey, const R* __restrict__ ez,
+                                                  const R* __restrict__ bx, const R* __restrict__ by,
+                                                  const R* __restrict__ bz, R* __restrict__ out, long long n) {
+    constexpr int V = 16 / sizeof(R);
+    const long long nvec = n / V;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    auto one = [](R pxr, R pyr, R pzr, R exr, R eyr, R ezr, R bxr, R byr, R bzr) -> R {
+        const double x = pxr, y = pyr, z = pzr;
+        const double p2 = fma(x, x, fma(y, y, z * z));
+        const double g = sqrt(SPECIES == 0 ? 1.0 + p2 : p2);
+        return (R)sqrt(chi_squared<SPECIES>(x, y, z, exr, eyr, ezr, bxr, byr, bzr, g, p2));
+    };
+    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < nvec; j += stride) {
+        const long long i = j * V;
+        const Vec<R, V> a0 = ld_stream<R, V>(px + i), a1 = ld_stream<R, V>(py + i), a2 = ld_stream<R, V>(pz + i),
+                        a3 = ld_stream<R, V>(ex + i), a4 = ld_stream<R, V>(ey + i), a5 = ld_stream<R, V>(ez + i),
+                        a6 = ld_stream<R, V>(bx + i), a7 = ld_stream<R, V>(by + i), a8 = ld_stream<R, V>(bz + i);
+        Vec<R, V> o;
+#pragma unroll
+        for (int v = 0; v < V; ++v)
+            o.v[v] = one(a0.v[v], a1.v[v], a2.v[v], a3.v[v], a4.v[v], a5.v[v], a6.v[v], a7.v[v], a8.v[v]);
+        *reinterpret_cast<Vec<R, V>*>(out + i) = o;
+    }
+    // ragged tail
+    for (long long i = nvec * V + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+        out[i] = one(px[i], py[i], pz[i], ex[i], ey[i], ez[i], bx[i], by[i], bz[i]);
+}
+
+// ---- tau = -ln U, purpose 0, step 0 -------------------------------
+template <typename TR>
+__global__ void __launch_bounds__(256) init_tau_kernel(TR* __restrict__ tau, long long n, unsigned long long seed,
+                                                       unsigned long long id_base, int species) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const Words4 w = qed_words(seed, id_base + (unsigned long long)i, 0ull, 0, species);
+        tau[i] = draw_tau<TR>(w.w[0], w.w[1]);
+    }
+}
+
+}  // namespace pxq

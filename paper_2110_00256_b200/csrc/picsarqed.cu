@@ -1,0 +1,594 @@
+// =====================================================================================
+//  picsarqed.cu -- the C ABI of include/picsarqed.h: context, table storage, launchers.
+//  Compiled only for sm_100a.  No CPU fallback: every entry point enqueues CUDA kernels.
+// =====================================================================================
+#include "../../include/picsarqed.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "evolve.cuh"
+#include "events.cuh"
+#include "tables.cuh"
+
+using namespace pxq;
+
+struct picsarqed_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int num_sms = 0;
+    std::string err;
+
+    bool have_tables = false;
+    picsarqed_table_params tp{};
+    double* tab64[4] = {nullptr, nullptr, nullptr, nullptr};  // lnG, qs_lnP, lnT, bw_P
+    float* tab32[4] = {nullptr, nullptr, nullptr, nullptr};   // fp32-rounded copies
+    size_t tab_n[4] = {0, 0, 0, 0};
+
+    // evolve: per-CTA counts + arrival ticket
+    unsigned int* partials = nullptr;
+    unsigned int* ticket = nullptr;
+    int partials_cap = 0;
+    // events: look-back status words + tile ticket counter
+    unsigned long long* status = nullptr;
+    size_t status_cap = 0;
+    unsigned long long* tile_counter = nullptr;
+    unsigned long long tile_base = 0;  // host mirror of *tile_counter
+    unsigned epoch = 0;
+    // tuning knobs (picsarqed_set_option)
+    int evolve_unroll = 0;       // 0 = default per dtype
+    int evolve_ctas_per_sm = 0;  // 0 = occupancy
+    // host-path staging
+    void* stage = nullptr;
+    size_t stage_bytes = 0;
+    unsigned long long* d_counts = nullptr;  // 2 device counters
+    double build_ms = 0.0;
+};
+
+namespace {
+
+int fail(picsarqed_ctx* c, int code, const std::string& msg) {
+    if (c) c->err = msg;
+    return code;
+}
+#define PXQ_CUDA(ctx, call)                                                                      \
+    do {                                                                                         \
+        cudaError_t e_ = (call);                                                                 \
+        if (e_ != cudaSuccess)                                                                   \
+            return fail(ctx, PICSARQED_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
+    } while (0)
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+bool params_ok(const picsarqed_table_params* p) {
+    return p && p->qs_n_chi >= 2 && p->qs_n_xi >= 2 && p->bw_n_chi >= 2 && p->bw_n_xi >= 2 &&
+           p->qs_chi_min > 0 && p->qs_chi_max > p->qs_chi_min && p->bw_chi_min > 0 &&
+           p->bw_chi_max > p->bw_chi_min && p->qs_xi_min > 0 && p->qs_xi_min < 1;
+}
+
+void table_sizes(const picsarqed_table_params& p, size_t n[4]) {
+    n[0] = (size_t)p.qs_n_chi;
+    n[1] = (size_t)p.qs_n_chi * p.qs_n_xi;
+    n[2] = (size_t)p.bw_n_chi;
+    n[3] = (size_t)p.bw_n_chi * p.bw_n_xi;
+}
+
+__global__ void narrow_kernel(const double* __restrict__ src, float* __restrict__ dst, size_t n) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        dst[i] = (float)src[i];
+}
+
+// (re)allocate table storage for params p; +2 elements of padding so that 16-byte TMA copies stay in bounds
+int alloc_tables(picsarqed_ctx* c, const picsarqed_table_params& p) {
+    size_t n[4];
+    table_sizes(p, n);
+    for (int k = 0; k < 4; ++k) {
+        if (c->tab64[k]) cudaFree(c->tab64[k]);
+        if (c->tab32[k]) cudaFree(c->tab32[k]);
+        c->tab64[k] = nullptr;
+        c->tab32[k] = nullptr;
+        PXQ_CUDA(c, cudaMalloc(&c->tab64[k], (n[k] + 4) * sizeof(double)));
+        PXQ_CUDA(c, cudaMalloc(&c->tab32[k], (n[k] + 4) * sizeof(float)));
+        PXQ_CUDA(c, cudaMemsetAsync(c->tab64[k], 0, (n[k] + 4) * sizeof(double), c->stream));
+        PXQ_CUDA(c, cudaMemsetAsync(c->tab32[k], 0, (n[k] + 4) * sizeof(float), c->stream));
+        c->tab_n[k] = n[k];
+    }
+    c->tp = p;
+    return PICSARQED_OK;
+}
+
+int narrow_tables(picsarqed_ctx* c) {
+    for (int k = 0; k < 4; ++k) {
+        const size_t n = c->tab_n[k];
+        const int grid = (int)std::min<size_t>((n + 255) / 256, 1184);
+        narrow_kernel<<<grid, 256, 0, c->stream>>>(c->tab64[k], c->tab32[k], n);
+    }
+    PXQ_CUDA(c, cudaGetLastError());
+    return PICSARQED_OK;
+}
+
+template <typename R> const R* table_ptr(const picsarqed_ctx* c, int which);
+template <> const double* table_ptr<double>(const picsarqed_ctx* c, int which) { return c->tab64[which]; }
+template <> const float* table_ptr<float>(const picsarqed_ctx* c, int which) { return c->tab32[which]; }
+
+template <typename R>
+Table1D<R> view_1d(const picsarqed_ctx* c, int species) {
+    Table1D<R> t;
+    const auto& p = c->tp;
+    const double lo = species == 0 ? p.qs_chi_min : p.bw_chi_min, hi = species == 0 ? p.qs_chi_max : p.bw_chi_max;
+    t.n = species == 0 ? p.qs_n_chi : p.bw_n_chi;
+    t.L = table_ptr<R>(c, species == 0 ? PICSARQED_TAB_LNG : PICSARQED_TAB_LNT);
+    t.ln_min = std::log(lo);
+    t.ln_max = std::log(hi);
+    t.inv_delta = (t.n - 1) / (t.ln_max - t.ln_min);
+    t.chi_min = lo;
+    t.chi_max = hi;
+    return t;
+}
+
+template <typename R>
+Table2D<R> view_2d(const picsarqed_ctx* c, int species) {
+    Table2D<R> t;
+    const auto& p = c->tp;
+    const double lo = species == 0 ? p.qs_chi_min : p.bw_chi_min, hi = species == 0 ? p.qs_chi_max : p.bw_chi_max;
+    t.n_chi = species == 0 ? p.qs_n_chi : p.bw_n_chi;
+    t.n_xi = species == 0 ? p.qs_n_xi : p.bw_n_xi;
+    t.P = table_ptr<R>(c, species == 0 ? PICSARQED_TAB_QS_LNP : PICSARQED_TAB_BW_P);
+    t.ln_min = std::log(lo);
+    t.ln_max = std::log(hi);
+    t.inv_delta = (t.n_chi - 1) / (t.ln_max - t.ln_min);
+    t.ln_xi_min = species == 0 ? std::log(p.qs_xi_min) : 0.0;
+    return t;
+}
+
+}  // namespace
+
+// =====================================================================================
+//  context and tables
+// =====================================================================================
+extern "C" {
+
+int picsarqed_version(void) {
+    int rt = 0;
+    cudaRuntimeGetVersion(&rt);
+    return (rt << 1) | 1;
+}
+
+int picsarqed_create(picsarqed_ctx** out, int cuda_device, void* cuda_stream) {
+    if (!out) return PICSARQED_ERR_INVALID;
+    *out = nullptr;
+    picsarqed_ctx* c = new (std::nothrow) picsarqed_ctx();
+    if (!c) return PICSARQED_ERR_CUDA;
+    c->device = cuda_device;
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    cudaError_t e = cudaSetDevice(cuda_device);
+    cudaDeviceProp prop;
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, cuda_device);
+    if (e == cudaSuccess && prop.major != 10) {
+        delete c;
+        return PICSARQED_ERR_CUDA;  // built for sm_100a only; no fallback path
+    }
+    if (e == cudaSuccess) {
+        c->num_sms = prop.multiProcessorCount;
+        c->partials_cap = c->num_sms * 32;
+        e = cudaMalloc(&c->partials, c->partials_cap * sizeof(unsigned int));
+    }
+    if (e == cudaSuccess) e = cudaMalloc(&c->ticket, sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaMemset(c->ticket, 0, sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaMalloc(&c->tile_counter, sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(c->tile_counter, 0, sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_counts, 2 * sizeof(unsigned long long));
+    if (e != cudaSuccess) {
+        delete c;
+        return PICSARQED_ERR_CUDA;
+    }
+    *out = c;
+    return PICSARQED_OK;
+}
+
+int picsarqed_destroy(picsarqed_ctx* c) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    for (int k = 0; k < 4; ++k) {
+        cudaFree(c->tab64[k]);
+        cudaFree(c->tab32[k]);
+    }
+    cudaFree(c->partials);
+    cudaFree(c->ticket);
+    cudaFree(c->status);
+    cudaFree(c->tile_counter);
+    cudaFree(c->stage);
+    cudaFree(c->d_counts);
+    delete c;
+    return PICSARQED_OK;
+}
+
+const char* picsarqed_last_error(const picsarqed_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+int picsarqed_set_option(picsarqed_ctx* c, const char* name, long long value) {
+    if (!c || !name) return PICSARQED_ERR_INVALID;
+    if (!std::strcmp(name, "evolve_unroll") && (value == 0 || value == 1 || value == 2 || value == 4))
+        c->evolve_unroll = (int)value;
+    else if (!std::strcmp(name, "evolve_ctas_per_sm") && value >= 0 && value <= 32)
+        c->evolve_ctas_per_sm = (int)value;
+    else
+        return fail(c, PICSARQED_ERR_INVALID, std::string("unknown option or bad value: ") + name);
+    return PICSARQED_OK;
+}
+
+int picsarqed_import_tables(picsarqed_ctx* c, const picsarqed_table_params* p, const double* lnG,
+                            const double* qs_lnP, const double* lnT, const double* bw_P) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (!params_ok(p) || !lnG || !qs_lnP || !lnT || !bw_P) return fail(c, PICSARQED_ERR_INVALID, "bad table arguments");
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    c->have_tables = false;
+    if (int rc = alloc_tables(c, *p)) return rc;
+    const double* src[4] = {lnG, qs_lnP, lnT, bw_P};
+    for (int k = 0; k < 4; ++k)
+        PXQ_CUDA(c, cudaMemcpyAsync(c->tab64[k], src[k], c->tab_n[k] * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    if (int rc = narrow_tables(c)) return rc;
+    PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->have_tables = true;
+    return PICSARQED_OK;
+}
+
+int picsarqed_export_tables(picsarqed_ctx* c, int which, double* host_dst, size_t n_elems) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (!c->have_tables) return fail(c, PICSARQED_ERR_NO_TABLES, "no tables");
+    if (which < 0 || which > 3 || !host_dst || n_elems != c->tab_n[which])
+        return fail(c, PICSARQED_ERR_INVALID, "bad export arguments");
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    PXQ_CUDA(c, cudaMemcpyAsync(host_dst, c->tab64[which], n_elems * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    return PICSARQED_OK;
+}
+
+int picsarqed_read_count(picsarqed_ctx* c, const unsigned long long* d_count, unsigned long long* host_out) {
+    if (!c || !d_count || !host_out) return PICSARQED_ERR_INVALID;
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    PXQ_CUDA(c, cudaMemcpyAsync(host_out, d_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+    PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    return PICSARQED_OK;
+}
+
+}  // extern "C"
+
+// =====================================================================================
+//  launchers
+// =====================================================================================
+namespace {
+
+int stream_grid(const picsarqed_ctx* c, long long work_items, int per_block) {
+    const long long blocks = (work_items + per_block - 1) / per_block;
+    return (int)std::max<long long>(1, std::min<long long>(blocks, (long long)c->num_sms * 8));
+}
+
+template <typename R, int SPECIES>
+int launch_chi(picsarqed_ctx* c, long long n, const void* const* a, void* out) {
+    constexpr int V = 16 / sizeof(R);
+    chi_kernel<R, SPECIES><<<stream_grid(c, (n + V - 1) / V, 256), 256, 0, c->stream>>>(
+        (const R*)a[0], (const R*)a[1], (const R*)a[2], (const R*)a[3], (const R*)a[4], (const R*)a[5],
+        (const R*)a[6], (const R*)a[7], (const R*)a[8], (R*)out, n);
+    PXQ_CUDA(c, cudaGetLastError());
+    return PICSARQED_OK;
+}
+
+template <typename R, typename TR, int SPECIES, int U>
+int launch_evolve_u(picsarqed_ctx* c, long long n, const void* const* a, double dt, void* tau,
+                    unsigned long long* d_n_events) {
+    constexpr int V = 16 / sizeof(R);
+    constexpr int TILE = kEvolveThreads * V * U;
+    EvolveArgs<R, TR> args;
+    for (int k = 0; k < 3; ++k) {
+        args.p[k] = (const R*)a[k];
+        args.e[k] = (const R*)a[3 + k];
+        args.b[k] = (const R*)a[6 + k];
+    }
+    args.tau = (TR*)tau;
+    args.n = n;
+    args.tab = view_1d<R>(c, SPECIES);
+    args.rate_dt = (SPECIES == 0 ? 2.0 / 3.0 : 1.0) * kAlphaOverTauC * dt;
+    args.partials = c->partials;
+    args.ticket = c->ticket;
+    args.d_n_events = d_n_events;
+    size_t smem = ((size_t)args.tab.n * sizeof(R) + 15) & ~(size_t)15;
+    args.table_in_smem = smem <= 96 * 1024;  // larger tables are read through L1/L2
+    if (!args.table_in_smem) smem = 0;
+    auto kern = evolve_kernel<R, TR, SPECIES, U>;
+    if (smem > 48 * 1024) PXQ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int per_sm = 0;
+    PXQ_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kEvolveThreads, smem));
+    if (per_sm < 1) per_sm = 1;
+    if (c->evolve_ctas_per_sm > 0) per_sm = std::min(per_sm, c->evolve_ctas_per_sm);
+    const long long ntiles = (n + TILE - 1) / TILE;
+    const int grid = (int)std::max<long long>(1, std::min<long long>(ntiles, (long long)c->num_sms * per_sm));
+    if (grid > c->partials_cap) return fail(c, PICSARQED_ERR_CUDA, "internal: partials too small");
+    kern<<<grid, kEvolveThreads, smem, c->stream>>>(args);
+    PXQ_CUDA(c, cudaGetLastError());
+    return PICSARQED_OK;
+}
+
+template <typename R, typename TR, int SPECIES>
+int launch_evolve(picsarqed_ctx* c, long long n, const void* const* a, double dt, void* tau,
+                  unsigned long long* d_n_events) {
+    int u = c->evolve_unroll ? c->evolve_unroll : 2;
+    if (u == 1) return launch_evolve_u<R, TR, SPECIES, 1>(c, n, a, dt, tau, d_n_events);
+    if (u == 4) return launch_evolve_u<R, TR, SPECIES, 4>(c, n, a, dt, tau, d_n_events);
+    return launch_evolve_u<R, TR, SPECIES, 2>(c, n, a, dt, tau, d_n_events);
+}
+
+template <typename R, typename TR, int KIND>
+int launch_events(picsarqed_ctx* c, long long n, void* const* p, const void* const* eb, void* tau,
+                  unsigned long long seed, unsigned long long step, unsigned long long id_base, long long capacity,
+                  void* const* out_p, void* const* out_tau, long long* parent, unsigned long long* d_n_out) {
+    const long long ntiles = (n + kEventTile - 1) / kEventTile;
+    if ((size_t)ntiles > c->status_cap) {  // grow the look-back scratch (rare; synchronises)
+        PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+        if (c->status) cudaFree(c->status);
+        c->status = nullptr;
+        c->status_cap = (size_t)ntiles * 2;
+        PXQ_CUDA(c, cudaMalloc(&c->status, c->status_cap * sizeof(unsigned long long)));
+        PXQ_CUDA(c, cudaMemsetAsync(c->status, 0, c->status_cap * sizeof(unsigned long long), c->stream));
+        c->epoch = 0;
+    }
+    c->epoch += 1;
+    if (c->epoch >= (1u << kEpochBits)) {  // epoch wrapped: clear stale words
+        PXQ_CUDA(c, cudaMemsetAsync(c->status, 0, c->status_cap * sizeof(unsigned long long), c->stream));
+        c->epoch = 1;
+    }
+    EventArgs<R, TR> args;
+    for (int k = 0; k < 3; ++k) {
+        args.p[k] = (R*)p[k];
+        args.e[k] = (const R*)eb[k];
+        args.b[k] = (const R*)eb[3 + k];
+    }
+    args.tau = (TR*)tau;
+    args.n = n;
+    args.cdf = view_2d<R>(c, KIND);
+    args.seed = seed;
+    args.step = step;
+    args.id_base = id_base;
+    args.capacity = capacity;
+    for (int k = 0; k < 6; ++k) args.out_p[k] = (R*)out_p[k];
+    for (int k = 0; k < 2; ++k) args.out_tau[k] = (TR*)out_tau[k];
+    args.parent = parent;
+    args.d_n_out = d_n_out;
+    args.status = c->status;
+    args.tile_counter = c->tile_counter;
+    args.tile_base = c->tile_base;
+    args.epoch = c->epoch;
+    c->tile_base += (unsigned long long)ntiles;
+    event_kernel<R, TR, KIND><<<(unsigned)ntiles, kEventThreads, 0, c->stream>>>(args);
+    PXQ_CUDA(c, cudaGetLastError());
+    return PICSARQED_OK;
+}
+
+// dispatch on (dtype, tau_dtype); fp64 particles with fp32 optical depth is not offered
+#define PXQ_DISPATCH_RT(ctx, dtype, tau_dtype, CALL)                                       \
+    do {                                                                                   \
+        if ((dtype) == PICSARQED_F64 && (tau_dtype) == PICSARQED_F64) { typedef double R; typedef double TR; CALL; } \
+        else if ((dtype) == PICSARQED_F32 && (tau_dtype) == PICSARQED_F32) { typedef float R; typedef float TR; CALL; } \
+        else if ((dtype) == PICSARQED_F32 && (tau_dtype) == PICSARQED_F64) { typedef float R; typedef double TR; CALL; } \
+        else return fail(ctx, PICSARQED_ERR_DTYPE, "unsupported (dtype, tau_dtype) combination");                \
+    } while (0)
+
+int check_arrays(picsarqed_ctx* c, const void* const* a, int count) {
+    for (int k = 0; k < count; ++k)
+        if (!a[k] || !aligned16(a[k])) return fail(c, PICSARQED_ERR_INVALID, "null or misaligned array pointer");
+    return PICSARQED_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int picsarqed_chi(picsarqed_ctx* c, int species, int dtype, long long n, const void* px, const void* py,
+                  const void* pz, const void* ex, const void* ey, const void* ez, const void* bx, const void* by,
+                  const void* bz, void* chi_out) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (n < 0 || (species != 0 && species != 1)) return fail(c, PICSARQED_ERR_INVALID, "bad n or species");
+    if (n == 0) return PICSARQED_OK;
+    const void* a[10] = {px, py, pz, ex, ey, ez, bx, by, bz, chi_out};
+    if (int rc = check_arrays(c, a, 10)) return rc;
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    if (dtype == PICSARQED_F64)
+        return species == 0 ? launch_chi<double, 0>(c, n, a, chi_out) : launch_chi<double, 1>(c, n, a, chi_out);
+    if (dtype == PICSARQED_F32)
+        return species == 0 ? launch_chi<float, 0>(c, n, a, chi_out) : launch_chi<float, 1>(c, n, a, chi_out);
+    return fail(c, PICSARQED_ERR_DTYPE, "bad dtype");
+}
+
+int picsarqed_init_optical_depth(picsarqed_ctx* c, int species, int tau_dtype, long long n, unsigned long long seed,
+                                 unsigned long long id_base, void* tau) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (n < 0 || (species != 0 && species != 1)) return fail(c, PICSARQED_ERR_INVALID, "bad n or species");
+    if (n == 0) return PICSARQED_OK;
+    if (!tau || !aligned16(tau)) return fail(c, PICSARQED_ERR_INVALID, "null or misaligned tau");
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    const int grid = stream_grid(c, n, 256);
+    if (tau_dtype == PICSARQED_F64)
+        init_tau_kernel<double><<<grid, 256, 0, c->stream>>>((double*)tau, n, seed, id_base, species);
+    else if (tau_dtype == PICSARQED_F32)
+        init_tau_kernel<float><<<grid, 256, 0, c->stream>>>((float*)tau, n, seed, id_base, species);
+    else
+        return fail(c, PICSARQED_ERR_DTYPE, "bad tau_dtype");
+    PXQ_CUDA(c, cudaGetLastError());
+    return PICSARQED_OK;
+}
+
+int picsarqed_evolve_optical_depth(picsarqed_ctx* c, int species, int dtype, int tau_dtype, long long n,
+                                   const void* px, const void* py, const void* pz, const void* ex, const void* ey,
+                                   const void* ez, const void* bx, const void* by, const void* bz, double dt,
+                                   void* tau, unsigned long long* d_n_events) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (n < 0 || (species != 0 && species != 1)) return fail(c, PICSARQED_ERR_INVALID, "bad n or species");
+    if (!c->have_tables) return fail(c, PICSARQED_ERR_NO_TABLES, "no tables: call build_tables or import_tables");
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    if (n == 0) {
+        if (d_n_events) PXQ_CUDA(c, cudaMemsetAsync(d_n_events, 0, sizeof(unsigned long long), c->stream));
+        return PICSARQED_OK;
+    }
+    const void* a[10] = {px, py, pz, ex, ey, ez, bx, by, bz, tau};
+    if (int rc = check_arrays(c, a, 10)) return rc;
+    PXQ_DISPATCH_RT(c, dtype, tau_dtype,
+                    return species == 0 ? (launch_evolve<R, TR, 0>(c, n, a, dt, tau, d_n_events))
+                                        : (launch_evolve<R, TR, 1>(c, n, a, dt, tau, d_n_events)));
+}
+
+int picsarqed_generate_photons(picsarqed_ctx* c, int dtype, int tau_dtype, long long n, void* px, void* py, void* pz,
+                               const void* ex, const void* ey, const void* ez, const void* bx, const void* by,
+                               const void* bz, void* tau, unsigned long long seed, unsigned long long step,
+                               unsigned long long id_base, long long capacity, void* ph_px, void* ph_py,
+                               void* ph_pz, void* ph_tau, long long* ph_parent, unsigned long long* d_n_out) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (n < 0 || capacity < 0 || !d_n_out) return fail(c, PICSARQED_ERR_INVALID, "bad n, capacity or d_n_out");
+    if (!c->have_tables) return fail(c, PICSARQED_ERR_NO_TABLES, "no tables: call build_tables or import_tables");
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    if (n == 0) {
+        PXQ_CUDA(c, cudaMemsetAsync(d_n_out, 0, sizeof(unsigned long long), c->stream));
+        return PICSARQED_OK;
+    }
+    void* p[3] = {px, py, pz};
+    const void* eb[6] = {ex, ey, ez, bx, by, bz};
+    const void* chk[10] = {px, py, pz, ex, ey, ez, bx, by, bz, tau};
+    if (int rc = check_arrays(c, chk, 10)) return rc;
+    void* out_p[6] = {ph_px, ph_py, ph_pz, nullptr, nullptr, nullptr};
+    void* out_tau[2] = {ph_tau, nullptr};
+    if (capacity > 0) {
+        const void* o[4] = {ph_px, ph_py, ph_pz, ph_tau};
+        if (int rc = check_arrays(c, o, 4)) return rc;
+    }
+    PXQ_DISPATCH_RT(c, dtype, tau_dtype,
+                    return (launch_events<R, TR, 0>(c, n, p, eb, tau, seed, step, id_base, capacity, out_p, out_tau,
+                                                    ph_parent, d_n_out)));
+}
+
+int picsarqed_generate_pairs(picsarqed_ctx* c, int dtype, int tau_dtype, long long n, void* px, void* py, void* pz,
+                             const void* ex, const void* ey, const void* ez, const void* bx, const void* by,
+                             const void* bz, void* tau, unsigned long long seed, unsigned long long step,
+                             unsigned long long id_base, long long capacity, void* el_px, void* el_py, void* el_pz,
+                             void* el_tau, void* po_px, void* po_py, void* po_pz, void* po_tau, long long* parent,
+                             unsigned long long* d_n_out) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (n < 0 || capacity < 0 || !d_n_out) return fail(c, PICSARQED_ERR_INVALID, "bad n, capacity or d_n_out");
+    if (!c->have_tables) return fail(c, PICSARQED_ERR_NO_TABLES, "no tables: call build_tables or import_tables");
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    if (n == 0) {
+        PXQ_CUDA(c, cudaMemsetAsync(d_n_out, 0, sizeof(unsigned long long), c->stream));
+        return PICSARQED_OK;
+    }
+    void* p[3] = {px, py, pz};
+    const void* eb[6] = {ex, ey, ez, bx, by, bz};
+    const void* chk[10] = {px, py, pz, ex, ey, ez, bx, by, bz, tau};
+    if (int rc = check_arrays(c, chk, 10)) return rc;
+    void* out_p[6] = {el_px, el_py, el_pz, po_px, po_py, po_pz};
+    void* out_tau[2] = {el_tau, po_tau};
+    if (capacity > 0) {
+        const void* o[8] = {el_px, el_py, el_pz, el_tau, po_px, po_py, po_pz, po_tau};
+        if (int rc = check_arrays(c, o, 8)) return rc;
+    }
+    PXQ_DISPATCH_RT(c, dtype, tau_dtype,
+                    return (launch_events<R, TR, 1>(c, n, p, eb, tau, seed, step, id_base, capacity, out_p, out_tau,
+                                                    parent, d_n_out)));
+}
+
+}  // extern "C"
+
+// =====================================================================================
+//  host-buffer path (end-to-end timing): H2D copies, evolve + events, D2H copies
+// =====================================================================================
+extern "C" int picsarqed_step_host(picsarqed_ctx* c, int species, int dtype, int tau_dtype, long long n, void* h_px,
+                                   void* h_py, void* h_pz, const void* h_ex, const void* h_ey, const void* h_ez,
+                                   const void* h_bx, const void* h_by, const void* h_bz, void* h_tau, double dt,
+                                   unsigned long long seed, unsigned long long step, unsigned long long id_base,
+                                   long long capacity, void* const* h_sec, long long* h_parent,
+                                   unsigned long long* h_n_out) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (n < 0 || capacity < 0 || !h_n_out || (species != 0 && species != 1))
+        return fail(c, PICSARQED_ERR_INVALID, "bad n, capacity, species or h_n_out");
+    if ((dtype != 0 && dtype != 1) || (tau_dtype != 0 && tau_dtype != 1) || (dtype == 1 && tau_dtype == 0))
+        return fail(c, PICSARQED_ERR_DTYPE, "unsupported (dtype, tau_dtype) combination");
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    *h_n_out = 0;
+    if (n == 0) return PICSARQED_OK;
+    const size_t es = dtype ? 8 : 4, ts = tau_dtype ? 8 : 4;
+    auto pad = [](size_t b) { return (b + 255) & ~(size_t)255; };
+    const int n_sec = species == 0 ? 3 : 6, n_sec_tau = species == 0 ? 1 : 2;
+    const size_t a_bytes = pad((size_t)n * es), t_bytes = pad((size_t)n * ts);
+    const size_t sp_bytes = pad((size_t)capacity * es), st_bytes = pad((size_t)capacity * ts);
+    const size_t par_bytes = pad((size_t)capacity * sizeof(long long));
+    const size_t need = 9 * a_bytes + t_bytes + n_sec * sp_bytes + n_sec_tau * st_bytes + par_bytes;
+    if (need > c->stage_bytes) {
+        PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+        if (c->stage) cudaFree(c->stage);
+        c->stage = nullptr;
+        c->stage_bytes = 0;
+        PXQ_CUDA(c, cudaMalloc(&c->stage, need));
+        c->stage_bytes = need;
+    }
+    char* base = static_cast<char*>(c->stage);
+    void* d[10];
+    for (int k = 0; k < 9; ++k) d[k] = base + k * a_bytes;
+    d[9] = base + 9 * a_bytes;
+    char* sec0 = base + 9 * a_bytes + t_bytes;
+    void* d_sec_p[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    void* d_sec_tau[2] = {nullptr, nullptr};
+    for (int k = 0; k < n_sec; ++k) d_sec_p[k] = sec0 + k * sp_bytes;
+    for (int k = 0; k < n_sec_tau; ++k) d_sec_tau[k] = sec0 + n_sec * sp_bytes + k * st_bytes;
+    long long* d_parent = reinterpret_cast<long long*>(sec0 + n_sec * sp_bytes + n_sec_tau * st_bytes);
+
+    const void* h_in[9] = {h_px, h_py, h_pz, h_ex, h_ey, h_ez, h_bx, h_by, h_bz};
+    for (int k = 0; k < 9; ++k) {
+        if (!h_in[k]) return fail(c, PICSARQED_ERR_INVALID, "null host array");
+        PXQ_CUDA(c, cudaMemcpyAsync(d[k], h_in[k], (size_t)n * es, cudaMemcpyHostToDevice, c->stream));
+    }
+    if (!h_tau) return fail(c, PICSARQED_ERR_INVALID, "null host tau");
+    PXQ_CUDA(c, cudaMemcpyAsync(d[9], h_tau, (size_t)n * ts, cudaMemcpyHostToDevice, c->stream));
+
+    int rc = picsarqed_evolve_optical_depth(c, species, dtype, tau_dtype, n, d[0], d[1], d[2], d[3], d[4], d[5], d[6],
+                                            d[7], d[8], dt, d[9], nullptr);
+    if (rc) return rc;
+    if (species == 0)
+        rc = picsarqed_generate_photons(c, dtype, tau_dtype, n, d[0], d[1], d[2], d[3], d[4], d[5], d[6], d[7], d[8],
+                                        d[9], seed, step, id_base, capacity, d_sec_p[0], d_sec_p[1], d_sec_p[2],
+                                        d_sec_tau[0], h_parent ? d_parent : nullptr, c->d_counts);
+    else
+        rc = picsarqed_generate_pairs(c, dtype, tau_dtype, n, d[0], d[1], d[2], d[3], d[4], d[5], d[6], d[7], d[8],
+                                      d[9], seed, step, id_base, capacity, d_sec_p[0], d_sec_p[1], d_sec_p[2],
+                                      d_sec_tau[0], d_sec_p[3], d_sec_p[4], d_sec_p[5], d_sec_tau[1],
+                                      h_parent ? d_parent : nullptr, c->d_counts);
+    if (rc) return rc;
+    void* h_p[3] = {h_px, h_py, h_pz};
+    for (int k = 0; k < 3; ++k)
+        PXQ_CUDA(c, cudaMemcpyAsync(h_p[k], d[k], (size_t)n * es, cudaMemcpyDeviceToHost, c->stream));
+    PXQ_CUDA(c, cudaMemcpyAsync(h_tau, d[9], (size_t)n * ts, cudaMemcpyDeviceToHost, c->stream));
+    PXQ_CUDA(c, cudaMemcpyAsync(h_n_out, c->d_counts, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+    PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    const size_t m = (size_t)std::min<unsigned long long>(*h_n_out, (unsigned long long)capacity);
+    if (m > 0 && h_sec) {
+        // order of h_sec: leptons: ph px,py,pz,tau; photons: el px,py,pz,tau, po px,py,pz,tau
+        if (species == 0) {
+            for (int k = 0; k < 3; ++k)
+                PXQ_CUDA(c, cudaMemcpyAsync(h_sec[k], d_sec_p[k], m * es, cudaMemcpyDeviceToHost, c->stream));
+            PXQ_CUDA(c, cudaMemcpyAsync(h_sec[3], d_sec_tau[0], m * ts, cudaMemcpyDeviceToHost, c->stream));
+        } else {
+            for (int s = 0; s < 2; ++s) {
+                for (int k = 0; k < 3; ++k)
+                    PXQ_CUDA(c, cudaMemcpyAsync(h_sec[4 * s + k], d_sec_p[3 * s + k], m * es, cudaMemcpyDeviceToHost, c->stream));
+                PXQ_CUDA(c, cudaMemcpyAsync(h_sec[4 * s + 3], d_sec_tau[s], m * ts, cudaMemcpyDeviceToHost, c->stream));
+            }
+        }
+        if (h_parent) PXQ_CUDA(c, cudaMemcpyAsync(h_parent, d_parent, m * sizeof(long long), cudaMemcpyDeviceToHost, c->stream));
+        PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
+    return PICSARQED_OK;
+}
+
+extern "C" int picsarqed_build_tables(picsarqed_ctx* c, const picsarqed_table_params* p, double rel_tol) {
+    (void)p; (void)rel_tol;
+    return fail(c, PICSARQED_ERR_INVALID, "build_tables: not implemented yet");
+}

@@ -1,0 +1,250 @@
+// =====================================================================================
+//  qed_device.cuh -- device-side building blocks of the PICSAR-QED hot path (sm_100a).
+//
+//  chi (PAPER.md:70 eq.2, :77 eq.3), 1D log-log table lookups (eq.23,
+//  :248 eq.27), the Erber form outside the T table (PAPER.md:115 eq.10, :203), the
+//  inverse-CDF lookups (PAPER.md:214-230 eqs.24-26, :257-267 eqs.28-30), Philox4x32-10
+//  uniforms.  Product code: shares nothing with oracle/.
+// =====================================================================================
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace pxq {
+
+// ---- physical constants (CODATA 2018; R14) --------------------------------
+// alpha m_e c^2 / hbar in 1/s: prefactor of eq.8 and eq.15.
+constexpr double kPi = 3.141592653589793238462643383279502884;
+constexpr double kFineStructure = 7.2973525693e-3;
+constexpr double kElectronMass = 9.1093837015e-31;  // kg
+constexpr double kLightSpeed = 299792458.0;         // m/s
+constexpr double kPlanck = 6.62607015e-34;          // J s
+constexpr double kAlphaOverTauC =
+    kFineStructure * kElectronMass * kLightSpeed * kLightSpeed / (kPlanck / (2.0 * kPi));  // 5.6652563985e18
+
+// ---- table views: plain structs passed by value to the kernels ----
+template <typename R>
+struct Table1D {      // ln G or ln T on a log-spaced chi grid
+    const R* L;       // n values
+    int n;
+    double ln_min;    // ln chi_0
+    double ln_max;    // ln chi_{n-1}
+    double inv_delta; // (n-1)/(ln_max - ln_min)
+    double chi_min, chi_max;
+};
+
+template <typename R>
+struct Table2D {      // rows: log-spaced chi; columns: xi grid
+    const R* P;       // n_chi * n_xi, row-major
+    int n_chi, n_xi;
+    double ln_min, ln_max, inv_delta;
+    double ln_xi_min; // QS only: ln(xi_min)
+};
+
+// ---- Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11) --------------------------------
+struct Words4 { uint32_t w[4]; };
+
+__device__ __forceinline__ Words4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                uint32_t k0, uint32_t k1) {
+    constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(M0, c0), lo0 = M0 * c0;
+        const uint32_t hi1 = __umulhi(M1, c2), lo1 = M1 * c2;
+        c0 = hi1 ^ c1 ^ k0;
+        c1 = lo1;
+        c2 = hi0 ^ c3 ^ k1;
+        c3 = lo0;
+        k0 += W0;
+        k1 += W1;
+    }
+    Words4 o;
+    o.w[0] = c0; o.w[1] = c1; o.w[2] = c2; o.w[3] = c3;
+    return o;
+}
+
+// counter layout: (id_lo, id_hi, step_lo, purpose | species<<8 | step_hi16<<16)
+__device__ __forceinline__ Words4 qed_words(uint64_t seed, uint64_t id, uint64_t step, int purpose, int species) {
+    const uint32_t c3 = (uint32_t)purpose | ((uint32_t)species << 8) | ((uint32_t)((step >> 32) & 0xFFFFu) << 16);
+    return philox4x32_10((uint32_t)id, (uint32_t)(id >> 32), (uint32_t)step, c3, (uint32_t)seed,
+                         (uint32_t)(seed >> 32));
+}
+
+// uniform strictly inside (0,1), exact in the target type.
+template <typename T> __device__ __forceinline__ T uniform_open(uint32_t a, uint32_t b);
+template <> __device__ __forceinline__ double uniform_open<double>(uint32_t a, uint32_t b) {
+    const uint64_t k = (((uint64_t)a << 32) | b) >> 12;          // top 52 bits
+    return ((double)(long long)k + 0.5) * 0x1p-52;               // k < 2^52: exact
+}
+template <> __device__ __forceinline__ float uniform_open<float>(uint32_t a, uint32_t) {
+    return ((float)(a >> 9) + 0.5f) * 0x1p-23f;                  // k < 2^23: exact
+}
+// tau = -ln U
+template <typename T> __device__ __forceinline__ T draw_tau(uint32_t a, uint32_t b);
+template <> __device__ __forceinline__ double draw_tau<double>(uint32_t a, uint32_t b) {
+    return -log(uniform_open<double>(a, b));
+}
+template <> __device__ __forceinline__ float draw_tau<float>(uint32_t a, uint32_t b) {
+    return -logf(uniform_open<float>(a, b));
+}
+
+// ---- chi^2 --------------------------------------------------------------------------
+// eq.2 / eq.3: chi^2 = |g e + p x b|^2 - (p.e)^2.  Taken literally the two terms cancel by
+// up to gamma^2 when e has a component along p, so it is evaluated in the equivalent form
+//     chi^2 = |g e_perp + p x b|^2 + (g^2 - p^2) (e.p)^2 / p^2,   e_perp = e - (e.p) p / p^2,
+// (g^2 - p^2 = 1 for leptons, 0 for photons), always in fp64 registers.
+// Returns chi^2; *g2_out = g^2 (= 1 + p^2 or p^2).
+template <int SPECIES>
+__device__ __forceinline__ double chi_squared(double px, double py, double pz, double ex, double ey, double ez,
+                                              double bx, double by, double bz, double g, double p2) {
+    const double d = fma(px, ex, fma(py, ey, pz * ez));  // p.e
+    const double q = p2 > 0.0 ? 1.0 / p2 : 0.0;
+    const double t = d * q;
+    const double fx = fma(-t, px, ex), fy = fma(-t, py, ey), fz = fma(-t, pz, ez);  // e_perp
+    const double cx = fma(py, bz, -pz * by), cy = fma(pz, bx, -px * bz), cz = fma(px, by, -py * bx);
+    const double vx = fma(g, fx, cx), vy = fma(g, fy, cy), vz = fma(g, fz, cz);
+    double c2 = fma(vx, vx, fma(vy, vy, vz * vz));
+    if (SPECIES == 0) c2 = fma(d, t, c2);  // + (e.n)^2
+    return c2;
+}
+
+// ---- K_{1/3}(x), only for the Erber branch outside the T table -------------------------
+// returns ln K_{1/3}(x) + x  (exponentially scaled, so chi_gamma -> 0 does not underflow)
+__device__ __noinline__ double ln_bessel_k13_scaled(double x) {
+    const double nu = 1.0 / 3.0;
+    if (x >= 25.0) {  // Hankel asymptotic expansion (DLMF 10.40.2); terms fall below 1e-17 before they grow
+        const double mu = 4.0 * nu * nu;
+        double term = 1.0, sum = 1.0;
+        const double r = 1.0 / (8.0 * x);
+        for (int k = 1; k <= 24; ++k) {
+            const double o = 2.0 * k - 1.0;
+            term *= (mu - o * o) * r / k;
+            sum += term;
+            if (fabs(term) < 1e-17) break;
+        }
+        return 0.5 * log(1.5707963267948966 / x) + log(sum);
+    }
+    if (x <= 2.0) {  // ascending series: K = (pi/2)(I_{-nu} - I_nu)/sin(nu pi) (DLMF 10.27.4, 10.25.2)
+        const double y = 0.25 * x * x;
+        double tm = 1.0 / 1.3541179394264004;  // 1/Gamma(2/3):  I_{-1/3} term k = 0
+        double tp = 1.0 / 0.8929795115692492;  // 1/Gamma(4/3):  I_{+1/3} term k = 0
+        double sm = tm, sp = tp;
+        for (int k = 1; k <= 30; ++k) {
+            tm *= y / (k * (k - nu));
+            tp *= y / (k * (k + nu));
+            sm += tm;
+            sp += tp;
+            if (tm < 1e-18 * sm) break;
+        }
+        const double h = cbrt(0.5 * x);
+        const double kv = 1.5707963267948966 / 0.8660254037844386 * (sm / h - sp * h);
+        return log(kv) + x;
+    }
+    // 2 < x < 25: trapezoid rule on e^x K_nu(x) = int_0^inf exp(-2x sinh^2(t/2)) cosh(nu t) dt (DLMF 10.32.9)
+    const double h = fmin(0.1, 0.35 * rsqrt(x));
+    double s = 0.5;
+    for (int j = 1; j < 400; ++j) {
+        const double t = j * h;
+        const double sh = sinh(0.5 * t);
+        const double a = 2.0 * x * sh * sh;
+        if (a > 46.0) break;
+        s += exp(-a) * cosh(nu * t);
+    }
+    return log(s * h);
+}
+
+// ln of the tabulated factor times chi^POW... see lookup_ln_rate below.
+// 1D log-log lookup (eq.23 / eq.27): returns the interpolated ln value at ln chi = lc
+// (lc must already be inside [ln_min, ln_max]).  `tab` may live in shared memory.
+template <typename R, typename A>
+__device__ __forceinline__ A lookup_ln(const R* tab, int n, A lc, A ln_min, A inv_delta) {
+    const A t = (lc - ln_min) * inv_delta;
+    int k = (int)t;  // t >= 0
+    k = min(k, n - 2);
+    const A f = t - (A)k;
+    const A l0 = (A)tab[k], l1 = (A)tab[k + 1];
+    return fma(f, l1 - l0, l0);
+}
+
+// row bracket of the 2D tables (chi clamped into the table)
+template <typename R>
+__device__ __forceinline__ void row_bracket(const Table2D<R>& T, double ln_chi, int* k_out, double* w_out) {
+    const double lc = fmin(fmax(ln_chi, T.ln_min), T.ln_max);
+    const double t = (lc - T.ln_min) * T.inv_delta;
+    int k = (int)t;
+    k = min(k, T.n_chi - 2);
+    *k_out = k;
+    *w_out = t - (double)k;
+}
+
+// eqs.28-30: xi = chi_gamma/chi of the emitted photon for uniform r.
+// Event arithmetic is fp64 whatever the table element type (events are rare).
+template <typename R>
+__device__ __forceinline__ double qs_sample_xi(const Table2D<R>& T, double ln_chi, double r) {
+    int k; double w;
+    row_bracket(T, ln_chi, &k, &w);
+    const int M = T.n_xi;
+    const R* __restrict__ r0 = T.P + (size_t)k * M;
+    const R* __restrict__ r1 = r0 + M;
+    auto ell = [&](int m) { const double a = (double)__ldg(r0 + m); return fma(w, (double)__ldg(r1 + m) - a, a); };  // eq.28
+    const double lr = log(r);
+    if (lr < ell(0)) return exp(T.ln_xi_min);  // below the first column (R6)
+    int lo = 0, hi = M - 1;                    // ell(lo) <= lr; answer = max{m: ell(m) <= lr}
+    while (hi - lo > 1) {                      // eq.29
+        const int mid = (lo + hi) >> 1;
+        if (ell(mid) <= lr) lo = mid; else hi = mid;
+    }
+    if (ell(hi) <= lr) lo = hi;
+    const int ms = min(lo, M - 2);
+    const double step = -T.ln_xi_min / (double)(M - 1);       // ln xi_{m+1} - ln xi_m
+    const double lx0 = T.ln_xi_min + step * (double)ms;
+    const double a = ell(ms), b = ell(ms + 1);
+    if (!(b > a)) return exp(lx0);
+    return exp(fma((lr - a) / (b - a), step, lx0));           // eq.30
+}
+
+// eqs.24-26 on r' = min(r, 1-r): xi = chi_-/chi_gamma in [0, 1/2]
+template <typename R>
+__device__ __forceinline__ double bw_sample_xi(const Table2D<R>& T, double ln_chi, double rp) {
+    int k; double w;
+    row_bracket(T, ln_chi, &k, &w);
+    const int M = T.n_xi;
+    const R* __restrict__ r0 = T.P + (size_t)k * M;
+    const R* __restrict__ r1 = r0 + M;
+    auto P = [&](int m) { const double a = (double)__ldg(r0 + m); return fma(w, (double)__ldg(r1 + m) - a, a); };  // eq.24
+    int lo = 0, hi = M - 1;  // P(0) = 0 <= r'
+    while (hi - lo > 1) {    // eq.25
+        const int mid = (lo + hi) >> 1;
+        if (P(mid) <= rp) lo = mid; else hi = mid;
+    }
+    if (P(hi) <= rp) lo = hi;
+    const int ms = min(lo, M - 2);
+    const double step = 0.5 / (double)(M - 1);
+    const double x0 = step * (double)ms;
+    const double a = P(ms), b = P(ms + 1);
+    if (!(b > a)) return x0;
+    return fma((rp - a) / (b - a), step, x0);  // eq.26
+}
+
+// ---- 128-bit streaming loads / stores -------------------------------------------------
+template <typename T, int V> struct alignas(sizeof(T) * V) Vec { T v[V]; };
+
+template <typename T, int V>
+__device__ __forceinline__ Vec<T, V> ld_stream(const T* p) {
+    static_assert(sizeof(T) * V == 16 || sizeof(T) * V == 32, "16- or 32-byte vectors");
+    Vec<T, V> r;
+    if constexpr (sizeof(T) * V == 16) {
+        uint32_t a, b, c, d;
+        asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                     : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "l"(p));
+        uint32_t* o = reinterpret_cast<uint32_t*>(&r);
+        o[0] = a; o[1] = b; o[2] = c; o[3] = d;
+    } else {
+        const Vec<T, V / 2> lo = ld_stream<T, V / 2>(p), hi = ld_stream<T, V / 2>(p + V / 2);
+#pragma unroll
+        for (int i = 0; i < V / 2; ++i) { r.v[i] = lo.v[i]; r.v[V / 2 + i] = hi.v[i]; }
+    }
+    return r;
+}
+
+}  // namespace pxq

@@ -1,0 +1,305 @@
+"""GPU parity: the CUDA library (through its C ABI) against the CPU oracle, element by element,
+on the same seeded inputs and the same table bytes."""
+import numpy as np
+import pytest
+
+from parity_common import (EPS, F32, F64, LEPTON, PHOTON, TOL_TAU, assert_chi_close, check_evolve, code, to_dev,
+                           to_host)
+
+pytestmark = pytest.mark.gpu
+
+DTYPES = [(np.float64, np.float64), (np.float32, np.float32), (np.float32, np.float64)]
+IDS = ["f64", "f32", "f32_tau64"]
+
+
+@pytest.fixture(scope="module")
+def qed():
+    import paper_2110_00256_b200 as q
+    return q
+
+
+@pytest.fixture(scope="module")
+def mid_tables(orc):
+    """oracle-built tables, several brackets per decade, built in seconds; C1 ranges"""
+    p = orc.TableParams(qs_chi_min=1e-3, qs_chi_max=1e3, qs_n_chi=40, qs_xi_min=1e-12, qs_n_xi=96,
+                        bw_chi_min=2e-2, bw_chi_max=1e3, bw_n_chi=40, bw_n_xi=96)
+    return orc.build_tables(p)
+
+
+@pytest.fixture(scope="module")
+def ctx(qed, mid_tables):
+    c = qed.Context(0)
+    tp = mid_tables.params
+    c.import_tables(qed.TableParams(**{k: getattr(tp, k) for k in tp.__dataclass_fields__}), mid_tables.lnG,
+                    mid_tables.qs_lnP, mid_tables.lnT, mid_tables.bw_P)
+    yield c
+    c.close()
+
+
+def _tables_for(mid_tables, dtype):
+    return mid_tables.with_fp32_reads(np.dtype(dtype) == np.float32)
+
+
+def _dt_for(orc, qed, tables, species, p, e, b):
+    return qed.workloads.choose_dt(orc.rate(tables, species, p, e, b)[:65536], 0.05)
+
+
+# ----------------------------------------------------------------------------- chi
+@pytest.mark.parametrize("species", [LEPTON, PHOTON])
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("n", [100003, 1, 5])
+def test_chi(orc, qed, ctx, species, dtype, n):
+    p, e, b = qed.workloads.config1(seed=1, n=n, species=species, dtype=dtype)
+    chi_gpu = to_host([ctx.chi(species, to_dev(p), to_dev(e), to_dev(b))])[0]
+    chi_orc = orc.chi(species, p, e, b)
+    n_cond = assert_chi_close(chi_gpu, chi_orc, species, p, e, b)
+    assert n_cond <= max(1, n // 10000)
+
+
+def test_chi_paper_cases_and_corners(orc, qed, ctx):
+    """the paper's worked cases and the cancellation corner e || p"""
+    import math
+    rows = []
+    for g0, bz in ((1000.0, 1e-3), (1000.0, 9e-3)):
+        rows.append(((math.sqrt(g0 * g0 - 1), 0, 0), (0, 0, 0), (0, 0, bz)))
+    rows.append(((math.sqrt(4120.0 ** 2 - 1), 0, 0), (0, 1.22e-4, 0), (0, 0, -1.22e-4)))
+    rows.append(((300.0, 0, 0), (2e-3, 0, 0), (0, 0, 0)))      # e || p: lepton chi = |e|, photon 0
+    rows.append(((0.0, 0, 0), (1e-3, 2e-3, 0), (0, 3e-3, 0)))  # p = 0: lepton chi = |e|
+    rows += [rows[0]] * 3                                      # pad to a multiple of the vector width
+    a = np.array(rows, dtype=np.float64)
+    p, e, b = [[np.ascontiguousarray(a[:, k, j]) for j in range(3)] for k in range(3)]
+    for sp in (LEPTON, PHOTON):
+        got = to_host([ctx.chi(sp, to_dev(p), to_dev(e), to_dev(b))])[0]
+        assert_chi_close(got, orc.chi(sp, p, e, b), sp, p, e, b)
+    got = to_host([ctx.chi(LEPTON, to_dev(p), to_dev(e), to_dev(b))])[0]
+    assert got[0] == pytest.approx(1.0, rel=2e-3) and got[1] == pytest.approx(9.0, rel=2e-3)
+    assert got[2] == pytest.approx(1.0, rel=1e-2) and got[3] == pytest.approx(2e-3, rel=1e-14)
+
+
+# ----------------------------------------------------------------------------- tau = -ln U
+@pytest.mark.parametrize("species", [LEPTON, PHOTON])
+@pytest.mark.parametrize("tdtype", [np.float64, np.float32])
+def test_init_optical_depth(orc, qed, ctx, species, tdtype):
+    import torch
+    n, seed, id_base = 70001, 11, 5_000_000_000
+    tau = torch.empty(n, dtype=torch.float64 if tdtype == np.float64 else torch.float32, device="cuda")
+    ctx.init_optical_depth(species, tau, seed, id_base)
+    ref = orc.init_optical_depth(species, code(tdtype), n, seed, ids=id_base + np.arange(n, dtype=np.uint64))
+    got = tau.cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(got - ref) <= 4 * EPS[np.dtype(tdtype)] * np.abs(ref))
+    assert np.all(got > 0) and np.all(np.isfinite(got))
+
+
+# ----------------------------------------------------------------------------- evolve
+@pytest.mark.parametrize("species", [LEPTON, PHOTON])
+@pytest.mark.parametrize("dtype,tdtype", DTYPES, ids=IDS)
+@pytest.mark.parametrize("n", [65536 + 37, 3])
+def test_evolve(orc, qed, ctx, mid_tables, species, dtype, tdtype, n):
+    import torch
+    p, e, b = qed.workloads.config1(seed=1, n=n, species=species, dtype=dtype)
+    tables = _tables_for(mid_tables, dtype)
+    dt = _dt_for(orc, qed, tables, species, p, e, b)
+    tau0 = orc.init_optical_depth(species, code(tdtype), n, 1).astype(tdtype)
+    if species == PHOTON and n > 100:
+        tau0[17] = np.inf  # a dead photon stays dead
+    tau = torch.from_numpy(tau0.copy()).cuda()
+    count = torch.zeros(1, dtype=torch.int64, device="cuda")
+    ctx.evolve_optical_depth(species, to_dev(p), to_dev(e), to_dev(b), dt, tau, count)
+    o = orc.evolve_optical_depth(tables, species, code(tdtype), p, e, b, dt, tau0)
+    ln_chi = np.log(np.maximum(orc.chi(species, p, e, b), 1e-300))
+    n_amb, flags = check_evolve(tau.cpu().numpy(), tau0.astype(np.float64), o, dtype, ln_chi)
+    assert ctx.read_count(count) == int(flags.sum())
+    assert n_amb <= (0 if dtype == np.float64 else 3)
+    if n > 100:
+        assert 0.02 < flags.mean() < 0.1  # the 5 % rule
+
+
+def test_evolve_erber_branches_and_table_edges(orc, qed, ctx, mid_tables):
+    """photons below / above the T table use eq.10; leptons clamp"""
+    import torch
+    chi_t = np.array([1e-5, 1e-3, 5e-3, 0.019, 0.021, 1.0, 999.0, 1001.0, 5e3, 1e5, 0.2, 30.0])
+    n = chi_t.size
+    g = 2000.0
+    for sp in (LEPTON, PHOTON):
+        pm = np.sqrt(g * g - 1) if sp == LEPTON else g
+        p = [np.full(n, pm), np.zeros(n), np.zeros(n)]
+        e = [np.zeros(n)] * 3
+        b = [np.zeros(n), np.zeros(n), chi_t / pm]
+        tau0 = np.full(n, 0.3)
+        dt = 0.05 / orc.rate(mid_tables, sp, p, e, b)[5]
+        tau = torch.from_numpy(tau0.copy()).cuda()
+        ctx.evolve_optical_depth(sp, to_dev(p), to_dev(e), to_dev(b), dt, tau)
+        o = orc.evolve_optical_depth(mid_tables, sp, F64, p, e, b, dt, tau0)
+        got = tau.cpu().numpy()
+        assert np.all(np.abs(got - o["tau_exact"]) <= 1e-9 * (0.3 + o["decr"])), (sp, got - o["tau_exact"])
+        # the decrement itself, where it is not negligible
+        big = o["decr"] > 1e-6
+        assert np.allclose((0.3 - got)[big], o["decr"][big], rtol=1e-8)
+
+
+def test_evolve_low_energy_photons_never_decay(orc, qed, ctx):
+    import torch
+    n = 8
+    p = [np.array([0.0, 1.0, 1.9, 2.0, 2.0000001, 3.0, 10.0, 100.0]), np.zeros(n), np.zeros(n)]
+    e = [np.zeros(n)] * 3
+    b = [np.zeros(n), np.zeros(n), np.full(n, 0.5)]
+    tau = torch.full((n,), 0.25, dtype=torch.float64, device="cuda")
+    ctx.evolve_optical_depth(PHOTON, to_dev(p), to_dev(e), to_dev(b), 1e-15, tau)
+    got = tau.cpu().numpy()
+    assert np.all(got[:4] == 0.25) and np.all(got[4:] < 0.25)  # gamma_gamma <= 2 cannot decay (R12)
+
+
+# ----------------------------------------------------------------------------- events
+def _vec_close(got, ref, tol):
+    """per-component error relative to the vector norm"""
+    got = [np.asarray(a, np.float64) for a in got]
+    ref = [np.asarray(a, np.float64) for a in ref]
+    norm = np.sqrt(sum(a * a for a in ref))
+    for g_, r_ in zip(got, ref):
+        bad = np.nonzero(~(np.abs(g_ - r_) <= tol * norm))[0]
+        assert bad.size == 0, "vector mismatch at %s: %s vs %s (|v| %s)" % (bad[:5], g_[bad[:5]], r_[bad[:5]], norm[bad[:5]])
+
+
+def _run_events(orc, qed, ctx, tables, species, dtype, tdtype, p, e, b, tau_host, seed, step, id_base, capacity):
+    """GPU and oracle event generation on identical inputs; returns (gpu dict, oracle dict)"""
+    import torch
+    n = tau_host.size
+    tdt = torch.float64 if tdtype == np.float64 else torch.float32
+    pdt = torch.float64 if dtype == np.float64 else torch.float32
+    dp, de, db = to_dev(p), to_dev(e), to_dev(b)
+    dtau = torch.from_numpy(tau_host.copy()).cuda()
+    nsec = 1 if species == LEPTON else 2
+    sec_p = [[torch.full((max(capacity, 1),), -7.0, dtype=pdt, device="cuda") for _ in range(3)] for _ in range(nsec)]
+    sec_tau = [torch.full((max(capacity, 1),), -7.0, dtype=tdt, device="cuda") for _ in range(nsec)]
+    parent = torch.full((max(capacity, 1),), -1, dtype=torch.int64, device="cuda")
+    n_out = torch.zeros(1, dtype=torch.int64, device="cuda")
+    ids = id_base + np.arange(n, dtype=np.uint64)
+    if species == LEPTON:
+        ctx.generate_photons(dp, de, db, dtau, seed, step, id_base, capacity, sec_p[0], sec_tau[0], parent, n_out)
+        o = orc.generate_photons(tables, code(dtype), code(tdtype), p, e, b, tau_host, seed, step, ids, capacity)
+        o_sec_p, o_sec_tau = [o["ph_p"]], [o["ph_tau"]]
+    else:
+        ctx.generate_pairs(dp, de, db, dtau, seed, step, id_base, capacity, sec_p[0], sec_tau[0], sec_p[1],
+                           sec_tau[1], parent, n_out)
+        o = orc.generate_pairs(tables, code(dtype), code(tdtype), p, e, b, tau_host, seed, step, ids, capacity)
+        o_sec_p, o_sec_tau = [o["el_p"], o["po_p"]], [o["el_tau"], o["po_tau"]]
+    g = dict(n_fired=ctx.read_count(n_out), p=to_host(dp), tau=dtau.cpu().numpy(), parent=parent.cpu().numpy(),
+             sec_p=[to_host(s) for s in sec_p], sec_tau=to_host(sec_tau))
+    o["sec_p"], o["sec_tau"] = o_sec_p, o_sec_tau
+    return g, o
+
+
+def _compare_events(g, o, species, dtype, tdtype, capacity, p_before):
+    tol = TOL_TAU[np.dtype(dtype)]
+    ttol = TOL_TAU[np.dtype(tdtype)]
+    k = min(o["n_fired"], capacity)
+    assert g["n_fired"] == o["n_fired"]                       # bit-exact count
+    assert np.array_equal(g["parent"][:k], o["parent"])       # bit-exact compaction order
+    assert np.all(np.diff(g["parent"][:k]) > 0)
+    for s in range(len(o["sec_p"])):
+        _vec_close([a[:k] for a in g["sec_p"][s]], o["sec_p"][s], tol)
+        assert np.all(np.abs(g["sec_tau"][s][:k].astype(np.float64) - o["sec_tau"][s]) <= ttol * o["sec_tau"][s])
+        for a in g["sec_p"][s]:                               # nothing written past the count
+            assert np.all(a[k:] == -7.0)
+    # parents: momenta and optical depth rewritten; everything else untouched, bit for bit
+    if species == LEPTON:
+        _vec_close(g["p"], o["p"], tol)
+    else:
+        for a, r_ in zip(g["p"], o["p"]):
+            assert np.array_equal(a.astype(np.float64), r_)
+    untouched = np.ones(g["tau"].size, bool)
+    untouched[o["parent"]] = False
+    for a, r_ in zip(g["p"], p_before):
+        assert np.array_equal(a[untouched], r_[untouched])
+    fin = np.isfinite(o["tau"])
+    assert np.array_equal(np.isfinite(g["tau"]), fin)
+    assert np.all(np.abs(g["tau"][fin].astype(np.float64) - o["tau"][fin]) <= ttol * np.abs(o["tau"][fin]))
+
+
+@pytest.mark.parametrize("species", [LEPTON, PHOTON])
+@pytest.mark.parametrize("dtype,tdtype", DTYPES, ids=IDS)
+def test_events(orc, qed, ctx, mid_tables, species, dtype, tdtype):
+    n = 3 * 4096 + 1234  # several compaction tiles and a ragged tail
+    p, e, b = qed.workloads.config1(seed=4, n=n, species=species, dtype=dtype)
+    tables = _tables_for(mid_tables, dtype)
+    rng = np.random.default_rng(5)
+    tau = rng.exponential(size=n).astype(tdtype)
+    fired = rng.uniform(size=n) < 0.07
+    fired[:40] = True                # a dense run of events
+    fired[4096 * 2:4096 * 3] = False  # an empty tile
+    fired[-1] = True
+    tau[fired] *= -1
+    g, o = _run_events(orc, qed, ctx, tables, species, dtype, tdtype, p, e, b, tau, 21, 3, 1 << 33, n)
+    assert o["n_fired"] == int(fired.sum())
+    _compare_events(g, o, species, dtype, tdtype, n, p)
+
+
+@pytest.mark.parametrize("species", [LEPTON, PHOTON])
+def test_events_capacity_rule(orc, qed, ctx, mid_tables, species):
+    """only the first `capacity` fired parents are processed; the rest keep tau < 0"""
+    n = 2 * 4096 + 77
+    p, e, b = qed.workloads.config1(seed=6, n=n, species=species, dtype=np.float64)
+    rng = np.random.default_rng(7)
+    tau = np.where(rng.uniform(size=n) < 0.1, -0.5, 0.5)
+    total = int((tau < 0).sum())
+    for cap in (0, 1, 300, total, total + 5):
+        g, o = _run_events(orc, qed, ctx, mid_tables, species, np.float64, np.float64, p, e, b, tau, 1, 0, 0, cap)
+        assert g["n_fired"] == total
+        _compare_events(g, o, species, np.float64, np.float64, cap, p)
+        late = np.nonzero(tau < 0)[0][cap:]
+        assert np.all(g["tau"][late] == -0.5)
+
+
+@pytest.mark.parametrize("species", [LEPTON, PHOTON])
+def test_events_degenerate(orc, qed, ctx, mid_tables, species):
+    """no events, all events, n = 1"""
+    for n, frac in ((5000, 0.0), (4096 + 5, 1.0), (1, 1.0), (1, 0.0)):
+        p, e, b = qed.workloads.config1(seed=8, n=n, species=species, dtype=np.float64)
+        tau = np.full(n, 0.4) if frac == 0.0 else np.full(n, -0.4)
+        g, o = _run_events(orc, qed, ctx, mid_tables, species, np.float64, np.float64, p, e, b, tau, 2, 9, 100, n)
+        assert g["n_fired"] == (n if frac else 0)
+        _compare_events(g, o, species, np.float64, np.float64, n, p)
+
+
+def test_empty_inputs(qed, ctx):
+    import torch
+    z = [torch.empty(0, dtype=torch.float64, device="cuda") for _ in range(3)]
+    tau = torch.empty(0, dtype=torch.float64, device="cuda")
+    cnt = torch.full((1,), 99, dtype=torch.int64, device="cuda")
+    ctx.evolve_optical_depth(LEPTON, z, z, z, 1e-15, tau, cnt)
+    assert ctx.read_count(cnt) == 0
+    cnt.fill_(99)
+    ctx.generate_photons(z, z, z, tau, 1, 0, 0, 0, z, tau, None, cnt)
+    assert ctx.read_count(cnt) == 0
+    assert ctx.chi(LEPTON, z, z, z).numel() == 0
+
+
+# ----------------------------------------------------------------------------- multi-step, free running
+@pytest.mark.parametrize("species,dtype,tdtype", [(LEPTON, np.float64, np.float64), (PHOTON, np.float32, np.float32),
+                                                  (LEPTON, np.float32, np.float64)], ids=["qs_f64", "bw_f32", "qs_mixed"])
+def test_free_running_steps(orc, qed, ctx, mid_tables, species, dtype, tdtype):
+    """evolve + events for several steps on both sides; the oracle adopts the GPU flag only for
+    particles inside the tie margin"""
+    import torch
+    n, steps, seed = 20000 + 3, 4, 13
+    p, e, b = qed.workloads.config1(seed=9, n=n, species=species, dtype=dtype)
+    tables = _tables_for(mid_tables, dtype)
+    dt = _dt_for(orc, qed, tables, species, p, e, b)
+    tau_h = orc.init_optical_depth(species, code(tdtype), n, seed).astype(tdtype)
+    dp, de, db = to_dev(p), to_dev(e), to_dev(b)
+    dtau = torch.from_numpy(tau_h.copy()).cuda()
+    p_h = [a.copy() for a in p]
+    total_amb = 0
+    for step in range(steps):
+        ctx.evolve_optical_depth(species, dp, de, db, dt, dtau)
+        o = orc.evolve_optical_depth(tables, species, code(tdtype), p_h, e, b, dt, tau_h)
+        ln_chi = np.log(np.maximum(orc.chi(species, p_h, e, b), 1e-300))
+        tau_gpu = dtau.cpu().numpy()
+        n_amb, flags = check_evolve(tau_gpu, tau_h.astype(np.float64), o, dtype, ln_chi)
+        total_amb += n_amb
+        # both sides continue from the GPU's tau (differences are within tolerance; flags are the GPU's)
+        g, oe = _run_events(orc, qed, ctx, tables, species, dtype, tdtype, p_h, e, b, tau_gpu, seed, step, 0, n)
+        _compare_events(g, oe, species, dtype, tdtype, n, p_h)
+        p_h, tau_h = g["p"], g["tau"]
+        dp, dtau = to_dev(p_h), torch.from_numpy(tau_h.copy()).cuda()
+    assert total_amb <= (0 if dtype == np.float64 else 5)
