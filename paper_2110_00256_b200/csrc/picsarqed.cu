@@ -589,6 +589,36 @@ extern "C" int picsarqed_step_host(picsarqed_ctx* c, int species, int dtype, int
 }
 
 extern "C" int picsarqed_build_tables(picsarqed_ctx* c, const picsarqed_table_params* p, double rel_tol) {
-    (void)p; (void)rel_tol;
-    return fail(c, PICSARQED_ERR_INVALID, "build_tables: not implemented yet");
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (!params_ok(p)) return fail(c, PICSARQED_ERR_INVALID, "bad table parameters");
+    if (rel_tol > 0 && rel_tol < 1e-10)
+        return fail(c, PICSARQED_ERR_INVALID, "rel_tol below the builder's design accuracy (1e-10)");
+    if ((size_t)std::max(p->qs_n_xi, p->bw_n_xi) * sizeof(double) > 200 * 1024)
+        return fail(c, PICSARQED_ERR_INVALID, "n_xi too large for the row builder (max 25600)");
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    c->have_tables = false;
+    if (int rc = alloc_tables(c, *p)) return rc;
+    for (int kind = 0; kind < 2; ++kind) {
+        TableBuildArgs a;
+        a.chi_min = kind == 0 ? p->qs_chi_min : p->bw_chi_min;
+        a.chi_max = kind == 0 ? p->qs_chi_max : p->bw_chi_max;
+        a.n_chi = kind == 0 ? p->qs_n_chi : p->bw_n_chi;
+        a.n_xi = kind == 0 ? p->qs_n_xi : p->bw_n_xi;
+        a.xi_min = p->qs_xi_min;
+        a.rows = c->tab64[kind == 0 ? PICSARQED_TAB_QS_LNP : PICSARQED_TAB_BW_P];
+        a.ln1d = c->tab64[kind == 0 ? PICSARQED_TAB_LNG : PICSARQED_TAB_LNT];
+        const size_t smem = (size_t)a.n_xi * sizeof(double);
+        if (kind == 0) {
+            if (smem > 48 * 1024) PXQ_CUDA(c, cudaFuncSetAttribute(table_rows_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            table_rows_kernel<0><<<a.n_chi, kTabThreads, smem, c->stream>>>(a);
+        } else {
+            if (smem > 48 * 1024) PXQ_CUDA(c, cudaFuncSetAttribute(table_rows_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            table_rows_kernel<1><<<a.n_chi, kTabThreads, smem, c->stream>>>(a);
+        }
+        PXQ_CUDA(c, cudaGetLastError());
+    }
+    if (int rc = narrow_tables(c)) return rc;
+    PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->have_tables = true;
+    return PICSARQED_OK;
 }
