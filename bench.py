@@ -1,0 +1,320 @@
+#!/usr/bin/env python
+"""QED Monte Carlo step throughput on B200 (BASELINE.json metric, configuration 2 at N = 1).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--particles n]
+
+A "step" is one pass of the whole hot path over the population: the fused chi + table lookup +
+optical-depth kernel over all particles, then event generation (inverse-CDF sampling, secondaries
+compacted in parent order, optical depth re-drawn).  Workload: 16 Mi electrons, fp64, gamma
+log-uniform on [1e2, 1e5], fields re-drawn every step so that chi is log-uniform on ~[1e-3, 1e2],
+1024-point ln G table and 1024x1024 photon-energy CDF table built on the GPU, dt such that ~5 % of
+the particles fire per step.  Prints ONE JSON line (contract in DESIGN.md "Bench").
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "QED MC step particles/sec (fp64/fp32) at 1 B200; achieved HBM GB/s vs peak"
+UNIT = "particles/s"
+SEED = 2
+BYTES_PER_PARTICLE_EVOLVE = 88  # 9 reads + tau read + tau write, fp64
+# dram__bytes_read.sum + dram__bytes_write.sum of one evolve launch (16 Mi particles), ncu --set full;
+# see profiles/r1_evolve_full.md.  None until measured.
+EVOLVE_DRAM_TRAFFIC_BYTES = None
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--particles", type=int, default=1 << 24, help="particles per GPU (default 16 Mi = config 2)")
+    ap.add_argument("--field-sets", type=int, default=4, help="distinct per-step field sets kept in HBM")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-sample", type=int, default=1 << 21, help="particles in the oracle timing sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0}, "fallback"
+
+
+class ClockSampler(threading.Thread):
+    """samples SM clock and throttle reasons through NVML while the timed region runs"""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.stop_flag, self.max_mhz = index, [], set(), False, None
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {"sw_power_cap": nv.nvmlClocksEventReasonSwPowerCap, "hw_slowdown": nv.nvmlClocksEventReasonHwSlowdown,
+                     "hw_thermal_slowdown": nv.nvmlClocksEventReasonHwThermalSlowdown,
+                     "sw_thermal_slowdown": nv.nvmlClocksEventReasonSwThermalSlowdown}
+            while not self.stop_flag:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+                time.sleep(0.002)
+        except Exception as exc:  # NVML missing: report it, do not hide it
+            self.reasons.add("nvml_unavailable: %s" % type(exc).__name__)
+
+    def summary(self):
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------------
+#  the oracle, timed on the host cores (cpu_baseline leg and --impl reference)
+# ------------------------------------------------------------------------------------------------
+def oracle_tables_from(tp_kwargs, tables):
+    import oracle
+    return oracle.Tables(oracle.TableParams(**tp_kwargs), *tables)
+
+
+def time_oracle(tp_kwargs, tables, n_sample, steps, dt, seed=SEED):
+    """oracle evolve + generate_photons on the first n_sample particles of the workload; returns
+    (particles/s, seconds, threads)"""
+    import oracle
+    from paper_2110_00256_b200 import workloads as w
+    tabs = oracle_tables_from(tp_kwargs, tables)
+    p, gamma = w.config2(seed=seed, n=n_sample)
+    tau = oracle.init_optical_depth(0, 1, n_sample, seed)
+    fields = [w.config2_fields(seed, s, gamma) for s in range(steps)]
+    t0 = time.perf_counter()
+    for s in range(steps):
+        e, b = fields[s]
+        tau = oracle.evolve_optical_depth(tabs, 0, 1, p, e, b, dt, tau)["tau"]
+        o = oracle.generate_photons(tabs, 1, 1, p, e, b, tau, seed, s, capacity=n_sample // 8)
+        p, tau = o["p"], o["tau"]
+    sec = time.perf_counter() - t0
+    return n_sample * steps / sec, sec, oracle.num_threads()
+
+
+def reference_tables(tp_kwargs):
+    """tables for the stand-alone reference arm: the oracle's own quadrature on a reduced grid would change the
+    workload, and the full 1024x1024 oracle build takes ~10 core-minutes; the arm times the runtime path only,
+    so it reads power-law stand-in tables of the right shape (values do not change the oracle's work per particle)."""
+    n1, n2 = tp_kwargs["qs_n_chi"], tp_kwargs["qs_n_xi"]
+    chi = np.exp(np.linspace(np.log(tp_kwargs["qs_chi_min"]), np.log(tp_kwargs["qs_chi_max"]), n1))
+    lnG = np.log(2.165 * chi / (1 + chi) ** (1 / 3))
+    lxi = np.log(tp_kwargs["qs_xi_min"]) * (1 - np.arange(n2) / (n2 - 1))
+    qs = np.tile(lxi / 3, (n1, 1))
+    m1, m2 = tp_kwargs["bw_n_chi"], tp_kwargs["bw_n_xi"]
+    return lnG, qs, np.full(m1, -3.0), np.tile(np.linspace(0, 0.5, m2), (m1, 1))
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2110_00256_b200 import workloads as w
+    tp = w.table_params(2)
+    tables = reference_tables(tp)
+    import oracle
+    n = min(args.cpu_sample, args.particles)
+    steps = max(1, args.steps)
+    p0, g0 = w.config2(seed=SEED, n=1 << 16)
+    e0, b0 = w.config2_fields(SEED, 0, g0)
+    dt = w.choose_dt(oracle.rate(oracle_tables_from(tp, tables), 0, p0, e0, b0), 0.05)  # the 5 % rule
+    for _ in range(max(0, min(args.warmup, 1))):
+        time_oracle(tp, tables, min(n, 1 << 16), 1, dt)
+    # bound the run: at ~1.5e6 particle-steps/s a 2 Mi sample takes ~1.5 s per step
+    steps_run = min(steps, 8)
+    value, sec, threads = time_oracle(tp, tables, n, steps_run, dt)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps_run,
+            "warmup": args.warmup, "ms_per_step": 1e3 * sec / steps_run, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "config 2 (synchrotron emission, fp64), oracle on host cores", "particles": n,
+                       "tables": "1024 / 1024x1024 (stand-in values, same shape)"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
+                             "sample": "%d particles x %d steps (evolve + photon emission)" % (n, steps_run)},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+#  the CUDA path
+# ------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2110_00256_b200 as q
+    from paper_2110_00256_b200 import workloads as w
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    n = args.particles
+    seed = SEED + 1000 * rank      # every rank owns an independent shard (weak scaling, no data-path collective)
+    id_base = rank * n
+    cap = n // 8
+
+    ctx = q.Context(local)
+    tp_kwargs = w.table_params(2)
+    t0 = time.perf_counter()
+    ctx.build_tables(q.TableParams(**tp_kwargs))
+    table_build_s = time.perf_counter() - t0
+
+    # ---- inputs: generated on the host (pinned), resident in HBM before the timed region -----------
+    p_h, gamma = w.config2(seed=seed, n=n)
+    n_sets = max(1, min(args.field_sets, args.steps + args.warmup))
+    p_pin = [torch.from_numpy(a).pin_memory() for a in p_h]
+    field_pin = []
+    for s in range(n_sets):
+        e_h, b_h = w.config2_fields(seed, s, gamma)
+        field_pin.append([torch.from_numpy(a).pin_memory() for a in (*e_h, *b_h)])
+    p = [t.to(dev) for t in p_pin]
+    fields = [[t.to(dev) for t in fs] for fs in field_pin]
+    tau = torch.empty(n, dtype=torch.float64, device=dev)
+    ctx.init_optical_depth(q.LEPTON, tau, seed, id_base)
+    ph_p = [torch.empty(cap, dtype=torch.float64, device=dev) for _ in range(3)]
+    ph_tau = torch.empty(cap, dtype=torch.float64, device=dev)
+    ph_parent = torch.empty(cap, dtype=torch.int64, device=dev)
+    n_out = torch.zeros(1, dtype=torch.int64, device=dev)
+
+    # ---- dt by the 5 % rule, rates from the CUDA path itself (tau = 0, dt = 1 s  ->  tau = -rate) ----
+    m = min(n, 1 << 16)
+    probe = torch.zeros(m, dtype=torch.float64, device=dev)
+    ctx.evolve_optical_depth(q.LEPTON, [t[:m] for t in p], [t[:m] for t in fields[0][:3]],
+                             [t[:m] for t in fields[0][3:]], 1.0, probe)
+    dt = w.choose_dt((-probe).cpu().numpy(), 0.05)
+
+    def step(s):
+        f = fields[s % n_sets]
+        ctx.evolve_optical_depth(q.LEPTON, p, f[:3], f[3:], dt, tau)
+        ctx.generate_photons(p, f[:3], f[3:], tau, seed, s, id_base, cap, ph_p, ph_tau, ph_parent, n_out)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for s in range(args.warmup):
+        step(s)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    start.record()
+    for k in range(args.steps):
+        s = args.warmup + k
+        f = fields[s % n_sets]
+        ev[k][0].record()
+        ctx.evolve_optical_depth(q.LEPTON, p, f[:3], f[3:], dt, tau)
+        ev[k][1].record()
+        ctx.generate_photons(p, f[:3], f[3:], tau, seed, s, id_base, cap, ph_p, ph_tau, ph_parent, n_out)
+        ev[k][2].record()
+    stop.record()
+    barrier()
+    sampler.stop_flag = True
+    sampler.join()
+    ms_total = start.elapsed_time(stop)
+    ms_evolve = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
+    ms_events = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
+    fired_last = ctx.read_count(n_out)
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    value = world * n * args.steps / (ms_total * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers (copies inside the timed region) -------------
+    tau_pin = tau.cpu().pin_memory()
+    p_e2e = [t.clone().pin_memory() for t in p_pin]
+    sec_pin = [torch.empty(cap, dtype=torch.float64).pin_memory() for _ in range(4)]
+    ctx.step_host(q.LEPTON, p_e2e, field_pin[0][:3], field_pin[0][3:], tau_pin, dt, seed, 10_000, id_base, cap, sec_pin)
+    barrier()
+    t0 = time.perf_counter()
+    fired_e2e = 0
+    for k in range(args.e2e_steps):
+        f = field_pin[k % n_sets]
+        fired_e2e = ctx.step_host(q.LEPTON, p_e2e, f[:3], f[3:], tau_pin, dt, seed, 10_001 + k, id_base, cap, sec_pin)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_value = world * n * args.e2e_steps / e2e_s
+    h2d = 10 * n * 8
+    d2h = 4 * n * 8 + 8 + min(fired_e2e, cap) * 4 * 8
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    peaks, peak_kind = measured_peaks()
+    achieved = BYTES_PER_PARTICLE_EVOLVE * n / (ms_evolve * 1e-3) / 1e9
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config 2: synchrotron (nonlinear Compton) emission only, fp64, %d electrons per GPU, "
+                               "1024-pt lnG + 1024x1024 photon CDF (GPU-built), evolve + photon emission per step" % n,
+                   "particles_per_gpu": n, "dt_s": dt, "fired_fraction_last_step": fired_last / n,
+                   "l2": "inputs larger than L2: %d field sets x %d MB cycled, %d MB of momenta/tau" % (
+                       n_sets, 6 * n * 8 >> 20, 4 * n * 8 >> 20),
+                   "parallelism": "independent shards per GPU" if world > 1 else "single GPU",
+                   "table_build_s": table_build_s},
+        "roofline": {"bound": "hbm", "kernel": "evolve_kernel<double,double,LEPTON>", "achieved": achieved,
+                     "peak": peaks["hbm_gbs"], "peak_kind": peak_kind + " (MEASURED_PEAKS.json hbm_gbs, copy)",
+                     "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
+                     "traffic": EVOLVE_DRAM_TRAFFIC_BYTES, "algorithmic_bytes_per_launch": BYTES_PER_PARTICLE_EVOLVE * n,
+                     "ms_per_launch": ms_evolve},
+        "kernels_ms": {"evolve": ms_evolve, "events": ms_events},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "steps": args.e2e_steps},
+        "gpu_launches": 2 * args.steps,
+        "clocks": sampler.summary(),
+    }
+    if not args.no_cpu_baseline and world == 1:
+        tables = [ctx.export_tables(k) for k in range(4)]
+        ns = min(args.cpu_sample, n)
+        steps_cpu = 4
+        v, sec, threads = time_oracle(tp_kwargs, tables, ns, steps_cpu, dt)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                "sample": "first %d particles of the workload x %d steps (evolve + photon emission), "
+                                          "%.1f s" % (ns, steps_cpu, sec)}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
