@@ -27,9 +27,9 @@ METRIC = "QED MC step particles/sec (fp64/fp32) at 1 B200; achieved HBM GB/s vs 
 UNIT = "particles/s"
 SEED = 2
 BYTES_PER_PARTICLE_EVOLVE = 88  # 9 reads + tau read + tau write, fp64
-# dram__bytes_read.sum + dram__bytes_write.sum of one evolve launch (16 Mi particles), ncu --set full;
-# see profiles/r1_evolve_full.md.  None until measured.
-EVOLVE_DRAM_TRAFFIC_BYTES = None
+# dram__bytes_read.sum + dram__bytes_write.sum of one step_kernel launch (16 Mi particles), ncu --set full;
+# see profiles/.  None until measured.
+STEP_DRAM_TRAFFIC_BYTES = None
 
 
 def parse():
@@ -208,8 +208,7 @@ def run_ours(args):
 
     def step(s):
         f = fields[s % n_sets]
-        ctx.evolve_optical_depth(q.LEPTON, p, f[:3], f[3:], dt, tau)
-        ctx.generate_photons(p, f[:3], f[3:], tau, seed, s, id_base, cap, ph_p, ph_tau, ph_parent, n_out)
+        ctx.qed_step(q.LEPTON, p, f[:3], f[3:], tau, dt, seed, s, id_base, cap, ph_p, ph_tau, None, None, ph_parent, n_out)
 
     def barrier():
         if world > 1:
@@ -221,25 +220,33 @@ def run_ours(args):
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(args.steps)]
     start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     start.record()
     for k in range(args.steps):
-        s = args.warmup + k
-        f = fields[s % n_sets]
         ev[k][0].record()
-        ctx.evolve_optical_depth(q.LEPTON, p, f[:3], f[3:], dt, tau)
+        step(args.warmup + k)      # one launch: step_kernel<double,double,LEPTON>
         ev[k][1].record()
-        ctx.generate_photons(p, f[:3], f[3:], tau, seed, s, id_base, cap, ph_p, ph_tau, ph_parent, n_out)
-        ev[k][2].record()
     stop.record()
     barrier()
     sampler.stop_flag = True
     sampler.join()
     ms_total = start.elapsed_time(stop)
-    ms_evolve = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
-    ms_events = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
+    ms_kernel = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
     fired_last = ctx.read_count(n_out)
+    # the two-kernel path (evolve, then generate_photons) on the same state, for the per-kernel split
+    split = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(5)]
+    for k in range(5):
+        s = args.warmup + args.steps + k
+        f = fields[s % n_sets]
+        split[k][0].record()
+        ctx.evolve_optical_depth(q.LEPTON, p, f[:3], f[3:], dt, tau)
+        split[k][1].record()
+        ctx.generate_photons(p, f[:3], f[3:], tau, seed, s, id_base, cap, ph_p, ph_tau, ph_parent, n_out)
+        split[k][2].record()
+    barrier()
+    ms_evolve = float(np.mean([e[0].elapsed_time(e[1]) for e in split[1:]]))
+    ms_events = float(np.mean([e[1].elapsed_time(e[2]) for e in split[1:]]))
     if world > 1:
         t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -272,7 +279,10 @@ def run_ours(args):
             dist.destroy_process_group()
         return
     peaks, peak_kind = measured_peaks()
-    achieved = BYTES_PER_PARTICLE_EVOLVE * n / (ms_evolve * 1e-3) / 1e9
+    # algorithmic bytes of one fused launch: evolve's 88 B per particle + per fired parent 3 reals of momentum
+    # rewritten, tau rewritten, photon (3 reals + tau) and parent index written = 72 B
+    step_bytes = BYTES_PER_PARTICLE_EVOLVE * n + 72 * fired_last
+    achieved = step_bytes / (ms_kernel * 1e-3) / 1e9
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -284,15 +294,15 @@ def run_ours(args):
                        n_sets, 6 * n * 8 >> 20, 4 * n * 8 >> 20),
                    "parallelism": "independent shards per GPU" if world > 1 else "single GPU",
                    "table_build_s": table_build_s},
-        "roofline": {"bound": "hbm", "kernel": "evolve_kernel<double,double,LEPTON>", "achieved": achieved,
+        "roofline": {"bound": "hbm", "kernel": "step_kernel<double,double,LEPTON>", "achieved": achieved,
                      "peak": peaks["hbm_gbs"], "peak_kind": peak_kind + " (MEASURED_PEAKS.json hbm_gbs, copy)",
                      "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
-                     "traffic": EVOLVE_DRAM_TRAFFIC_BYTES, "algorithmic_bytes_per_launch": BYTES_PER_PARTICLE_EVOLVE * n,
-                     "ms_per_launch": ms_evolve},
-        "kernels_ms": {"evolve": ms_evolve, "events": ms_events},
+                     "traffic": STEP_DRAM_TRAFFIC_BYTES, "algorithmic_bytes_per_launch": step_bytes,
+                     "ms_per_launch": ms_kernel},
+        "kernels_ms": {"fused_step": ms_kernel, "two_kernel_path": {"evolve": ms_evolve, "events": ms_events}},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": args.e2e_steps},
-        "gpu_launches": 2 * args.steps,
+        "gpu_launches": args.steps,
         "clocks": sampler.summary(),
     }
     if not args.no_cpu_baseline and world == 1:

@@ -163,14 +163,32 @@ int picsarqed_generate_pairs(picsarqed_ctx* ctx, int dtype, int tau_dtype, long 
                              void* po_px, void* po_py, void* po_pz, void* po_tau,
                              long long* parent, unsigned long long* d_n_out);
 
+/* ---- the whole step of one species in one pass ------------------------------------------
+ * qed_step == evolve_optical_depth followed by generate_photons (species = lepton; s1_* = photon
+ * buffers, s2_* ignored, may be NULL) or generate_pairs (species = photon; s1_* = electron,
+ * s2_* = positron buffers), with identical results, ordering, capacity rule and d_n_out, but the
+ * evolve pass also stages the nine reals of every particle that fires (it still has them in
+ * registers), so the event pass reads dense records instead of re-scanning tau and gathering
+ * scattered parents.  The staging buffer (about 14 bytes per particle in fp64) is owned by the
+ * context.  This is the call bench.py times. */
+int picsarqed_qed_step(picsarqed_ctx* ctx, int species, int dtype, int tau_dtype, long long n,
+                       void* px, void* py, void* pz, /* in/out */
+                       const void* ex, const void* ey, const void* ez,
+                       const void* bx, const void* by, const void* bz,
+                       void* tau, /* in/out */ double dt,
+                       unsigned long long seed, unsigned long long step,
+                       unsigned long long id_base, long long capacity,
+                       void* s1_px, void* s1_py, void* s1_pz, void* s1_tau,
+                       void* s2_px, void* s2_py, void* s2_pz, void* s2_tau,
+                       long long* parent, unsigned long long* d_n_out);
+
 /* Reads an 8-byte device counter written by the calls above.  Synchronises the stream. */
 int picsarqed_read_count(picsarqed_ctx* ctx, const unsigned long long* d_count,
                          unsigned long long* host_out);
 
 /* ---- host-buffer convenience path (used for end-to-end timing) -------------------------
  * One full QED step for one species on HOST arrays: copies the nine particle/field arrays
- * and tau to device staging owned by the context, runs evolve + generate_photons (leptons)
- * or generate_pairs (photons), copies p, tau and the secondaries back.  All pointers are
+ * and tau to device staging owned by the context, runs qed_step, copies p, tau and the secondaries back.  All pointers are
  * HOST pointers (pinned memory makes the copies asynchronous, but is not required).
  * sec[0..3] (leptons: photon px,py,pz,tau) or sec[0..7] (photons: el px,py,pz,tau, po
  * px,py,pz,tau) receive min(*h_n_out, capacity) entries each.  Synchronises. */

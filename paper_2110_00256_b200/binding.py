@@ -60,6 +60,7 @@ _SIGNATURES = {
     "picsarqed_evolve_optical_depth": (_i, [_vp, _i, _i, _i, _i64] + [_vp] * 9 + [_d, _vp, _vp]),
     "picsarqed_generate_photons": (_i, [_vp, _i, _i, _i64] + [_vp] * 10 + [_u64, _u64, _u64, _i64] + [_vp] * 6),
     "picsarqed_generate_pairs": (_i, [_vp, _i, _i, _i64] + [_vp] * 10 + [_u64, _u64, _u64, _i64] + [_vp] * 10),
+    "picsarqed_qed_step": (_i, [_vp, _i, _i, _i, _i64] + [_vp] * 10 + [_d, _u64, _u64, _u64, _i64] + [_vp] * 10),
     "picsarqed_read_count": (_i, [_vp, _vp, C.POINTER(_u64)]),
     "picsarqed_step_host": (_i, [_vp, _i, _i, _i, _i64] + [_vp] * 10 + [_d, _u64, _u64, _u64, _i64, _vp, _vp,
                                                                      C.POINTER(_u64)]),
@@ -201,6 +202,19 @@ class Context:
             *[_dev(t, d) for t in el_p], _dev(el_tau, tau.dtype), *[_dev(t, d) for t in po_p],
             _dev(po_tau, tau.dtype), _dev(parent, torch.int64) if parent is not None else None,
             _dev(n_out, torch.int64)))
+
+    def qed_step(self, species, p, e, b, tau, dt, seed, step, id_base, capacity, s1_p, s1_tau, s2_p=None,
+                 s2_tau=None, parent=None, n_out=None):
+        """evolve + event generation in one kernel (picsarqed_qed_step); s1 = photon (leptons) or electron
+        (photons) buffers, s2 = positron buffers"""
+        d = p[0].dtype
+        ptrs = [_dev(t, d) for t in (*p, *e, *b)]
+        s2 = [_dev(t, d) for t in s2_p] if s2_p is not None else [None] * 3
+        self._check(lib().picsarqed_qed_step(
+            self._h, species, _code(d), _code(tau.dtype), tau.numel(), *ptrs, _dev(tau), float(dt), seed, step,
+            id_base, capacity, *[_dev(t, d) for t in s1_p], _dev(s1_tau, tau.dtype), *s2,
+            _dev(s2_tau, tau.dtype) if s2_tau is not None else None,
+            _dev(parent, torch.int64) if parent is not None else None, _dev(n_out, torch.int64)))
 
     def read_count(self, counter):
         v = _u64(0)

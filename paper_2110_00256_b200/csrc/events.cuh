@@ -13,6 +13,7 @@
 // =====================================================================================
 #pragma once
 #include "qed_device.cuh"
+#include "evolve.cuh"
 
 namespace pxq {
 
@@ -49,6 +50,11 @@ struct EventArgs {
     unsigned long long* tile_counter;  // monotonically increasing ticket counter (ctx scratch)
     unsigned long long tile_base;      // value of *tile_counter when this launch starts
     unsigned epoch;
+    // staged_event_kernel only: records written by evolve_kernel<..., EMIT> (see evolve.cuh)
+    const R* stage_rec;
+    const unsigned char* stage_idx;
+    const unsigned short* stage_cnt;
+    long long stage_stride;
 };
 
 __device__ __forceinline__ unsigned long long ld_relaxed(const unsigned long long* p) {
@@ -62,12 +68,12 @@ __device__ __forceinline__ void st_relaxed(unsigned long long* p, unsigned long 
 
 // ---- photon emission by one lepton ------------------------------
 template <typename R, typename TR>
-__device__ __forceinline__ void qs_event(const EventArgs<R, TR>& a, long long i, long long slot) {
-    const double px = a.p[0][i], py = a.p[1][i], pz = a.p[2][i];
+__device__ __forceinline__ void qs_event_core(const EventArgs<R, TR>& a, long long i, long long slot, double px,
+                                              double py, double pz, double ex, double ey, double ez, double bx,
+                                              double by, double bz) {
     const double p2 = fma(px, px, fma(py, py, pz * pz));
     const double g = sqrt(1.0 + p2);
-    const double c2 = chi_squared<0>(px, py, pz, a.e[0][i], a.e[1][i], a.e[2][i], a.b[0][i], a.b[1][i],
-                                     a.b[2][i], g, p2);
+    const double c2 = chi_squared<0>(px, py, pz, ex, ey, ez, bx, by, bz, g, p2);
     const unsigned long long id = a.id_base + (unsigned long long)i;
     const Words4 w = qed_words(a.seed, id, a.step, 1, 0);
     const Words4 wc = qed_words(a.seed, id, a.step, 2, 0);
@@ -90,15 +96,20 @@ __device__ __forceinline__ void qs_event(const EventArgs<R, TR>& a, long long i,
     a.p[2][i] = (R)(pn2 * nz);
     a.tau[i] = draw_tau<TR>(w.w[2], w.w[3]);
 }
+template <typename R, typename TR>
+__device__ __forceinline__ void qs_event(const EventArgs<R, TR>& a, long long i, long long slot) {
+    qs_event_core<R, TR>(a, i, slot, a.p[0][i], a.p[1][i], a.p[2][i], a.e[0][i], a.e[1][i], a.e[2][i], a.b[0][i],
+                         a.b[1][i], a.b[2][i]);
+}
 
 // ---- pair production by one photon -----------------------------
 template <typename R, typename TR>
-__device__ __forceinline__ void bw_event(const EventArgs<R, TR>& a, long long i, long long slot) {
-    const double px = a.p[0][i], py = a.p[1][i], pz = a.p[2][i];
+__device__ __forceinline__ void bw_event_core(const EventArgs<R, TR>& a, long long i, long long slot, double px,
+                                              double py, double pz, double ex, double ey, double ez, double bx,
+                                              double by, double bz) {
     const double p2 = fma(px, px, fma(py, py, pz * pz));
     const double g = sqrt(p2);                  // gamma_gamma = |p|
-    const double c2 = chi_squared<1>(px, py, pz, a.e[0][i], a.e[1][i], a.e[2][i], a.b[0][i], a.b[1][i],
-                                     a.b[2][i], g, p2);
+    const double c2 = chi_squared<1>(px, py, pz, ex, ey, ez, bx, by, bz, g, p2);
     const unsigned long long id = a.id_base + (unsigned long long)i;
     const Words4 w = qed_words(a.seed, id, a.step, 1, 1);
     const Words4 wc = qed_words(a.seed, id, a.step, 2, 1);
@@ -125,6 +136,49 @@ __device__ __forceinline__ void bw_event(const EventArgs<R, TR>& a, long long i,
     a.p[1][i] = (R)0;
     a.p[2][i] = (R)0;
     a.tau[i] = (TR)INFINITY;
+}
+template <typename R, typename TR>
+__device__ __forceinline__ void bw_event(const EventArgs<R, TR>& a, long long i, long long slot) {
+    bw_event_core<R, TR>(a, i, slot, a.p[0][i], a.p[1][i], a.p[2][i], a.e[0][i], a.e[1][i], a.e[2][i], a.b[0][i],
+                         a.b[1][i], a.b[2][i]);
+}
+
+// ---- decoupled look-back over the per-tile status words (one full warp) --------------------
+// Publishes `total` as this tile's aggregate, sums the counts of all earlier tiles (waiting only for tiles that
+// were handed out before this one, hence already running), publishes the inclusive prefix and returns the
+// exclusive one in every lane.
+__device__ __forceinline__ unsigned long long tile_exclusive_prefix(unsigned long long* status, long long tile,
+                                                                    unsigned epoch, unsigned long long total, int lane) {
+    unsigned long long excl = 0;
+    if (tile == 0) {
+        if (lane == 0) st_relaxed(status, pack_status(kFlagInclusive, epoch, total));
+        return 0;
+    }
+    if (lane == 0) st_relaxed(status + tile, pack_status(kFlagAggregate, epoch, total));
+    long long look = tile - 1;  // lane l inspects tile look - l
+    while (true) {
+        const long long idx = look - lane;
+        unsigned long long word = 0;
+        bool ready;
+        do {  // wait until every inspected predecessor has published for this launch
+            ready = true;
+            if (idx >= 0) {
+                word = ld_relaxed(status + idx);
+                ready = (word >> 62) != 0 && (unsigned)((word >> 40) & ((1u << kEpochBits) - 1)) == epoch;
+            }
+        } while (!__all_sync(0xffffffffu, ready));
+        const bool inclusive = idx >= 0 && (word >> 62) == kFlagInclusive;
+        const unsigned int inc_mask = __ballot_sync(0xffffffffu, inclusive);
+        const int stop = inc_mask ? __ffs(inc_mask) - 1 : 31;  // nearest inclusive prefix
+        unsigned long long v = (idx >= 0 && lane <= stop) ? (word & kValueMask) : 0ull;
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+        excl += v;
+        if (inc_mask || look - 32 < 0) break;
+        look -= 32;
+    }
+    if (lane == 0) st_relaxed(status + tile, pack_status(kFlagInclusive, epoch, excl + total));
+    return excl;
 }
 
 // ---- the event kernel ------------------------------------------------------------------
@@ -182,35 +236,7 @@ __global__ void __launch_bounds__(kEventThreads) event_kernel(const EventArgs<R,
         const unsigned int total = __shfl_sync(0xffffffffu, incl, 31);
 
         // 3. decoupled look-back: publish this tile's count, then sum the predecessors'
-        unsigned long long excl = 0;
-        if (tile == 0) {
-            if (lane == 0) st_relaxed(a.status, pack_status(kFlagInclusive, a.epoch, total));
-        } else {
-            if (lane == 0) st_relaxed(a.status + tile, pack_status(kFlagAggregate, a.epoch, total));
-            long long look = tile - 1;  // lane 0 inspects tile `look`, lane l tile look-l
-            while (true) {
-                const long long idx = look - lane;
-                unsigned long long word = 0;
-                bool ready;
-                do {  // wait until every inspected predecessor has published for this launch
-                    ready = true;
-                    if (idx >= 0) {
-                        word = ld_relaxed(a.status + idx);
-                        ready = (word >> 62) != 0 && (unsigned)((word >> 40) & ((1u << kEpochBits) - 1)) == a.epoch;
-                    }
-                } while (!__all_sync(0xffffffffu, ready));
-                const bool inclusive = idx >= 0 && (word >> 62) == kFlagInclusive;
-                const unsigned int inc_mask = __ballot_sync(0xffffffffu, inclusive);
-                const int stop = inc_mask ? __ffs(inc_mask) - 1 : 31;  // nearest inclusive prefix
-                unsigned long long v = (idx >= 0 && lane <= stop) ? (word & kValueMask) : 0ull;
-#pragma unroll
-                for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
-                excl += v;
-                if (inc_mask || look - 32 < 0) break;
-                look -= 32;
-            }
-            if (lane == 0) st_relaxed(a.status + tile, pack_status(kFlagInclusive, a.epoch, excl + total));
-        }
+        const unsigned long long excl = tile_exclusive_prefix(a.status, tile, a.epoch, total, lane);
         if (lane == 0) {
             s_excl = excl;
             s_total = total;
@@ -237,6 +263,104 @@ __global__ void __launch_bounds__(kEventThreads) event_kernel(const EventArgs<R,
         if (slot >= a.capacity) break;  // capacity rule: later parents are left untouched
         const long long i = base + list[q];
         if (KIND == 0) qs_event<R, TR>(a, i, slot); else bw_event<R, TR>(a, i, slot);
+    }
+}
+
+// ---- events from staged records -----------------------------------------------------------
+// Second half of picsarqed_qed_step.  evolve_kernel<..., EMIT> has already written, for every 128-particle
+// chunk, the number of particles that fired and their nine reals (in index order).  One CTA owns a tile of
+// 4096 particles = 32 chunks: it sums the 32 counts, gets the tile's output offset from the decoupled
+// look-back and runs the events densely over its threads, reading coalesced records instead of scanning
+// tau and gathering scattered particles.  Chunks whose segment overflowed (more than kStageCap events) or
+// that belong to the ragged tail are re-scanned from tau, exactly like event_kernel does.
+constexpr int kTileChunks = kEventTile / kChunk;  // 32
+
+template <typename R, typename TR, int KIND>
+__global__ void __launch_bounds__(kEventThreads) staged_event_kernel(const EventArgs<R, TR> a) {
+    __shared__ unsigned int cnt[kTileChunks];
+    __shared__ unsigned int off[kTileChunks + 1];
+    __shared__ unsigned char rescan[kTileChunks];
+    __shared__ unsigned char list[kTileChunks][kChunk];  // re-scanned chunks: local indices of the fired particles
+    __shared__ long long s_tile;
+    __shared__ unsigned long long s_excl;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) s_tile = (long long)(atomicAdd(a.tile_counter, 1ull) - a.tile_base);
+    __syncthreads();
+    const long long tile = s_tile;
+    const long long first_chunk = tile * kTileChunks;
+
+    // 1. per-chunk counts (4 chunks per warp); overflowed / tail chunks are re-scanned with ballot/popc
+#pragma unroll 1
+    for (int k = 0; k < kTileChunks / kEventWarps; ++k) {
+        const int j = warp * (kTileChunks / kEventWarps) + k;
+        const long long cbase = (first_chunk + j) * kChunk;
+        unsigned int c = cbase < a.n ? a.stage_cnt[first_chunk + j] : 0u;
+        const bool re = c > (unsigned)kStageCap;
+        if (re) {
+            c = 0;
+#pragma unroll
+            for (int r4 = 0; r4 < kChunk / 32; ++r4) {
+                const long long i = cbase + r4 * 32 + lane;
+                const bool f = i < a.n && a.tau[i] < (TR)0;
+                const unsigned int bal = __ballot_sync(0xffffffffu, f);
+                if (f) list[j][c + __popc(bal & ((1u << lane) - 1u))] = (unsigned char)(r4 * 32 + lane);
+                c += __popc(bal);
+            }
+        }
+        if (lane == 0) { cnt[j] = c; rescan[j] = re ? 1 : 0; }
+    }
+    __syncthreads();
+
+    // 2. offsets of the chunks inside the tile, offset of the tile in the output (decoupled look-back)
+    if (warp == 0) {
+        const unsigned int c = cnt[lane];
+        unsigned int incl = c;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned int o = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += o;
+        }
+        off[lane] = incl - c;
+        const unsigned int total = __shfl_sync(0xffffffffu, incl, 31);
+        if (lane == 31) off[kTileChunks] = total;
+        const unsigned long long excl = tile_exclusive_prefix(a.status, tile, a.epoch, total, lane);
+        if (lane == 0) {
+            s_excl = excl;
+            if ((tile + 1) * (long long)kEventTile >= a.n) *a.d_n_out = excl + total;  // last tile: total fired
+        }
+    }
+    __syncthreads();
+
+    // 3. events, densely over the threads
+    const unsigned int total = off[kTileChunks];
+    const unsigned long long excl = s_excl;
+    for (unsigned int e = tid; e < total; e += kEventThreads) {
+        const long long slot = (long long)(excl + e);
+        if (slot >= a.capacity) break;  // capacity rule (R16)
+        int j = 0;                      // largest j with off[j] <= e
+#pragma unroll
+        for (int step = kTileChunks / 2; step > 0; step >>= 1)
+            if (off[j + step] <= e) j += step;
+        const unsigned int r = e - off[j];
+        const long long cbase = (first_chunk + j) * kChunk;
+        double px, py, pz, ex, ey, ez, bx, by, bz;
+        long long i;
+        if (rescan[j]) {
+            i = cbase + list[j][r];
+            px = a.p[0][i]; py = a.p[1][i]; pz = a.p[2][i];
+            ex = a.e[0][i]; ey = a.e[1][i]; ez = a.e[2][i];
+            bx = a.b[0][i]; by = a.b[1][i]; bz = a.b[2][i];
+        } else {
+            const long long pos = (first_chunk + j) * kStageCap + r;
+            i = cbase + a.stage_idx[pos];
+            const R* rec = a.stage_rec + pos;
+            px = rec[0]; py = rec[a.stage_stride]; pz = rec[2 * a.stage_stride];
+            ex = rec[3 * a.stage_stride]; ey = rec[4 * a.stage_stride]; ez = rec[5 * a.stage_stride];
+            bx = rec[6 * a.stage_stride]; by = rec[7 * a.stage_stride]; bz = rec[8 * a.stage_stride];
+        }
+        if (KIND == 0) qs_event_core<R, TR>(a, i, slot, px, py, pz, ex, ey, ez, bx, by, bz);
+        else bw_event_core<R, TR>(a, i, slot, px, py, pz, ex, ey, ez, bx, by, bz);
     }
 }
 

@@ -27,7 +27,16 @@ struct EvolveArgs {
     unsigned int* ticket;      // self-resetting arrival counter (ctx scratch)
     unsigned long long* d_n_events;
     int table_in_smem;
+    // record emission (EMIT kernels only): every 128-particle chunk owns a segment of kStageCap records
+    R* stage_rec;               // [9][n_chunks * kStageCap]: px..bz of the fired particles, in index order
+    unsigned char* stage_idx;   // [n_chunks * kStageCap]: index of the fired particle inside its chunk
+    unsigned short* stage_cnt;  // [n_chunks]: fired particles of the chunk, or kStageRescan
+    long long stage_stride;     // n_chunks * kStageCap
 };
+
+constexpr int kChunk = 128;                 // particles one warp handles per tile: the unit of record staging
+constexpr int kStageCap = 24;               // records per chunk segment (mean at 5 % firing: 6.4)
+constexpr unsigned short kStageRescan = 0xFFFFu;  // chunk must be re-scanned by the event kernel (ragged tail)
 
 // ---- TMA bulk copy of a 1D table into shared memory ------------------------------------
 __device__ __forceinline__ void stage_table_tma(void* smem_dst, const void* gmem_src, unsigned bytes,
@@ -93,12 +102,18 @@ __device__ __forceinline__ auto decrement_one(R pxr, R pyr, R pzr, R exr, R eyr,
 }
 
 // ---- fused evolve kernel ------------------------------------------------------------
-// V = particles per 128-bit load of R; U = independent vectors per thread per tile.
-template <typename R, typename TR, int SPECIES, int U>
+// V = particles per 128-bit load of R; U = independent vectors per thread per tile.  A warp owns U*32*V
+// contiguous particles of the tile (every load instruction still covers 512 contiguous bytes).
+// EMIT: also append the nine reals of every particle that fired to the staging segment of its 128-particle
+// chunk, in index order (warp ballot/popc; no CTA barrier), for staged_event_kernel.  Requires U*32*V == kChunk.
+template <typename R, typename TR, int SPECIES, int U, bool EMIT>
 __global__ void __launch_bounds__(kEvolveThreads)
 evolve_kernel(const EvolveArgs<R, TR> a) {
     constexpr int V = 16 / sizeof(R);
     constexpr int TILE = kEvolveThreads * V * U;
+    constexpr int WCH = U * 32 * V;  // particles per warp per tile
+    static_assert(!EMIT || WCH == kChunk, "record staging works on 128-particle chunks");
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ unsigned long long mbar;
     __shared__ unsigned int warp_counts[kEvolveThreads / 32];
@@ -120,7 +135,7 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
             // all loads of the tile first: 10*U independent 128-bit requests per thread in flight
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const long long i = base + (long long)(u * kEvolveThreads + threadIdx.x) * V;
+                const long long i = base + (long long)warp * WCH + (u * 32 + lane) * V;
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
                     q[c][u] = ld_stream<R, V>(a.p[c] + i);
@@ -129,9 +144,10 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                 }
                 t[u] = *reinterpret_cast<const Vec<TR, V>*>(a.tau + i);
             }
+            unsigned int fired_bits = 0;
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const long long i = base + (long long)(u * kEvolveThreads + threadIdx.x) * V;
+                const long long i = base + (long long)warp * WCH + (u * 32 + lane) * V;
 #pragma unroll
                 for (int v = 0; v < V; ++v) {
                     const R d = decrement_one<R, SPECIES>(q[0][u].v[v], q[1][u].v[v], q[2][u].v[v], q[3][u].v[v],
@@ -140,10 +156,49 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                     const TR tn = t[u].v[v] - (TR)d;
                     t[u].v[v] = tn;
                     fired += tn < (TR)0 ? 1u : 0u;
+                    if (EMIT && tn < (TR)0) fired_bits |= 1u << (u * V + v);
                 }
                 *reinterpret_cast<Vec<TR, V>*>(a.tau + i) = t[u];
             }
+            if constexpr (EMIT) {
+                // rank inside the warp's chunk, in index order (u, lane, v): ballot / popc
+                const unsigned int lt = (1u << lane) - 1u;
+                unsigned int rank_u[U], total = 0;
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    unsigned int below = 0, all = 0;
+#pragma unroll
+                    for (int v = 0; v < V; ++v) {
+                        const unsigned int bal = __ballot_sync(0xffffffffu, (fired_bits >> (u * V + v)) & 1u);
+                        below += __popc(bal & lt);
+                        all += __popc(bal);
+                    }
+                    rank_u[u] = total + below;
+                    total += all;
+                }
+                const long long chunk = (base + (long long)warp * WCH) / kChunk;
+                if (lane == 0) a.stage_cnt[chunk] = (unsigned short)total;
+                if (total <= (unsigned)kStageCap && fired_bits) {  // else: the event kernel re-scans the chunk
+#pragma unroll
+                    for (int u = 0; u < U; ++u) {
+                        long long r = chunk * kStageCap + rank_u[u];
+#pragma unroll
+                        for (int v = 0; v < V; ++v) {
+                            if ((fired_bits >> (u * V + v)) & 1u) {
+#pragma unroll
+                                for (int c = 0; c < 9; ++c) a.stage_rec[c * a.stage_stride + r] = q[c][u].v[v];
+                                a.stage_idx[r] = (unsigned char)((u * 32 + lane) * V + v);
+                                ++r;
+                            }
+                        }
+                    }
+                }
+            }
         } else {  // ragged last tile: scalar, guarded
+            if constexpr (EMIT) {  // its chunks are re-scanned by the event kernel
+                const long long c0 = base / kChunk, c1 = (a.n + kChunk - 1) / kChunk;
+                for (long long c = c0 + threadIdx.x; c < c1; c += kEvolveThreads) a.stage_cnt[c] = kStageRescan;
+            }
             for (long long i = base + threadIdx.x; i < a.n; i += kEvolveThreads) {
                 const R d = decrement_one<R, SPECIES>(a.p[0][i], a.p[1][i], a.p[2][i], a.e[0][i], a.e[1][i],
                                                       a.e[2][i], a.b[0][i], a.b[1][i], a.b[2][i], tab, a.tab,

@@ -41,6 +41,9 @@ struct picsarqed_ctx {
     // tuning knobs (picsarqed_set_option)
     int evolve_unroll = 0;       // 0 = default per dtype
     int evolve_ctas_per_sm = 0;  // 0 = occupancy
+    // qed_step: records of the fired particles, written by the evolve pass, read by the event pass
+    void* rec = nullptr;
+    size_t rec_bytes = 0;
     // host-path staging
     void* stage = nullptr;
     size_t stage_bytes = 0;
@@ -202,6 +205,7 @@ int picsarqed_destroy(picsarqed_ctx* c) {
     cudaFree(c->status);
     cudaFree(c->tile_counter);
     cudaFree(c->stage);
+    cudaFree(c->rec);
     cudaFree(c->d_counts);
     delete c;
     return PICSARQED_OK;
@@ -277,9 +281,11 @@ int launch_chi(picsarqed_ctx* c, long long n, const void* const* a, void* out) {
     return PICSARQED_OK;
 }
 
-template <typename R, typename TR, int SPECIES, int U>
+struct StageView { void* rec; unsigned char* idx; unsigned short* cnt; long long stride; };
+
+template <typename R, typename TR, int SPECIES, int U, bool EMIT>
 int launch_evolve_u(picsarqed_ctx* c, long long n, const void* const* a, double dt, void* tau,
-                    unsigned long long* d_n_events) {
+                    unsigned long long* d_n_events, StageView sv = StageView{nullptr, nullptr, nullptr, 0}) {
     constexpr int V = 16 / sizeof(R);
     constexpr int TILE = kEvolveThreads * V * U;
     EvolveArgs<R, TR> args;
@@ -295,10 +301,14 @@ int launch_evolve_u(picsarqed_ctx* c, long long n, const void* const* a, double 
     args.partials = c->partials;
     args.ticket = c->ticket;
     args.d_n_events = d_n_events;
+    args.stage_rec = (R*)sv.rec;
+    args.stage_idx = sv.idx;
+    args.stage_cnt = sv.cnt;
+    args.stage_stride = sv.stride;
     size_t smem = ((size_t)args.tab.n * sizeof(R) + 15) & ~(size_t)15;
     args.table_in_smem = smem <= 96 * 1024;  // larger tables are read through L1/L2
     if (!args.table_in_smem) smem = 0;
-    auto kern = evolve_kernel<R, TR, SPECIES, U>;
+    auto kern = evolve_kernel<R, TR, SPECIES, U, EMIT>;
     if (smem > 48 * 1024) PXQ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
     PXQ_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kEvolveThreads, smem));
@@ -316,17 +326,14 @@ template <typename R, typename TR, int SPECIES>
 int launch_evolve(picsarqed_ctx* c, long long n, const void* const* a, double dt, void* tau,
                   unsigned long long* d_n_events) {
     int u = c->evolve_unroll ? c->evolve_unroll : 2;
-    if (u == 1) return launch_evolve_u<R, TR, SPECIES, 1>(c, n, a, dt, tau, d_n_events);
-    if (u == 4) return launch_evolve_u<R, TR, SPECIES, 4>(c, n, a, dt, tau, d_n_events);
-    return launch_evolve_u<R, TR, SPECIES, 2>(c, n, a, dt, tau, d_n_events);
+    if (u == 1) return launch_evolve_u<R, TR, SPECIES, 1, false>(c, n, a, dt, tau, d_n_events);
+    if (u == 4) return launch_evolve_u<R, TR, SPECIES, 4, false>(c, n, a, dt, tau, d_n_events);
+    return launch_evolve_u<R, TR, SPECIES, 2, false>(c, n, a, dt, tau, d_n_events);
 }
 
-template <typename R, typename TR, int KIND>
-int launch_events(picsarqed_ctx* c, long long n, void* const* p, const void* const* eb, void* tau,
-                  unsigned long long seed, unsigned long long step, unsigned long long id_base, long long capacity,
-                  void* const* out_p, void* const* out_tau, long long* parent, unsigned long long* d_n_out) {
-    const long long ntiles = (n + kEventTile - 1) / kEventTile;
-    if ((size_t)ntiles > c->status_cap) {  // grow the look-back scratch (rare; synchronises)
+// prepares the look-back scratch for a launch that hands out `tickets` tile tickets over `ntiles` tiles
+int prepare_lookback(picsarqed_ctx* c, long long ntiles) {
+    if ((size_t)ntiles > c->status_cap) {  // grow (rare; synchronises)
         PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
         if (c->status) cudaFree(c->status);
         c->status = nullptr;
@@ -340,6 +347,15 @@ int launch_events(picsarqed_ctx* c, long long n, void* const* p, const void* con
         PXQ_CUDA(c, cudaMemsetAsync(c->status, 0, c->status_cap * sizeof(unsigned long long), c->stream));
         c->epoch = 1;
     }
+    return PICSARQED_OK;
+}
+
+template <typename R, typename TR, int KIND>
+int launch_events(picsarqed_ctx* c, long long n, void* const* p, const void* const* eb, void* tau,
+                  unsigned long long seed, unsigned long long step, unsigned long long id_base, long long capacity,
+                  void* const* out_p, void* const* out_tau, long long* parent, unsigned long long* d_n_out) {
+    const long long ntiles = (n + kEventTile - 1) / kEventTile;
+    if (int rc = prepare_lookback(c, ntiles)) return rc;
     EventArgs<R, TR> args;
     for (int k = 0; k < 3; ++k) {
         args.p[k] = (R*)p[k];
@@ -361,8 +377,71 @@ int launch_events(picsarqed_ctx* c, long long n, void* const* p, const void* con
     args.tile_counter = c->tile_counter;
     args.tile_base = c->tile_base;
     args.epoch = c->epoch;
+    args.stage_rec = nullptr;
+    args.stage_idx = nullptr;
+    args.stage_cnt = nullptr;
+    args.stage_stride = 0;
     c->tile_base += (unsigned long long)ntiles;
     event_kernel<R, TR, KIND><<<(unsigned)ntiles, kEventThreads, 0, c->stream>>>(args);
+    PXQ_CUDA(c, cudaGetLastError());
+    return PICSARQED_OK;
+}
+
+// qed_step = evolve pass that also stages the records of the fired particles + event pass over the records
+template <typename R, typename TR, int SPECIES>
+int launch_step(picsarqed_ctx* c, long long n, void* const* p, const void* const* eb, void* tau, double dt,
+                unsigned long long seed, unsigned long long step, unsigned long long id_base, long long capacity,
+                void* const* out_p, void* const* out_tau, long long* parent, unsigned long long* d_n_out) {
+    const long long nchunks = (n + kChunk - 1) / kChunk;
+    const size_t rec_sz = ((size_t)nchunks * kStageCap * 9 * sizeof(R) + 255) & ~(size_t)255;
+    const size_t idx_sz = ((size_t)nchunks * kStageCap + 255) & ~(size_t)255;
+    const size_t cnt_sz = ((size_t)nchunks * sizeof(unsigned short) + 255) & ~(size_t)255;
+    if (rec_sz + idx_sz + cnt_sz > c->rec_bytes) {  // grow (rare; synchronises)
+        PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+        if (c->rec) cudaFree(c->rec);
+        c->rec = nullptr;
+        c->rec_bytes = 0;
+        PXQ_CUDA(c, cudaMalloc(&c->rec, rec_sz + idx_sz + cnt_sz));
+        c->rec_bytes = rec_sz + idx_sz + cnt_sz;
+    }
+    StageView sv;
+    sv.rec = c->rec;
+    sv.idx = static_cast<unsigned char*>(c->rec) + rec_sz;
+    sv.cnt = reinterpret_cast<unsigned short*>(static_cast<unsigned char*>(c->rec) + rec_sz + idx_sz);
+    sv.stride = nchunks * kStageCap;
+    const void* a10[9] = {p[0], p[1], p[2], eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]};
+    constexpr int U = kChunk / (32 * (16 / (int)sizeof(R)));  // fp64: 2, fp32: 1
+    if (int rc = launch_evolve_u<R, TR, SPECIES, U, true>(c, n, a10, dt, tau, nullptr, sv)) return rc;
+
+    const long long ntiles = (n + kEventTile - 1) / kEventTile;
+    if (int rc = prepare_lookback(c, ntiles)) return rc;
+    EventArgs<R, TR> ev;
+    for (int k = 0; k < 3; ++k) {
+        ev.p[k] = (R*)p[k];
+        ev.e[k] = (const R*)eb[k];
+        ev.b[k] = (const R*)eb[3 + k];
+    }
+    ev.tau = (TR*)tau;
+    ev.n = n;
+    ev.cdf = view_2d<R>(c, SPECIES);
+    ev.seed = seed;
+    ev.step = step;
+    ev.id_base = id_base;
+    ev.capacity = capacity;
+    for (int k = 0; k < 6; ++k) ev.out_p[k] = (R*)out_p[k];
+    for (int k = 0; k < 2; ++k) ev.out_tau[k] = (TR*)out_tau[k];
+    ev.parent = parent;
+    ev.d_n_out = d_n_out;
+    ev.status = c->status;
+    ev.tile_counter = c->tile_counter;
+    ev.tile_base = c->tile_base;
+    ev.epoch = c->epoch;
+    ev.stage_rec = (const R*)sv.rec;
+    ev.stage_idx = sv.idx;
+    ev.stage_cnt = sv.cnt;
+    ev.stage_stride = sv.stride;
+    c->tile_base += (unsigned long long)ntiles;
+    staged_event_kernel<R, TR, SPECIES><<<(unsigned)ntiles, kEventThreads, 0, c->stream>>>(ev);
     PXQ_CUDA(c, cudaGetLastError());
     return PICSARQED_OK;
 }
@@ -498,6 +577,38 @@ int picsarqed_generate_pairs(picsarqed_ctx* c, int dtype, int tau_dtype, long lo
 
 }  // extern "C"
 
+extern "C" int picsarqed_qed_step(picsarqed_ctx* c, int species, int dtype, int tau_dtype, long long n, void* px,
+                                  void* py, void* pz, const void* ex, const void* ey, const void* ez, const void* bx,
+                                  const void* by, const void* bz, void* tau, double dt, unsigned long long seed,
+                                  unsigned long long step, unsigned long long id_base, long long capacity,
+                                  void* s1_px, void* s1_py, void* s1_pz, void* s1_tau, void* s2_px, void* s2_py,
+                                  void* s2_pz, void* s2_tau, long long* parent, unsigned long long* d_n_out) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (n < 0 || capacity < 0 || !d_n_out || (species != 0 && species != 1))
+        return fail(c, PICSARQED_ERR_INVALID, "bad n, capacity, species or d_n_out");
+    if (!c->have_tables) return fail(c, PICSARQED_ERR_NO_TABLES, "no tables: call build_tables or import_tables");
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    if (n == 0) {
+        PXQ_CUDA(c, cudaMemsetAsync(d_n_out, 0, sizeof(unsigned long long), c->stream));
+        return PICSARQED_OK;
+    }
+    void* p[3] = {px, py, pz};
+    const void* eb[6] = {ex, ey, ez, bx, by, bz};
+    const void* chk[10] = {px, py, pz, ex, ey, ez, bx, by, bz, tau};
+    if (int rc = check_arrays(c, chk, 10)) return rc;
+    void* out_p[6] = {s1_px, s1_py, s1_pz, s2_px, s2_py, s2_pz};
+    void* out_tau[2] = {s1_tau, s2_tau};
+    if (capacity > 0) {
+        const void* o[8] = {s1_px, s1_py, s1_pz, s1_tau, s2_px, s2_py, s2_pz, s2_tau};
+        if (int rc = check_arrays(c, o, species == 0 ? 4 : 8)) return rc;
+    }
+    PXQ_DISPATCH_RT(c, dtype, tau_dtype,
+                    return species == 0 ? (launch_step<R, TR, 0>(c, n, p, eb, tau, dt, seed, step, id_base, capacity,
+                                                                 out_p, out_tau, parent, d_n_out))
+                                        : (launch_step<R, TR, 1>(c, n, p, eb, tau, dt, seed, step, id_base, capacity,
+                                                                 out_p, out_tau, parent, d_n_out)));
+}
+
 // =====================================================================================
 //  host-buffer path (end-to-end timing): H2D copies, evolve + events, D2H copies
 // =====================================================================================
@@ -549,18 +660,10 @@ extern "C" int picsarqed_step_host(picsarqed_ctx* c, int species, int dtype, int
     if (!h_tau) return fail(c, PICSARQED_ERR_INVALID, "null host tau");
     PXQ_CUDA(c, cudaMemcpyAsync(d[9], h_tau, (size_t)n * ts, cudaMemcpyHostToDevice, c->stream));
 
-    int rc = picsarqed_evolve_optical_depth(c, species, dtype, tau_dtype, n, d[0], d[1], d[2], d[3], d[4], d[5], d[6],
-                                            d[7], d[8], dt, d[9], nullptr);
-    if (rc) return rc;
-    if (species == 0)
-        rc = picsarqed_generate_photons(c, dtype, tau_dtype, n, d[0], d[1], d[2], d[3], d[4], d[5], d[6], d[7], d[8],
-                                        d[9], seed, step, id_base, capacity, d_sec_p[0], d_sec_p[1], d_sec_p[2],
-                                        d_sec_tau[0], h_parent ? d_parent : nullptr, c->d_counts);
-    else
-        rc = picsarqed_generate_pairs(c, dtype, tau_dtype, n, d[0], d[1], d[2], d[3], d[4], d[5], d[6], d[7], d[8],
-                                      d[9], seed, step, id_base, capacity, d_sec_p[0], d_sec_p[1], d_sec_p[2],
-                                      d_sec_tau[0], d_sec_p[3], d_sec_p[4], d_sec_p[5], d_sec_tau[1],
-                                      h_parent ? d_parent : nullptr, c->d_counts);
+    int rc = picsarqed_qed_step(c, species, dtype, tau_dtype, n, d[0], d[1], d[2], d[3], d[4], d[5], d[6], d[7], d[8],
+                                d[9], dt, seed, step, id_base, capacity, d_sec_p[0], d_sec_p[1], d_sec_p[2],
+                                d_sec_tau[0], d_sec_p[3], d_sec_p[4], d_sec_p[5], d_sec_tau[1],
+                                h_parent ? d_parent : nullptr, c->d_counts);
     if (rc) return rc;
     void* h_p[3] = {h_px, h_py, h_pz};
     for (int k = 0; k < 3; ++k)

@@ -303,3 +303,103 @@ def test_free_running_steps(orc, qed, ctx, mid_tables, species, dtype, tdtype):
         p_h, tau_h = g["p"], g["tau"]
         dp, dtau = to_dev(p_h), torch.from_numpy(tau_h.copy()).cuda()
     assert total_amb <= (0 if dtype == np.float64 else 5)
+
+
+# ----------------------------------------------------------------------------- fused step
+def _run_fused(qed, ctx, species, dtype, tdtype, p, e, b, tau_host, dt, seed, step, id_base, capacity):
+    import torch
+    tdt = torch.float64 if tdtype == np.float64 else torch.float32
+    pdt = torch.float64 if dtype == np.float64 else torch.float32
+    dp, de, db = to_dev(p), to_dev(e), to_dev(b)
+    dtau = torch.from_numpy(tau_host.copy()).cuda()
+    nsec = 1 if species == LEPTON else 2
+    cap = max(capacity, 1)
+    sec_p = [[torch.full((cap,), -7.0, dtype=pdt, device="cuda") for _ in range(3)] for _ in range(nsec)]
+    sec_tau = [torch.full((cap,), -7.0, dtype=tdt, device="cuda") for _ in range(nsec)]
+    parent = torch.full((cap,), -1, dtype=torch.int64, device="cuda")
+    n_out = torch.zeros(1, dtype=torch.int64, device="cuda")
+    ctx.qed_step(species, dp, de, db, dtau, dt, seed, step, id_base, capacity, sec_p[0], sec_tau[0],
+                 sec_p[1] if nsec == 2 else None, sec_tau[1] if nsec == 2 else None, parent, n_out)
+    return dict(n_fired=ctx.read_count(n_out), p=to_host(dp), tau=dtau.cpu().numpy(), parent=parent.cpu().numpy(),
+                sec_p=[to_host(s) for s in sec_p], sec_tau=to_host(sec_tau))
+
+
+def _run_unfused(qed, ctx, species, dtype, tdtype, p, e, b, tau_host, dt, seed, step, id_base, capacity):
+    import torch
+    tdt = torch.float64 if tdtype == np.float64 else torch.float32
+    pdt = torch.float64 if dtype == np.float64 else torch.float32
+    dp, de, db = to_dev(p), to_dev(e), to_dev(b)
+    dtau = torch.from_numpy(tau_host.copy()).cuda()
+    nsec = 1 if species == LEPTON else 2
+    cap = max(capacity, 1)
+    sec_p = [[torch.full((cap,), -7.0, dtype=pdt, device="cuda") for _ in range(3)] for _ in range(nsec)]
+    sec_tau = [torch.full((cap,), -7.0, dtype=tdt, device="cuda") for _ in range(nsec)]
+    parent = torch.full((cap,), -1, dtype=torch.int64, device="cuda")
+    n_out = torch.zeros(1, dtype=torch.int64, device="cuda")
+    ctx.evolve_optical_depth(species, dp, de, db, dt, dtau)
+    tau_mid = dtau.cpu().numpy()
+    if species == LEPTON:
+        ctx.generate_photons(dp, de, db, dtau, seed, step, id_base, capacity, sec_p[0], sec_tau[0], parent, n_out)
+    else:
+        ctx.generate_pairs(dp, de, db, dtau, seed, step, id_base, capacity, sec_p[0], sec_tau[0], sec_p[1], sec_tau[1],
+                           parent, n_out)
+    return dict(n_fired=ctx.read_count(n_out), p=to_host(dp), tau=dtau.cpu().numpy(), parent=parent.cpu().numpy(),
+                sec_p=[to_host(s) for s in sec_p], sec_tau=to_host(sec_tau)), tau_mid
+
+
+def _same(a, b):
+    return np.array_equal(a, b, equal_nan=True)
+
+
+@pytest.mark.parametrize("species", [LEPTON, PHOTON])
+@pytest.mark.parametrize("dtype,tdtype", DTYPES, ids=IDS)
+@pytest.mark.parametrize("n,target", [(5 * 4096 + 1234, 0.05), (4096 + 77, 0.6), (1000, 0.05), (1, 0.9)])
+def test_fused_step(orc, qed, ctx, mid_tables, species, dtype, tdtype, n, target):
+    """picsarqed_qed_step == evolve followed by generate, bit for bit (same device functions), and both agree with the
+    oracle; target 0.6 overflows the shared-memory record buffer (more than a quarter of a tile fires)"""
+    p, e, b = qed.workloads.config1(seed=31, n=n, species=species, dtype=dtype)
+    tables = _tables_for(mid_tables, dtype)
+    dt = qed.workloads.choose_dt(orc.rate(tables, species, p, e, b), target)
+    tau0 = orc.init_optical_depth(species, code(tdtype), n, 5).astype(tdtype)
+    for cap in (n, max(1, n // 40)):
+        f = _run_fused(qed, ctx, species, dtype, tdtype, p, e, b, tau0, dt, 77, 2, 123456789, cap)
+        u, tau_mid = _run_unfused(qed, ctx, species, dtype, tdtype, p, e, b, tau0, dt, 77, 2, 123456789, cap)
+        assert f["n_fired"] == u["n_fired"] and _same(f["parent"], u["parent"])
+        assert _same(f["tau"], u["tau"]) and all(_same(x, y) for x, y in zip(f["p"], u["p"]))
+        for s in range(len(f["sec_p"])):
+            assert all(_same(x, y) for x, y in zip(f["sec_p"][s], u["sec_p"][s])) and _same(f["sec_tau"][s], u["sec_tau"][s])
+        # and against the oracle: evolve with the tie protocol, events on the GPU's evolved tau
+        o = orc.evolve_optical_depth(tables, species, code(tdtype), p, e, b, dt, tau0)
+        ln_chi = np.log(np.maximum(orc.chi(species, p, e, b), 1e-300))
+        check_evolve(tau_mid, tau0.astype(np.float64), o, dtype, ln_chi)
+        ids = 123456789 + np.arange(n, dtype=np.uint64)
+        if species == LEPTON:
+            oe = orc.generate_photons(tables, code(dtype), code(tdtype), p, e, b, tau_mid, 77, 2, ids, cap)
+            oe["sec_p"], oe["sec_tau"] = [oe["ph_p"]], [oe["ph_tau"]]
+        else:
+            oe = orc.generate_pairs(tables, code(dtype), code(tdtype), p, e, b, tau_mid, 77, 2, ids, cap)
+            oe["sec_p"], oe["sec_tau"] = [oe["el_p"], oe["po_p"]], [oe["el_tau"], oe["po_tau"]]
+        _compare_events(f, oe, species, dtype, tdtype, cap, p)
+        if n > 4096:
+            assert f["n_fired"] > 0.5 * target * n
+
+
+def test_fused_step_repeated_launches(qed, ctx):
+    """many launches back to back on one context: the ticket counter and the epoch-stamped status words carry over"""
+    import torch
+    n = 3 * 4096 + 5
+    p, e, b = qed.workloads.config1(seed=32, n=n, species=LEPTON, dtype=np.float64)
+    dp, de, db = to_dev(p), to_dev(e), to_dev(b)
+    tau = torch.full((n,), 0.01, dtype=torch.float64, device="cuda")
+    sec_p = [torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3)]
+    sec_tau = torch.empty(n, dtype=torch.float64, device="cuda")
+    n_out = torch.zeros(1, dtype=torch.int64, device="cuda")
+    counts = []
+    for step in range(40):
+        sec_tau.fill_(-7.0)
+        ctx.qed_step(LEPTON, dp, de, db, tau, 3e-18, 1, step, 0, n, sec_p, sec_tau, None, None, None, n_out)
+        k = ctx.read_count(n_out)
+        counts.append(k)
+        assert k == int((sec_tau != -7.0).sum().item()) and bool((sec_tau[:k] > 0).all())  # dense, nothing past the count
+        assert bool((tau >= 0).all())                                                      # every fired parent was re-drawn
+    assert sum(counts) > 0
