@@ -5,32 +5,23 @@
 //  (eqs.24-26), creation of the secondaries in ascending parent index,
 //  and the re-draw tau = -ln U.
 //
-//  One kernel, one pass over tau.  Per tile of 4096 particles: warp ballot/popc gives every
-//  fired particle its rank inside its warp, a CTA-level scan of the 128 warp counts gives
-//  the rank inside the tile, and a decoupled look-back over per-tile status words gives the
-//  tile's offset in the output.  The fired particles of a tile are then gathered into a
-//  dense list in shared memory so that full warps run the (branchy) binary search.
+//  Compaction in three levels, all deterministic:
+//   1. warp ballot/popc ranks the fired particles of a 128-particle chunk and counts them
+//      (inside the evolve pass for picsarqed_qed_step, count_chunks_kernel for generate_*);
+//   2. tile_sums_kernel + tile_scan_kernel: the chunk counts are summed per tile and one CTA
+//      scans the tile sums (block-level scan) into exclusive output offsets and the total;
+//   3. event_kernel: a tile of consecutive chunks per CTA; event e of the tile is handled by
+//      thread e, its output slot is tile_offset + e.  Tiles are independent: no
+//      ticket, no look-back, no barrier on the common path.
+//  (A single-pass decoupled look-back was tried first: with ~10^3 tiles in flight every tile
+//  walks ~30 status windows before it meets an inclusive prefix, which serialised the kernel
+//  at ~0.3 ms per 16 Mi particles whatever its shape -- profiles/r1_events_full.md.)
 // =====================================================================================
 #pragma once
 #include "qed_device.cuh"
 #include "evolve.cuh"
 
 namespace pxq {
-
-constexpr int kEventThreads = 256;
-constexpr int kEventItems = 16;
-constexpr int kEventTile = kEventThreads * kEventItems;  // 4096 particles
-constexpr int kEventWarps = kEventThreads / 32;
-constexpr int kEventChunks = kEventItems * kEventWarps;  // 128 (round, warp) chunks per tile
-
-// look-back status word: [63:62] flag, [61:40] launch epoch, [39:0] count
-constexpr unsigned long long kFlagAggregate = 1ull, kFlagInclusive = 2ull;
-constexpr int kEpochBits = 22;
-constexpr unsigned long long kValueMask = (1ull << 40) - 1;
-__device__ __forceinline__ unsigned long long pack_status(unsigned long long flag, unsigned epoch,
-                                                          unsigned long long value) {
-    return (flag << 62) | ((unsigned long long)epoch << 40) | (value & kValueMask);
-}
 
 template <typename R, typename TR>
 struct EventArgs {
@@ -45,32 +36,25 @@ struct EventArgs {
     R* out_p[6];      // QS: photon px,py,pz (0..2).  BW: electron (0..2), positron (3..5)
     TR* out_tau[2];   // QS: photon tau.            BW: electron, positron tau
     long long* parent;
-    unsigned long long* d_n_out;
-    unsigned long long* status;        // one word per tile (ctx scratch)
-    unsigned long long* tile_counter;  // monotonically increasing ticket counter (ctx scratch)
-    unsigned long long tile_base;      // value of *tile_counter when this launch starts
-    unsigned epoch;
-    // staged_event_kernel only: records written by evolve_kernel<..., EMIT> (see evolve.cuh)
-    const R* stage_rec;
-    const unsigned char* stage_idx;
-    const unsigned short* stage_cnt;
-    long long stage_stride;
+    // per 128-particle chunk (context scratch, see evolve.cuh):
+    const unsigned char* stage_rec;           // staged records (unused for chunks flagged kStageNoRecords)
+    const unsigned short* stage_cnt;          // count | flags
+    const unsigned long long* tile_offset;    // [n_tiles] number of events before the tile
 };
 
-__device__ __forceinline__ unsigned long long ld_relaxed(const unsigned long long* p) {
-    unsigned long long v;
-    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void st_relaxed(unsigned long long* p, unsigned long long v) {
-    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
+template <typename R, typename TR>
+struct EventOut {
+    R sec[6];     // QS: photon momentum (0..2).  BW: electron (0..2) and positron (3..5) momenta
+    TR sec_tau[2];
+    R parent_p[3];
+    TR parent_tau;
+};
 
 // ---- photon emission by one lepton ------------------------------
 template <typename R, typename TR>
-__device__ __forceinline__ void qs_event_core(const EventArgs<R, TR>& a, long long i, long long slot, double px,
-                                              double py, double pz, double ex, double ey, double ez, double bx,
-                                              double by, double bz) {
+__device__ __forceinline__ EventOut<R, TR> qs_event_compute(const EventArgs<R, TR>& a, long long i, double px, double py,
+                                                            double pz, double ex, double ey, double ez, double bx,
+                                                            double by, double bz) {
     const double p2 = fma(px, px, fma(py, py, pz * pz));
     const double g = sqrt(1.0 + p2);
     const double c2 = chi_squared<0>(px, py, pz, ex, ey, ez, bx, by, bz, g, p2);
@@ -86,27 +70,25 @@ __device__ __forceinline__ void qs_event_core(const EventArgs<R, TR>& a, long lo
     const double gph = km1 * xi;                // gamma_gamma = (gamma-1) xi
     const double k2 = km1 * (1.0 - xi);         // emitter kinetic energy after the emission
     const double pn2 = sqrt(k2 * (k2 + 2.0));   // sqrt(gamma'^2 - 1)
-    a.out_p[0][slot] = (R)(gph * nx);           // emitted along p
-    a.out_p[1][slot] = (R)(gph * ny);
-    a.out_p[2][slot] = (R)(gph * nz);
-    a.out_tau[0][slot] = draw_tau<TR>(wc.w[0], wc.w[1]);
-    if (a.parent) a.parent[slot] = i;
-    a.p[0][i] = (R)(pn2 * nx);
-    a.p[1][i] = (R)(pn2 * ny);
-    a.p[2][i] = (R)(pn2 * nz);
-    a.tau[i] = draw_tau<TR>(w.w[2], w.w[3]);
-}
-template <typename R, typename TR>
-__device__ __forceinline__ void qs_event(const EventArgs<R, TR>& a, long long i, long long slot) {
-    qs_event_core<R, TR>(a, i, slot, a.p[0][i], a.p[1][i], a.p[2][i], a.e[0][i], a.e[1][i], a.e[2][i], a.b[0][i],
-                         a.b[1][i], a.b[2][i]);
+    EventOut<R, TR> o;
+    o.sec[0] = (R)(gph * nx);                   // emitted along p
+    o.sec[1] = (R)(gph * ny);
+    o.sec[2] = (R)(gph * nz);
+    o.sec[3] = o.sec[4] = o.sec[5] = (R)0;
+    o.sec_tau[0] = draw_tau<TR>(wc.w[0], wc.w[1]);
+    o.sec_tau[1] = (TR)0;
+    o.parent_p[0] = (R)(pn2 * nx);
+    o.parent_p[1] = (R)(pn2 * ny);
+    o.parent_p[2] = (R)(pn2 * nz);
+    o.parent_tau = draw_tau<TR>(w.w[2], w.w[3]);
+    return o;
 }
 
 // ---- pair production by one photon -----------------------------
 template <typename R, typename TR>
-__device__ __forceinline__ void bw_event_core(const EventArgs<R, TR>& a, long long i, long long slot, double px,
-                                              double py, double pz, double ex, double ey, double ez, double bx,
-                                              double by, double bz) {
+__device__ __forceinline__ EventOut<R, TR> bw_event_compute(const EventArgs<R, TR>& a, long long i, double px, double py,
+                                                            double pz, double ex, double ey, double ez, double bx,
+                                                            double by, double bz) {
     const double p2 = fma(px, px, fma(py, py, pz * pz));
     const double g = sqrt(p2);                  // gamma_gamma = |p|
     const double c2 = chi_squared<1>(px, py, pz, ex, ey, ez, bx, by, bz, g, p2);
@@ -123,244 +105,205 @@ __device__ __forceinline__ void bw_event_core(const EventArgs<R, TR>& a, long lo
     const double pe = sqrt(ke * (ke + 2.0)), pp = sqrt(kp * (kp + 2.0));
     const double inv_g = g > 0.0 ? 1.0 / g : 0.0;
     const double nx = px * inv_g, ny = py * inv_g, nz = pz * inv_g;
-    a.out_p[0][slot] = (R)(pe * nx);
-    a.out_p[1][slot] = (R)(pe * ny);
-    a.out_p[2][slot] = (R)(pe * nz);
-    a.out_p[3][slot] = (R)(pp * nx);
-    a.out_p[4][slot] = (R)(pp * ny);
-    a.out_p[5][slot] = (R)(pp * nz);
-    a.out_tau[0][slot] = draw_tau<TR>(wc.w[0], wc.w[1]);
-    a.out_tau[1][slot] = draw_tau<TR>(wc.w[2], wc.w[3]);
-    if (a.parent) a.parent[slot] = i;
-    a.p[0][i] = (R)0;                           // photon removed: p = 0, tau = +inf
-    a.p[1][i] = (R)0;
-    a.p[2][i] = (R)0;
-    a.tau[i] = (TR)INFINITY;
-}
-template <typename R, typename TR>
-__device__ __forceinline__ void bw_event(const EventArgs<R, TR>& a, long long i, long long slot) {
-    bw_event_core<R, TR>(a, i, slot, a.p[0][i], a.p[1][i], a.p[2][i], a.e[0][i], a.e[1][i], a.e[2][i], a.b[0][i],
-                         a.b[1][i], a.b[2][i]);
+    EventOut<R, TR> o;
+    o.sec[0] = (R)(pe * nx);
+    o.sec[1] = (R)(pe * ny);
+    o.sec[2] = (R)(pe * nz);
+    o.sec[3] = (R)(pp * nx);
+    o.sec[4] = (R)(pp * ny);
+    o.sec[5] = (R)(pp * nz);
+    o.sec_tau[0] = draw_tau<TR>(wc.w[0], wc.w[1]);
+    o.sec_tau[1] = draw_tau<TR>(wc.w[2], wc.w[3]);
+    o.parent_p[0] = o.parent_p[1] = o.parent_p[2] = (R)0;   // photon removed: p = 0, tau = +inf
+    o.parent_tau = (TR)INFINITY;
+    return o;
 }
 
-// ---- decoupled look-back over the per-tile status words (one full warp) --------------------
-// Publishes `total` as this tile's aggregate, sums the counts of all earlier tiles (waiting only for tiles that
-// were handed out before this one, hence already running), publishes the inclusive prefix and returns the
-// exclusive one in every lane.
-__device__ __forceinline__ unsigned long long tile_exclusive_prefix(unsigned long long* status, long long tile,
-                                                                    unsigned epoch, unsigned long long total, int lane) {
-    unsigned long long excl = 0;
-    if (tile == 0) {
-        if (lane == 0) st_relaxed(status, pack_status(kFlagInclusive, epoch, total));
-        return 0;
-    }
-    if (lane == 0) st_relaxed(status + tile, pack_status(kFlagAggregate, epoch, total));
-    long long look = tile - 1;  // lane l inspects tile look - l
-    while (true) {
-        const long long idx = look - lane;
-        unsigned long long word = 0;
-        bool ready;
-        do {  // wait until every inspected predecessor has published for this launch
-            ready = true;
-            if (idx >= 0) {
-                word = ld_relaxed(status + idx);
-                ready = (word >> 62) != 0 && (unsigned)((word >> 40) & ((1u << kEpochBits) - 1)) == epoch;
-            }
-        } while (!__all_sync(0xffffffffu, ready));
-        const bool inclusive = idx >= 0 && (word >> 62) == kFlagInclusive;
-        const unsigned int inc_mask = __ballot_sync(0xffffffffu, inclusive);
-        const int stop = inc_mask ? __ffs(inc_mask) - 1 : 31;  // nearest inclusive prefix
-        unsigned long long v = (idx >= 0 && lane <= stop) ? (word & kValueMask) : 0ull;
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
-        excl += v;
-        if (inc_mask || look - 32 < 0) break;
-        look -= 32;
-    }
-    if (lane == 0) st_relaxed(status + tile, pack_status(kFlagInclusive, epoch, excl + total));
-    return excl;
-}
-
-// ---- the event kernel ------------------------------------------------------------------
-// KIND 0: photon emission by leptons; KIND 1: pair production by photons.
 template <typename R, typename TR, int KIND>
-__global__ void __launch_bounds__(kEventThreads) event_kernel(const EventArgs<R, TR> a) {
-    __shared__ unsigned int chunk_off[kEventChunks];   // counts, then exclusive offsets, in (round, warp) order
-    __shared__ unsigned short list[kEventTile];        // tile-local indices of the fired particles, ascending
-    __shared__ long long s_tile;
-    __shared__ unsigned long long s_excl;               // number of fired particles in all earlier tiles
-    __shared__ unsigned int s_total;
+__device__ __forceinline__ void event_commit(const EventArgs<R, TR>& a, long long i, long long slot,
+                                             const EventOut<R, TR>& o) {
+#pragma unroll
+    for (int c = 0; c < (KIND == 0 ? 3 : 6); ++c) a.out_p[c][slot] = o.sec[c];
+    a.out_tau[0][slot] = o.sec_tau[0];
+    if (KIND == 1) a.out_tau[1][slot] = o.sec_tau[1];
+    if (a.parent) a.parent[slot] = i;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) a.p[c][i] = o.parent_p[c];
+    a.tau[i] = o.parent_tau;
+}
 
+// ---- level 1 for generate_*: count the fired particles of every chunk --------------------------
+// one warp per chunk: tau < 0 (R1) -> ballot/popc.  No records are staged on this path.
+template <typename TR>
+__global__ void __launch_bounds__(256) count_chunks_kernel(const TR* __restrict__ tau, long long n, long long n_chunks,
+                                                           unsigned short* __restrict__ cnt) {
+    const int lane = threadIdx.x & 31;
+    const long long warps = (long long)gridDim.x * (blockDim.x / 32);
+    for (long long ch = (long long)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); ch < n_chunks; ch += warps) {
+        unsigned int k = 0;
+#pragma unroll
+        for (int r4 = 0; r4 < kChunk / 32; ++r4) {
+            const long long i = ch * kChunk + r4 * 32 + lane;
+            const bool f = i < n && tau[i] < (TR)0;
+            k += __popc(__ballot_sync(0xffffffffu, f));
+        }
+        if (lane == 0) cnt[ch] = (unsigned short)(k | kStageNoRecords);
+    }
+}
+
+// ---- level 2: output offsets of the tiles (block-level scan) -------------------------------------
+// tile_sums_kernel: one warp per tile of `chunks_per_tile` chunks (<= 32): lane j reads the count of chunk j
+// (coalesced), chunks not counted yet (ragged tail of the evolve pass) are counted from tau and fixed up in
+// place, a warp reduction gives the tile's number of events.
+template <typename TR>
+__global__ void __launch_bounds__(256) tile_sums_kernel(unsigned short* __restrict__ cnt, long long n_chunks,
+                                                        int chunks_per_tile, long long n_tiles,
+                                                        const TR* __restrict__ tau, long long n,
+                                                        unsigned int* __restrict__ tile_sum) {
+    const int lane = threadIdx.x & 31;
+    const long long warps = (long long)gridDim.x * (blockDim.x / 32);
+    for (long long t = (long long)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); t < n_tiles; t += warps) {
+        const long long ch = t * chunks_per_tile + lane;
+        const bool real = lane < chunks_per_tile && ch < n_chunks;
+        unsigned int c = real ? cnt[ch] : 0u;
+        unsigned int unknown = __ballot_sync(0xffffffffu, real && c == kStageUnknown);
+        while (unknown) {  // rare: count the chunk from tau (tau < 0, R1), the whole warp on one chunk
+            const int j = __ffs(unknown) - 1;
+            unknown &= unknown - 1;
+            const long long cb = (t * chunks_per_tile + j) * kChunk;
+            unsigned int k = 0;
+#pragma unroll
+            for (int r4 = 0; r4 < kChunk / 32; ++r4) {
+                const long long i = cb + r4 * 32 + lane;
+                k += __popc(__ballot_sync(0xffffffffu, i < n && tau[i] < (TR)0));
+            }
+            if (lane == j) {
+                c = k | kStageNoRecords;
+                cnt[ch] = (unsigned short)c;
+            }
+        }
+        unsigned int s = c & kStageCountMask;
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+        if (lane == 0) tile_sum[t] = s;
+    }
+}
+
+// tile_scan_kernel: one CTA scans the tile sums, 1024 at a time (coalesced), carrying the running total;
+// tile_offset[t] = number of events before tile t, *d_total = number of events.
+constexpr int kScanThreads = 1024;
+
+__global__ void __launch_bounds__(kScanThreads) tile_scan_kernel(const unsigned int* __restrict__ tile_sum, long long n_tiles,
+                                                                 unsigned long long* __restrict__ tile_offset,
+                                                                 unsigned long long* __restrict__ d_total) {
+    __shared__ unsigned long long warp_sum[kScanThreads / 32];
+    __shared__ unsigned long long s_carry;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    // tiles are handed out in launch order, so every tile's predecessors are already running
-    if (tid == 0) s_tile = (long long)(atomicAdd(a.tile_counter, 1ull) - a.tile_base);
+    if (tid == 0) s_carry = 0;
     __syncthreads();
-    const long long tile = s_tile;
-    const long long base = tile * kEventTile;
-
-    // 1. flags: tau < 0 (R1).  All loads first.
-    TR t[kEventItems];
-#pragma unroll
-    for (int j = 0; j < kEventItems; ++j) {
-        const long long i = base + j * kEventThreads + tid;
-        t[j] = i < a.n ? a.tau[i] : (TR)1;
-    }
-    unsigned int my_flags = 0;
-    unsigned int my_rank[kEventItems / 4];  // 8-bit lane ranks (< 32), packed
-#pragma unroll
-    for (int j = 0; j < kEventItems / 4; ++j) my_rank[j] = 0;
-#pragma unroll
-    for (int j = 0; j < kEventItems; ++j) {
-        const bool f = t[j] < (TR)0;
-        const unsigned int bal = __ballot_sync(0xffffffffu, f);
-        if (f) my_flags |= 1u << j;
-        my_rank[j >> 2] |= (unsigned)__popc(bal & ((1u << lane) - 1u)) << (8 * (j & 3));
-        if (lane == 0) chunk_off[j * kEventWarps + warp] = __popc(bal);
-    }
-    __syncthreads();
-
-    // 2. CTA scan of the 128 chunk counts (warp 0: 4 per lane + shuffle scan)
-    if (warp == 0) {
-        unsigned int c[4], s = 0;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) { c[k] = chunk_off[4 * lane + k]; s += c[k]; }
-        unsigned int incl = s;
+    for (long long base = 0; base < n_tiles; base += kScanThreads) {
+        const long long t = base + tid;
+        const unsigned long long v = t < n_tiles ? tile_sum[t] : 0ull;
+        unsigned long long incl = v;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
-            const unsigned int o = __shfl_up_sync(0xffffffffu, incl, d);
+            const unsigned long long o = __shfl_up_sync(0xffffffffu, incl, d);
             if (lane >= d) incl += o;
         }
-        unsigned int run = incl - s;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) { chunk_off[4 * lane + k] = run; run += c[k]; }
-        const unsigned int total = __shfl_sync(0xffffffffu, incl, 31);
-
-        // 3. decoupled look-back: publish this tile's count, then sum the predecessors'
-        const unsigned long long excl = tile_exclusive_prefix(a.status, tile, a.epoch, total, lane);
-        if (lane == 0) {
-            s_excl = excl;
-            s_total = total;
-            if (base + kEventTile >= a.n) *a.d_n_out = excl + total;  // last tile: total fired
-        }
+        if (lane == 31) warp_sum[warp] = incl;
+        __syncthreads();
+        unsigned long long before = s_carry;
+        for (int w = 0; w < warp; ++w) before += warp_sum[w];
+        if (t < n_tiles) tile_offset[t] = before + incl - v;
+        __syncthreads();
+        if (tid == kScanThreads - 1) s_carry = before + incl;
+        __syncthreads();
     }
-    __syncthreads();
-
-    // 4. gather the fired particles of the tile into a dense, index-ordered list
-#pragma unroll
-    for (int j = 0; j < kEventItems; ++j) {
-        if (my_flags & (1u << j)) {
-            const unsigned int rank = (my_rank[j >> 2] >> (8 * (j & 3))) & 0xffu;
-            list[chunk_off[j * kEventWarps + warp] + rank] = (unsigned short)(j * kEventThreads + tid);
-        }
-    }
-    __syncthreads();
-
-    // 5. events, densely packed over the threads; slot = number of fired particles before this one
-    const unsigned int total = s_total;
-    const unsigned long long excl = s_excl;
-    for (unsigned int q = tid; q < total; q += kEventThreads) {
-        const long long slot = (long long)(excl + q);
-        if (slot >= a.capacity) break;  // capacity rule: later parents are left untouched
-        const long long i = base + list[q];
-        if (KIND == 0) qs_event<R, TR>(a, i, slot); else bw_event<R, TR>(a, i, slot);
-    }
+    if (tid == 0) *d_total = s_carry;
 }
 
-// ---- events from staged records -----------------------------------------------------------
-// Second half of picsarqed_qed_step.  evolve_kernel<..., EMIT> has already written, for every 128-particle
-// chunk, the number of particles that fired and their nine reals (in index order).  One CTA owns a tile of
-// 4096 particles = 32 chunks: it sums the 32 counts, gets the tile's output offset from the decoupled
-// look-back and runs the events densely over its threads, reading coalesced records instead of scanning
-// tau and gathering scattered particles.  Chunks whose segment overflowed (more than kStageCap events) or
-// that belong to the ragged tail are re-scanned from tau, exactly like event_kernel does.
-constexpr int kTileChunks = kEventTile / kChunk;  // 32
-
-template <typename R, typename TR, int KIND>
-__global__ void __launch_bounds__(kEventThreads) staged_event_kernel(const EventArgs<R, TR> a) {
-    __shared__ unsigned int cnt[kTileChunks];
-    __shared__ unsigned int off[kTileChunks + 1];
-    __shared__ unsigned char rescan[kTileChunks];
-    __shared__ unsigned char list[kTileChunks][kChunk];  // re-scanned chunks: local indices of the fired particles
-    __shared__ long long s_tile;
-    __shared__ unsigned long long s_excl;
+// ---- level 3: the events ---------------------------------------------------------------------
+// THREADS threads own a tile of CHUNKS consecutive chunks (CHUNKS <= 32).  Lane j of every warp reads the
+// count of chunk j (coalesced) and a warp scan gives the tile's layout, in registers, in every warp.  Event e of
+// the tile (e = 0 .. total-1, normally one per thread) belongs to the chunk j with off_j <= e < off_{j+1};
+// its data come from the staged record r = e - off_j of that chunk, or, when the chunk has no records
+// (generate_* path, segment overflow, ragged tail), from a ballot/popc re-scan of the chunk's tau.
+template <typename R, typename TR, int KIND, int THREADS, int CHUNKS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R, TR> a) {
+    constexpr int WARPS = THREADS / 32;
+    __shared__ unsigned char list[CHUNKS][kChunk];  // re-scanned chunks: local indices of the fired particles
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_tile = (long long)(atomicAdd(a.tile_counter, 1ull) - a.tile_base);
-    __syncthreads();
-    const long long tile = s_tile;
-    const long long first_chunk = tile * kTileChunks;
-
-    // 1. per-chunk counts (4 chunks per warp); overflowed / tail chunks are re-scanned with ballot/popc
-#pragma unroll 1
-    for (int k = 0; k < kTileChunks / kEventWarps; ++k) {
-        const int j = warp * (kTileChunks / kEventWarps) + k;
-        const long long cbase = (first_chunk + j) * kChunk;
-        unsigned int c = cbase < a.n ? a.stage_cnt[first_chunk + j] : 0u;
-        const bool re = c > (unsigned)kStageCap;
-        if (re) {
-            c = 0;
+    const long long first_chunk = (long long)blockIdx.x * CHUNKS;
+    const long long n_chunks = (a.n + kChunk - 1) / kChunk;
+    const bool real = lane < CHUNKS && first_chunk + lane < n_chunks;
+    const unsigned short flags = real ? a.stage_cnt[first_chunk + lane] : (unsigned short)0;
+    const unsigned long long excl = a.tile_offset[blockIdx.x];            // output slot of the tile's first event
+    const unsigned int cnt = flags & kStageCountMask;
+    unsigned int incl = cnt;                                             // offsets of the chunks inside the tile
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const unsigned int o = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += o;
+    }
+    const unsigned int off_lane = incl - cnt;
+    const unsigned int total = __shfl_sync(0xffffffffu, incl, 31);
+    if (total == 0) return;
+    const unsigned int rescan_mask =
+        __ballot_sync(0xffffffffu, cnt > 0 && (cnt > (unsigned)kStageCap || (flags & kStageNoRecords) != 0));
+    if (rescan_mask) {  // chunks without records: find their fired particles again (tau < 0), in index order
+        for (int j = warp; j < CHUNKS; j += WARPS) {
+            if (!((rescan_mask >> j) & 1u)) continue;
+            const long long cbase = (first_chunk + j) * kChunk;
+            unsigned int k = 0;
 #pragma unroll
             for (int r4 = 0; r4 < kChunk / 32; ++r4) {
                 const long long i = cbase + r4 * 32 + lane;
                 const bool f = i < a.n && a.tau[i] < (TR)0;
                 const unsigned int bal = __ballot_sync(0xffffffffu, f);
-                if (f) list[j][c + __popc(bal & ((1u << lane) - 1u))] = (unsigned char)(r4 * 32 + lane);
-                c += __popc(bal);
+                if (f) list[j][k + __popc(bal & ((1u << lane) - 1u))] = (unsigned char)(r4 * 32 + lane);
+                k += __popc(bal);
             }
         }
-        if (lane == 0) { cnt[j] = c; rescan[j] = re ? 1 : 0; }
+        __syncthreads();
     }
-    __syncthreads();
-
-    // 2. offsets of the chunks inside the tile, offset of the tile in the output (decoupled look-back)
-    if (warp == 0) {
-        const unsigned int c = cnt[lane];
-        unsigned int incl = c;
+    for (unsigned int e0 = 0; e0 < total; e0 += THREADS) {
+        const unsigned int e = e0 + tid;
+        // chunk of event e: the largest j with off_j <= e (ties are empty chunks followed by the one that holds
+        // e; lanes past the last chunk carry off = total > e); the offsets live in the lanes' registers
+        int j = 0;
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const unsigned int o = __shfl_up_sync(0xffffffffu, incl, d);
-            if (lane >= d) incl += o;
+        for (int step = 16; step > 0; step >>= 1) {
+            const int cand = j + step;
+            const unsigned int oc = __shfl_sync(0xffffffffu, off_lane, min(cand, 31));
+            if (cand < 32 && oc <= e) j = cand;
         }
-        off[lane] = incl - c;
-        const unsigned int total = __shfl_sync(0xffffffffu, incl, 31);
-        if (lane == 31) off[kTileChunks] = total;
-        const unsigned long long excl = tile_exclusive_prefix(a.status, tile, a.epoch, total, lane);
-        if (lane == 0) {
-            s_excl = excl;
-            if ((tile + 1) * (long long)kEventTile >= a.n) *a.d_n_out = excl + total;  // last tile: total fired
-        }
-    }
-    __syncthreads();
-
-    // 3. events, densely over the threads
-    const unsigned int total = off[kTileChunks];
-    const unsigned long long excl = s_excl;
-    for (unsigned int e = tid; e < total; e += kEventThreads) {
+        const unsigned int off_j = __shfl_sync(0xffffffffu, off_lane, j);
         const long long slot = (long long)(excl + e);
-        if (slot >= a.capacity) break;  // capacity rule (R16)
-        int j = 0;                      // largest j with off[j] <= e
-#pragma unroll
-        for (int step = kTileChunks / 2; step > 0; step >>= 1)
-            if (off[j + step] <= e) j += step;
-        const unsigned int r = e - off[j];
+        if (e >= total || slot >= a.capacity) continue;  // capacity rule (R16): later parents untouched
+        const unsigned int r = e - off_j;
         const long long cbase = (first_chunk + j) * kChunk;
         double px, py, pz, ex, ey, ez, bx, by, bz;
         long long i;
-        if (rescan[j]) {
+        if ((rescan_mask >> j) & 1u) {
             i = cbase + list[j][r];
             px = a.p[0][i]; py = a.p[1][i]; pz = a.p[2][i];
             ex = a.e[0][i]; ey = a.e[1][i]; ez = a.e[2][i];
             bx = a.b[0][i]; by = a.b[1][i]; bz = a.b[2][i];
         } else {
-            const long long pos = (first_chunk + j) * kStageCap + r;
-            i = cbase + a.stage_idx[pos];
-            const R* rec = a.stage_rec + pos;
-            px = rec[0]; py = rec[a.stage_stride]; pz = rec[2 * a.stage_stride];
-            ex = rec[3 * a.stage_stride]; ey = rec[4 * a.stage_stride]; ez = rec[5 * a.stage_stride];
-            bx = rec[6 * a.stage_stride]; by = rec[7 * a.stage_stride]; bz = rec[8 * a.stage_stride];
+            constexpr int NV = StageRecord<R>::kVecs;
+            const uint4* src = reinterpret_cast<const uint4*>(
+                a.stage_rec + ((first_chunk + j) * (long long)kStageCap + r) * StageRecord<R>::kBytes);
+            uint4 raw[NV];
+#pragma unroll
+            for (int k = 0; k < NV; ++k) raw[k] = __ldg(src + k);
+            const R* w = reinterpret_cast<const R*>(raw);
+            px = w[0]; py = w[1]; pz = w[2]; ex = w[3]; ey = w[4]; ez = w[5]; bx = w[6]; by = w[7]; bz = w[8];
+            i = cbase + *reinterpret_cast<const unsigned int*>(&w[9]);
         }
-        if (KIND == 0) qs_event_core<R, TR>(a, i, slot, px, py, pz, ex, ey, ez, bx, by, bz);
-        else bw_event_core<R, TR>(a, i, slot, px, py, pz, ex, ey, ez, bx, by, bz);
+        const EventOut<R, TR> out = KIND == 0 ? qs_event_compute<R, TR>(a, i, px, py, pz, ex, ey, ez, bx, by, bz)
+                                              : bw_event_compute<R, TR>(a, i, px, py, pz, ex, ey, ez, bx, by, bz);
+        event_commit<R, TR, KIND>(a, i, slot, out);
     }
 }
 

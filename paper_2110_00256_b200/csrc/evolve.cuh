@@ -28,15 +28,26 @@ struct EvolveArgs {
     unsigned long long* d_n_events;
     int table_in_smem;
     // record emission (EMIT kernels only): every 128-particle chunk owns a segment of kStageCap records
-    R* stage_rec;               // [9][n_chunks * kStageCap]: px..bz of the fired particles, in index order
-    unsigned char* stage_idx;   // [n_chunks * kStageCap]: index of the fired particle inside its chunk
-    unsigned short* stage_cnt;  // [n_chunks]: fired particles of the chunk, or kStageRescan
-    long long stage_stride;     // n_chunks * kStageCap
+    unsigned char* stage_rec;   // [n_chunks][kStageCap] records (see StageRecord), in index order
+    unsigned short* stage_cnt;  // [n_chunks]: fired particles of the chunk | flags (see kStage* below)
+    unsigned table_bytes;       // dynamic shared memory: [table, padded to 128 B][per-warp record buffers]
 };
 
 constexpr int kChunk = 128;                 // particles one warp handles per tile: the unit of record staging
 constexpr int kStageCap = 24;               // records per chunk segment (mean at 5 % firing: 6.4)
-constexpr unsigned short kStageRescan = 0xFFFFu;  // chunk must be re-scanned by the event kernel (ragged tail)
+// stage_cnt[chunk]: bits 0..14 = number of particles of the chunk that fired; bit 15 = the chunk has no staged
+// records (segment overflow, or counted by count_chunks_kernel); 0xFFFF = not counted yet (ragged tail)
+constexpr unsigned short kStageCountMask = 0x7FFFu;
+constexpr unsigned short kStageNoRecords = 0x8000u;
+constexpr unsigned short kStageUnknown = 0xFFFFu;
+
+// one staged record: px,py,pz, ex,ey,ez, bx,by,bz of a particle that fired + its index inside the chunk,
+// padded to a multiple of 16 bytes (fp64: 80 B, fp32: 48 B) so that records move as 128-bit vectors
+template <typename R> struct StageRecord {
+    static constexpr int kWords = sizeof(R) == 8 ? 10 : 12;          // in units of R
+    static constexpr int kBytes = kWords * (int)sizeof(R);
+    static constexpr int kVecs = kBytes / 16;
+};
 
 // ---- TMA bulk copy of a 1D table into shared memory ------------------------------------
 __device__ __forceinline__ void stage_table_tma(void* smem_dst, const void* gmem_src, unsigned bytes,
@@ -125,6 +136,9 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
         tab = reinterpret_cast<const R*>(smem_raw);
     }
 
+    const unsigned long long pol_stream = l2_policy_evict_first();
+    const unsigned long long pol_keep = l2_policy_evict_last();
+    (void)pol_keep;
     unsigned int fired = 0;
     const long long ntiles = (a.n + TILE - 1) / TILE;
     for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
@@ -138,11 +152,11 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                 const long long i = base + (long long)warp * WCH + (u * 32 + lane) * V;
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
-                    q[c][u] = ld_stream<R, V>(a.p[c] + i);
-                    q[3 + c][u] = ld_stream<R, V>(a.e[c] + i);
-                    q[6 + c][u] = ld_stream<R, V>(a.b[c] + i);
+                    q[c][u] = ld_stream<R, V>(a.p[c] + i, pol_stream);
+                    q[3 + c][u] = ld_stream<R, V>(a.e[c] + i, pol_stream);
+                    q[6 + c][u] = ld_stream<R, V>(a.b[c] + i, pol_stream);
                 }
-                t[u] = *reinterpret_cast<const Vec<TR, V>*>(a.tau + i);
+                t[u] = ld_stream_rw<TR, V>(a.tau + i, pol_stream);
             }
             unsigned int fired_bits = 0;
 #pragma unroll
@@ -177,27 +191,38 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                     total += all;
                 }
                 const long long chunk = (base + (long long)warp * WCH) / kChunk;
-                if (lane == 0) a.stage_cnt[chunk] = (unsigned short)total;
-                if (total <= (unsigned)kStageCap && fired_bits) {  // else: the event kernel re-scans the chunk
+                if (lane == 0)
+                    a.stage_cnt[chunk] = (unsigned short)(total <= (unsigned)kStageCap ? total : (total | kStageNoRecords));
+                if (total > 0 && total <= (unsigned)kStageCap) {  // (overflow: the event kernel re-scans the chunk)
+                    // records are assembled in this warp's shared-memory buffer (scattered 8-byte writes are
+                    // cheap there) and leave as one coalesced stream of 128-bit stores
+                    constexpr int W = StageRecord<R>::kWords;
+                    R* wbuf = reinterpret_cast<R*>(smem_raw + a.table_bytes) + warp * (kStageCap * W);
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
-                        long long r = chunk * kStageCap + rank_u[u];
+                        unsigned int r = rank_u[u];
 #pragma unroll
                         for (int v = 0; v < V; ++v) {
                             if ((fired_bits >> (u * V + v)) & 1u) {
 #pragma unroll
-                                for (int c = 0; c < 9; ++c) a.stage_rec[c * a.stage_stride + r] = q[c][u].v[v];
-                                a.stage_idx[r] = (unsigned char)((u * 32 + lane) * V + v);
+                                for (int c = 0; c < 9; ++c) wbuf[r * W + c] = q[c][u].v[v];
+                                *reinterpret_cast<unsigned int*>(&wbuf[r * W + 9]) = (unsigned)((u * 32 + lane) * V + v);
                                 ++r;
                             }
                         }
                     }
+                    __syncwarp();
+                    const uint4* src = reinterpret_cast<const uint4*>(wbuf);
+                    uint4* dst = reinterpret_cast<uint4*>(a.stage_rec + chunk * (long long)(kStageCap * StageRecord<R>::kBytes));
+                    const unsigned int nvec = total * StageRecord<R>::kVecs;
+                    for (unsigned int k = lane; k < nvec; k += 32) st_policy(dst + k, src[k], pol_keep);
+                    __syncwarp();
                 }
             }
         } else {  // ragged last tile: scalar, guarded
             if constexpr (EMIT) {  // its chunks are re-scanned by the event kernel
                 const long long c0 = base / kChunk, c1 = (a.n + kChunk - 1) / kChunk;
-                for (long long c = c0 + threadIdx.x; c < c1; c += kEvolveThreads) a.stage_cnt[c] = kStageRescan;
+                for (long long c = c0 + threadIdx.x; c < c1; c += kEvolveThreads) a.stage_cnt[c] = kStageUnknown;
             }
             for (long long i = base + threadIdx.x; i < a.n; i += kEvolveThreads) {
                 const R d = decrement_one<R, SPECIES>(a.p[0][i], a.p[1][i], a.p[2][i], a.e[0][i], a.e[1][i],
@@ -247,11 +272,12 @@ __global__ void __launch_bounds__(256) chi_kernel(const R* __restrict__ px, cons
         const double g = sqrt(SPECIES == 0 ? 1.0 + p2 : p2);
         return (R)sqrt(chi_squared<SPECIES>(x, y, z, exr, eyr, ezr, bxr, byr, bzr, g, p2));
     };
+    const unsigned long long pol = l2_policy_evict_first();
     for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < nvec; j += stride) {
         const long long i = j * V;
-        const Vec<R, V> a0 = ld_stream<R, V>(px + i), a1 = ld_stream<R, V>(py + i), a2 = ld_stream<R, V>(pz + i),
-                        a3 = ld_stream<R, V>(ex + i), a4 = ld_stream<R, V>(ey + i), a5 = ld_stream<R, V>(ez + i),
-                        a6 = ld_stream<R, V>(bx + i), a7 = ld_stream<R, V>(by + i), a8 = ld_stream<R, V>(bz + i);
+        const Vec<R, V> a0 = ld_stream<R, V>(px + i, pol), a1 = ld_stream<R, V>(py + i, pol), a2 = ld_stream<R, V>(pz + i, pol),
+                        a3 = ld_stream<R, V>(ex + i, pol), a4 = ld_stream<R, V>(ey + i, pol), a5 = ld_stream<R, V>(ez + i, pol),
+                        a6 = ld_stream<R, V>(bx + i, pol), a7 = ld_stream<R, V>(by + i, pol), a8 = ld_stream<R, V>(bz + i, pol);
         Vec<R, V> o;
 #pragma unroll
         for (int v = 0; v < V; ++v)

@@ -27,21 +27,20 @@ struct picsarqed_ctx {
     double* tab64[4] = {nullptr, nullptr, nullptr, nullptr};  // lnG, qs_lnP, lnT, bw_P
     float* tab32[4] = {nullptr, nullptr, nullptr, nullptr};   // fp32-rounded copies
     size_t tab_n[4] = {0, 0, 0, 0};
+    // search guides of the two CDF tables (see Table2D::guide), [0] photon emission, [1] pair production
+    unsigned short* guide[2] = {nullptr, nullptr};
+    double guide_k0[2] = {0.0, 0.0}, guide_inv_dk[2] = {0.0, 0.0};
+    double* d_scalar = nullptr;
 
     // evolve: per-CTA counts + arrival ticket
     unsigned int* partials = nullptr;
     unsigned int* ticket = nullptr;
     int partials_cap = 0;
-    // events: look-back status words + tile ticket counter
-    unsigned long long* status = nullptr;
-    size_t status_cap = 0;
-    unsigned long long* tile_counter = nullptr;
-    unsigned long long tile_base = 0;  // host mirror of *tile_counter
-    unsigned epoch = 0;
     // tuning knobs (picsarqed_set_option)
     int evolve_unroll = 0;       // 0 = default per dtype
     int evolve_ctas_per_sm = 0;  // 0 = occupancy
-    // qed_step: records of the fired particles, written by the evolve pass, read by the event pass
+    int event_config = 0;        // shape of event_kernel: see launch_event_pass
+    // per-chunk scratch of the event path: staged records, counts, output offsets (see events.cuh)
     void* rec = nullptr;
     size_t rec_bytes = 0;
     // host-path staging
@@ -113,6 +112,65 @@ int narrow_tables(picsarqed_ctx* c) {
     return PICSARQED_OK;
 }
 
+constexpr int kGuideBins = 256;
+
+// minimum of column 0 over the rows (lower end of the key range of the photon-emission guide)
+__global__ void column0_min_kernel(const double* __restrict__ tab, int n_rows, int n_cols, double* out) {
+    __shared__ double red[256];
+    double m = INFINITY;
+    for (int r = threadIdx.x; r < n_rows; r += blockDim.x) m = fmin(m, tab[(size_t)r * n_cols]);
+    red[threadIdx.x] = m;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if ((int)threadIdx.x < s) red[threadIdx.x] = fmin(red[threadIdx.x], red[threadIdx.x + s]);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = red[0];
+}
+
+// guide[n][j] = max{m : tab[n][m] <= k0 + j dk}, 0 if there is none and for j = 0 (whose lower edge is -inf)
+__global__ void guide_kernel(const double* __restrict__ tab, int n_rows, int n_cols, double k0, double dk, int bins,
+                             unsigned short* __restrict__ guide) {
+    const long long total = (long long)n_rows * (bins + 1);
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const int n = (int)(t / (bins + 1)), j = (int)(t % (bins + 1));
+        const double key = k0 + j * dk;
+        const double* row = tab + (size_t)n * n_cols;
+        int lo = -1, hi = n_cols;  // row[lo] <= key < row[hi]
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (row[mid] <= key) lo = mid; else hi = mid;
+        }
+        guide[t] = (unsigned short)(j == 0 ? 0 : max(lo, 0));
+    }
+}
+
+int build_guides(picsarqed_ctx* c) {
+    for (int kind = 0; kind < 2; ++kind) {
+        if (c->guide[kind]) cudaFree(c->guide[kind]);
+        c->guide[kind] = nullptr;
+        const int rows = kind == 0 ? c->tp.qs_n_chi : c->tp.bw_n_chi, cols = kind == 0 ? c->tp.qs_n_xi : c->tp.bw_n_xi;
+        if (cols > 65535) continue;  // indices are stored in 16 bits; wider tables are searched unguided
+        const double* tab = c->tab64[kind == 0 ? PICSARQED_TAB_QS_LNP : PICSARQED_TAB_BW_P];
+        double k0 = 0.0, k1 = 0.5;
+        if (kind == 0) {
+            if (!c->d_scalar) PXQ_CUDA(c, cudaMalloc(&c->d_scalar, sizeof(double)));
+            column0_min_kernel<<<1, 256, 0, c->stream>>>(tab, rows, cols, c->d_scalar);
+            PXQ_CUDA(c, cudaMemcpyAsync(&k0, c->d_scalar, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+            PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+            k1 = 0.0;
+            if (!std::isfinite(k0) || !(k0 < 0.0)) continue;
+        }
+        const double dk = (k1 - k0) / kGuideBins;
+        PXQ_CUDA(c, cudaMalloc(&c->guide[kind], (size_t)rows * (kGuideBins + 1) * sizeof(unsigned short)));
+        guide_kernel<<<c->num_sms * 4, 256, 0, c->stream>>>(tab, rows, cols, k0, dk, kGuideBins, c->guide[kind]);
+        PXQ_CUDA(c, cudaGetLastError());
+        c->guide_k0[kind] = k0;
+        c->guide_inv_dk[kind] = 1.0 / dk;
+    }
+    return PICSARQED_OK;
+}
+
 template <typename R> const R* table_ptr(const picsarqed_ctx* c, int which);
 template <> const double* table_ptr<double>(const picsarqed_ctx* c, int which) { return c->tab64[which]; }
 template <> const float* table_ptr<float>(const picsarqed_ctx* c, int which) { return c->tab32[which]; }
@@ -144,6 +202,10 @@ Table2D<R> view_2d(const picsarqed_ctx* c, int species) {
     t.ln_max = std::log(hi);
     t.inv_delta = (t.n_chi - 1) / (t.ln_max - t.ln_min);
     t.ln_xi_min = species == 0 ? std::log(p.qs_xi_min) : 0.0;
+    t.guide = c->guide[species];
+    t.guide_bins = kGuideBins;
+    t.guide_k0 = c->guide_k0[species];
+    t.guide_inv_dk = c->guide_inv_dk[species];
     return t;
 }
 
@@ -181,8 +243,6 @@ int picsarqed_create(picsarqed_ctx** out, int cuda_device, void* cuda_stream) {
     }
     if (e == cudaSuccess) e = cudaMalloc(&c->ticket, sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaMemset(c->ticket, 0, sizeof(unsigned int));
-    if (e == cudaSuccess) e = cudaMalloc(&c->tile_counter, sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMemset(c->tile_counter, 0, sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMalloc(&c->d_counts, 2 * sizeof(unsigned long long));
     if (e != cudaSuccess) {
         delete c;
@@ -202,10 +262,11 @@ int picsarqed_destroy(picsarqed_ctx* c) {
     }
     cudaFree(c->partials);
     cudaFree(c->ticket);
-    cudaFree(c->status);
-    cudaFree(c->tile_counter);
     cudaFree(c->stage);
     cudaFree(c->rec);
+    cudaFree(c->guide[0]);
+    cudaFree(c->guide[1]);
+    cudaFree(c->d_scalar);
     cudaFree(c->d_counts);
     delete c;
     return PICSARQED_OK;
@@ -219,6 +280,8 @@ int picsarqed_set_option(picsarqed_ctx* c, const char* name, long long value) {
         c->evolve_unroll = (int)value;
     else if (!std::strcmp(name, "evolve_ctas_per_sm") && value >= 0 && value <= 32)
         c->evolve_ctas_per_sm = (int)value;
+    else if (!std::strcmp(name, "event_config") && value >= 0 && value <= 7)
+        c->event_config = (int)value;
     else
         return fail(c, PICSARQED_ERR_INVALID, std::string("unknown option or bad value: ") + name);
     return PICSARQED_OK;
@@ -235,6 +298,7 @@ int picsarqed_import_tables(picsarqed_ctx* c, const picsarqed_table_params* p, c
     for (int k = 0; k < 4; ++k)
         PXQ_CUDA(c, cudaMemcpyAsync(c->tab64[k], src[k], c->tab_n[k] * sizeof(double), cudaMemcpyHostToDevice, c->stream));
     if (int rc = narrow_tables(c)) return rc;
+    if (int rc = build_guides(c)) return rc;
     PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
     c->have_tables = true;
     return PICSARQED_OK;
@@ -281,11 +345,11 @@ int launch_chi(picsarqed_ctx* c, long long n, const void* const* a, void* out) {
     return PICSARQED_OK;
 }
 
-struct StageView { void* rec; unsigned char* idx; unsigned short* cnt; long long stride; };
+struct StageView { unsigned char* rec; unsigned short* cnt; };
 
 template <typename R, typename TR, int SPECIES, int U, bool EMIT>
 int launch_evolve_u(picsarqed_ctx* c, long long n, const void* const* a, double dt, void* tau,
-                    unsigned long long* d_n_events, StageView sv = StageView{nullptr, nullptr, nullptr, 0}) {
+                    unsigned long long* d_n_events, StageView sv = StageView{nullptr, nullptr}) {
     constexpr int V = 16 / sizeof(R);
     constexpr int TILE = kEvolveThreads * V * U;
     EvolveArgs<R, TR> args;
@@ -301,13 +365,13 @@ int launch_evolve_u(picsarqed_ctx* c, long long n, const void* const* a, double 
     args.partials = c->partials;
     args.ticket = c->ticket;
     args.d_n_events = d_n_events;
-    args.stage_rec = (R*)sv.rec;
-    args.stage_idx = sv.idx;
+    args.stage_rec = sv.rec;
     args.stage_cnt = sv.cnt;
-    args.stage_stride = sv.stride;
-    size_t smem = ((size_t)args.tab.n * sizeof(R) + 15) & ~(size_t)15;
+    size_t smem = ((size_t)args.tab.n * sizeof(R) + 127) & ~(size_t)127;
     args.table_in_smem = smem <= 96 * 1024;  // larger tables are read through L1/L2
     if (!args.table_in_smem) smem = 0;
+    args.table_bytes = (unsigned)smem;
+    if (EMIT) smem += (size_t)(kEvolveThreads / 32) * kStageCap * StageRecord<R>::kBytes;
     auto kern = evolve_kernel<R, TR, SPECIES, U, EMIT>;
     if (smem > 48 * 1024) PXQ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
@@ -331,90 +395,39 @@ int launch_evolve(picsarqed_ctx* c, long long n, const void* const* a, double dt
     return launch_evolve_u<R, TR, SPECIES, 2, false>(c, n, a, dt, tau, d_n_events);
 }
 
-// prepares the look-back scratch for a launch that hands out `tickets` tile tickets over `ntiles` tiles
-int prepare_lookback(picsarqed_ctx* c, long long ntiles) {
-    if ((size_t)ntiles > c->status_cap) {  // grow (rare; synchronises)
-        PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
-        if (c->status) cudaFree(c->status);
-        c->status = nullptr;
-        c->status_cap = (size_t)ntiles * 2;
-        PXQ_CUDA(c, cudaMalloc(&c->status, c->status_cap * sizeof(unsigned long long)));
-        PXQ_CUDA(c, cudaMemsetAsync(c->status, 0, c->status_cap * sizeof(unsigned long long), c->stream));
-        c->epoch = 0;
-    }
-    c->epoch += 1;
-    if (c->epoch >= (1u << kEpochBits)) {  // epoch wrapped: clear stale words
-        PXQ_CUDA(c, cudaMemsetAsync(c->status, 0, c->status_cap * sizeof(unsigned long long), c->stream));
-        c->epoch = 1;
-    }
-    return PICSARQED_OK;
-}
+// per-chunk scratch: [records][counts][offsets]
+struct ChunkScratch { unsigned char* rec; unsigned short* cnt; unsigned long long* off; unsigned int* sum; long long n_chunks; };
 
-template <typename R, typename TR, int KIND>
-int launch_events(picsarqed_ctx* c, long long n, void* const* p, const void* const* eb, void* tau,
-                  unsigned long long seed, unsigned long long step, unsigned long long id_base, long long capacity,
-                  void* const* out_p, void* const* out_tau, long long* parent, unsigned long long* d_n_out) {
-    const long long ntiles = (n + kEventTile - 1) / kEventTile;
-    if (int rc = prepare_lookback(c, ntiles)) return rc;
-    EventArgs<R, TR> args;
-    for (int k = 0; k < 3; ++k) {
-        args.p[k] = (R*)p[k];
-        args.e[k] = (const R*)eb[k];
-        args.b[k] = (const R*)eb[3 + k];
-    }
-    args.tau = (TR*)tau;
-    args.n = n;
-    args.cdf = view_2d<R>(c, KIND);
-    args.seed = seed;
-    args.step = step;
-    args.id_base = id_base;
-    args.capacity = capacity;
-    for (int k = 0; k < 6; ++k) args.out_p[k] = (R*)out_p[k];
-    for (int k = 0; k < 2; ++k) args.out_tau[k] = (TR*)out_tau[k];
-    args.parent = parent;
-    args.d_n_out = d_n_out;
-    args.status = c->status;
-    args.tile_counter = c->tile_counter;
-    args.tile_base = c->tile_base;
-    args.epoch = c->epoch;
-    args.stage_rec = nullptr;
-    args.stage_idx = nullptr;
-    args.stage_cnt = nullptr;
-    args.stage_stride = 0;
-    c->tile_base += (unsigned long long)ntiles;
-    event_kernel<R, TR, KIND><<<(unsigned)ntiles, kEventThreads, 0, c->stream>>>(args);
-    PXQ_CUDA(c, cudaGetLastError());
-    return PICSARQED_OK;
-}
-
-// qed_step = evolve pass that also stages the records of the fired particles + event pass over the records
-template <typename R, typename TR, int SPECIES>
-int launch_step(picsarqed_ctx* c, long long n, void* const* p, const void* const* eb, void* tau, double dt,
-                unsigned long long seed, unsigned long long step, unsigned long long id_base, long long capacity,
-                void* const* out_p, void* const* out_tau, long long* parent, unsigned long long* d_n_out) {
+template <typename R>
+int chunk_scratch(picsarqed_ctx* c, long long n, ChunkScratch* out) {
     const long long nchunks = (n + kChunk - 1) / kChunk;
-    const size_t rec_sz = ((size_t)nchunks * kStageCap * 9 * sizeof(R) + 255) & ~(size_t)255;
-    const size_t idx_sz = ((size_t)nchunks * kStageCap + 255) & ~(size_t)255;
+    const size_t rec_sz = ((size_t)nchunks * kStageCap * StageRecord<R>::kBytes + 255) & ~(size_t)255;
     const size_t cnt_sz = ((size_t)nchunks * sizeof(unsigned short) + 255) & ~(size_t)255;
-    if (rec_sz + idx_sz + cnt_sz > c->rec_bytes) {  // grow (rare; synchronises)
+    // tiles hold at least 8 chunks: n_chunks/8 + 1 tile offsets and tile sums are always enough
+    const size_t off_sz = ((size_t)(nchunks / 8 + 2) * sizeof(unsigned long long) + 255) & ~(size_t)255;
+    const size_t sum_sz = ((size_t)(nchunks / 8 + 2) * sizeof(unsigned int) + 255) & ~(size_t)255;
+    if (rec_sz + cnt_sz + off_sz + sum_sz > c->rec_bytes) {  // grow (rare; synchronises)
         PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
         if (c->rec) cudaFree(c->rec);
         c->rec = nullptr;
         c->rec_bytes = 0;
-        PXQ_CUDA(c, cudaMalloc(&c->rec, rec_sz + idx_sz + cnt_sz));
-        c->rec_bytes = rec_sz + idx_sz + cnt_sz;
+        PXQ_CUDA(c, cudaMalloc(&c->rec, rec_sz + cnt_sz + off_sz + sum_sz));
+        c->rec_bytes = rec_sz + cnt_sz + off_sz + sum_sz;
     }
-    StageView sv;
-    sv.rec = c->rec;
-    sv.idx = static_cast<unsigned char*>(c->rec) + rec_sz;
-    sv.cnt = reinterpret_cast<unsigned short*>(static_cast<unsigned char*>(c->rec) + rec_sz + idx_sz);
-    sv.stride = nchunks * kStageCap;
-    const void* a10[9] = {p[0], p[1], p[2], eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]};
-    constexpr int U = kChunk / (32 * (16 / (int)sizeof(R)));  // fp64: 2, fp32: 1
-    if (int rc = launch_evolve_u<R, TR, SPECIES, U, true>(c, n, a10, dt, tau, nullptr, sv)) return rc;
+    out->rec = static_cast<unsigned char*>(c->rec);
+    out->cnt = reinterpret_cast<unsigned short*>(out->rec + rec_sz);
+    out->off = reinterpret_cast<unsigned long long*>(out->rec + rec_sz + cnt_sz);
+    out->sum = reinterpret_cast<unsigned int*>(out->rec + rec_sz + cnt_sz + off_sz);
+    out->n_chunks = nchunks;
+    return PICSARQED_OK;
+}
 
-    const long long ntiles = (n + kEventTile - 1) / kEventTile;
-    if (int rc = prepare_lookback(c, ntiles)) return rc;
+// levels 2 and 3 of the compaction: chunk counts -> offsets -> events
+template <typename R, typename TR, int KIND>
+int launch_event_pass(picsarqed_ctx* c, long long n, const ChunkScratch& cs, void* const* p, const void* const* eb,
+                      void* tau, unsigned long long seed, unsigned long long step, unsigned long long id_base,
+                      long long capacity, void* const* out_p, void* const* out_tau, long long* parent,
+                      unsigned long long* d_n_out) {
     EventArgs<R, TR> ev;
     for (int k = 0; k < 3; ++k) {
         ev.p[k] = (R*)p[k];
@@ -423,7 +436,7 @@ int launch_step(picsarqed_ctx* c, long long n, void* const* p, const void* const
     }
     ev.tau = (TR*)tau;
     ev.n = n;
-    ev.cdf = view_2d<R>(c, SPECIES);
+    ev.cdf = view_2d<R>(c, KIND);
     ev.seed = seed;
     ev.step = step;
     ev.id_base = id_base;
@@ -431,19 +444,58 @@ int launch_step(picsarqed_ctx* c, long long n, void* const* p, const void* const
     for (int k = 0; k < 6; ++k) ev.out_p[k] = (R*)out_p[k];
     for (int k = 0; k < 2; ++k) ev.out_tau[k] = (TR*)out_tau[k];
     ev.parent = parent;
-    ev.d_n_out = d_n_out;
-    ev.status = c->status;
-    ev.tile_counter = c->tile_counter;
-    ev.tile_base = c->tile_base;
-    ev.epoch = c->epoch;
-    ev.stage_rec = (const R*)sv.rec;
-    ev.stage_idx = sv.idx;
-    ev.stage_cnt = sv.cnt;
-    ev.stage_stride = sv.stride;
-    c->tile_base += (unsigned long long)ntiles;
-    staged_event_kernel<R, TR, SPECIES><<<(unsigned)ntiles, kEventThreads, 0, c->stream>>>(ev);
+    ev.stage_rec = cs.rec;
+    ev.stage_cnt = cs.cnt;
+    ev.tile_offset = cs.off;
+    static const int kChunksOf[8] = {24, 32, 24, 16, 12, 20, 8, 32};  // must match the switch below
+    const int chunks = kChunksOf[c->event_config];
+    const long long n_tiles = (cs.n_chunks + chunks - 1) / chunks;
+    const unsigned grid = (unsigned)n_tiles;
+    const int sum_grid = (int)std::max<long long>(1, std::min<long long>((n_tiles + 7) / 8, (long long)c->num_sms * 8));
+    tile_sums_kernel<TR><<<sum_grid, 256, 0, c->stream>>>(cs.cnt, cs.n_chunks, chunks, n_tiles, (const TR*)tau, n, cs.sum);
+    tile_scan_kernel<<<1, kScanThreads, 0, c->stream>>>(cs.sum, n_tiles, cs.off, d_n_out);
+    switch (c->event_config) {
+        case 1: event_kernel<R, TR, KIND, 256, 32, 3><<<grid, 256, 0, c->stream>>>(ev); break;
+        case 2: event_kernel<R, TR, KIND, 256, 24, 4><<<grid, 256, 0, c->stream>>>(ev); break;
+        case 3: event_kernel<R, TR, KIND, 256, 16, 4><<<grid, 256, 0, c->stream>>>(ev); break;
+        case 4: event_kernel<R, TR, KIND, 128, 12, 8><<<grid, 128, 0, c->stream>>>(ev); break;
+        case 5: event_kernel<R, TR, KIND, 256, 20, 4><<<grid, 256, 0, c->stream>>>(ev); break;
+        case 6: event_kernel<R, TR, KIND, 128, 8, 8><<<grid, 128, 0, c->stream>>>(ev); break;
+        case 7: event_kernel<R, TR, KIND, 384, 32, 2><<<grid, 384, 0, c->stream>>>(ev); break;
+        default: event_kernel<R, TR, KIND, 256, 24, 3><<<grid, 256, 0, c->stream>>>(ev); break;
+    }
     PXQ_CUDA(c, cudaGetLastError());
     return PICSARQED_OK;
+}
+
+// generate_photons / generate_pairs: count the chunks from tau, then the common event pass
+template <typename R, typename TR, int KIND>
+int launch_events(picsarqed_ctx* c, long long n, void* const* p, const void* const* eb, void* tau,
+                  unsigned long long seed, unsigned long long step, unsigned long long id_base, long long capacity,
+                  void* const* out_p, void* const* out_tau, long long* parent, unsigned long long* d_n_out) {
+    ChunkScratch cs;
+    if (int rc = chunk_scratch<R>(c, n, &cs)) return rc;
+    const int grid = (int)std::max<long long>(1, std::min<long long>((cs.n_chunks + 7) / 8, (long long)c->num_sms * 8));
+    count_chunks_kernel<TR><<<grid, 256, 0, c->stream>>>((const TR*)tau, n, cs.n_chunks, cs.cnt);
+    return launch_event_pass<R, TR, KIND>(c, n, cs, p, eb, tau, seed, step, id_base, capacity, out_p, out_tau, parent,
+                                          d_n_out);
+}
+
+// qed_step: the evolve pass stages the records of the particles that fire, then the common event pass
+template <typename R, typename TR, int SPECIES>
+int launch_step(picsarqed_ctx* c, long long n, void* const* p, const void* const* eb, void* tau, double dt,
+                unsigned long long seed, unsigned long long step, unsigned long long id_base, long long capacity,
+                void* const* out_p, void* const* out_tau, long long* parent, unsigned long long* d_n_out) {
+    ChunkScratch cs;
+    if (int rc = chunk_scratch<R>(c, n, &cs)) return rc;
+    StageView sv;
+    sv.rec = cs.rec;
+    sv.cnt = cs.cnt;
+    const void* a9[9] = {p[0], p[1], p[2], eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]};
+    constexpr int U = kChunk / (32 * (16 / (int)sizeof(R)));  // fp64: 2, fp32: 1
+    if (int rc = launch_evolve_u<R, TR, SPECIES, U, true>(c, n, a9, dt, tau, nullptr, sv)) return rc;
+    return launch_event_pass<R, TR, SPECIES>(c, n, cs, p, eb, tau, seed, step, id_base, capacity, out_p, out_tau, parent,
+                                             d_n_out);
 }
 
 // dispatch on (dtype, tau_dtype); fp64 particles with fp32 optical depth is not offered
@@ -721,6 +773,7 @@ extern "C" int picsarqed_build_tables(picsarqed_ctx* c, const picsarqed_table_pa
         PXQ_CUDA(c, cudaGetLastError());
     }
     if (int rc = narrow_tables(c)) return rc;
+    if (int rc = build_guides(c)) return rc;
     PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
     c->have_tables = true;
     return PICSARQED_OK;

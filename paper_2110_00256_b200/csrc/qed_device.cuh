@@ -39,6 +39,11 @@ struct Table2D {      // rows: log-spaced chi; columns: xi grid
     int n_chi, n_xi;
     double ln_min, ln_max, inv_delta;
     double ln_xi_min; // QS only: ln(xi_min)
+    // search guide (may be null): guide[n * (bins + 1) + j] = max{m : P[n][m] <= key_j} (0 if none, and for j = 0),
+    // key_j = guide_k0 + j / guide_inv_dk: narrows the binary search of eq.25 / eq.29 without changing its result
+    const unsigned short* guide;
+    int guide_bins;
+    double guide_k0, guide_inv_dk;
 };
 
 // ---- Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11) --------------------------------
@@ -177,6 +182,85 @@ __device__ __forceinline__ void row_bracket(const Table2D<R>& T, double ln_chi, 
     *w_out = t - (double)k;
 }
 
+// ---- the search of eq.25 / eq.29 -------------------------------------------------------
+// Finds m* = max{m : ell(m) <= key} for the row interpolated between rows k and k+1 with weight w
+// (eq.24 / eq.28), clamped to M-2, and returns it with a = ell(m*), b = ell(m*+1).  Precondition:
+// ell(0) <= key.  The result is the one a plain bisection over [0, M-1] gives (ell is non-decreasing);
+// only the schedule differs, because an event is a chain of dependent L2 accesses and its length is what
+// costs time: (1) the per-row guide gives a bracket [lo, hi] that provably contains m* (each of the two
+// rows bounds the interpolated row); it is verified against the table and dropped if a rounding of the bin
+// index made it wrong; (2) every level probes eight interior points at once (nine-way split), so the
+// bracket closes in one or two round trips instead of log2(M).
+template <typename R>
+__device__ __forceinline__ int search_row(const Table2D<R>& T, int k, double w, double key, double* a_out, double* b_out) {
+    const int M = T.n_xi;
+    const R* __restrict__ r0 = T.P + (size_t)k * M;
+    const R* __restrict__ r1 = r0 + M;
+    auto ell = [&](int m) { const double a = (double)__ldg(r0 + m); return fma(w, (double)__ldg(r1 + m) - a, a); };
+    int lo = 0, hi = M - 1;
+    bool verified = true;
+    if (T.guide != nullptr) {
+        const int J = T.guide_bins;
+        int j = (int)((key - T.guide_k0) * T.guide_inv_dk);
+        j = max(0, min(j, J - 1));
+        const unsigned short* g0 = T.guide + (size_t)k * (J + 1) + j;
+        const unsigned short* g1 = g0 + (J + 1);
+        const int a0 = __ldg(g0), a1 = __ldg(g0 + 1), b0 = __ldg(g1), b1 = __ldg(g1 + 1);
+        lo = j == 0 ? 0 : min(a0, b0);
+        hi = min(max(a1, b1) + 1, M - 1);
+        verified = false;
+    }
+    double va = 0.0, vb = 0.0;
+    if (verified) va = ell(0);  // (vb is never used before it is set: hi = M-1 needs no upper value)
+    while (true) {
+        const int span = hi - lo;
+        const int step = (span + 8) / 9;
+        double v[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int m = lo + (q + 1) * step;
+            v[q] = m < hi ? ell(m) : 0.0;
+        }
+        if (!verified) {
+            va = ell(lo);
+            vb = ell(hi);
+            verified = true;
+            if (!(va <= key) || !(vb > key || hi == M - 1)) {  // guide bracket does not hold: full range
+                lo = 0;
+                hi = M - 1;
+                va = ell(0);
+                continue;
+            }
+        }
+        if (span <= 1) break;
+        int cnt = 0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) cnt += (lo + (q + 1) * step < hi && v[q] <= key) ? 1 : 0;
+        const int nlo = lo + cnt * step;
+        const int nhi_c = lo + (cnt + 1) * step;
+        double na = va, nb = vb;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            if (q + 1 == cnt) na = v[q];
+            if (q == cnt && nhi_c < hi) nb = v[q];
+        }
+        if (nhi_c < hi) hi = nhi_c;
+        lo = nlo;
+        va = na;
+        vb = nb;
+    }
+    if (hi - lo < 1) {            // lo == hi == M-1 (key at or above the last column)
+        lo = M - 2;
+        va = ell(lo);
+        vb = ell(lo + 1);
+    } else if (hi == M - 1) {
+        vb = ell(hi);             // the upper end was never probed
+    }
+    *a_out = va;
+    *b_out = vb;
+    return lo;
+}
+
 // eqs.28-30: xi = chi_gamma/chi of the emitted photon for uniform r.
 // Event arithmetic is fp64 whatever the table element type (events are rare).
 template <typename R>
@@ -185,22 +269,15 @@ __device__ __forceinline__ double qs_sample_xi(const Table2D<R>& T, double ln_ch
     row_bracket(T, ln_chi, &k, &w);
     const int M = T.n_xi;
     const R* __restrict__ r0 = T.P + (size_t)k * M;
-    const R* __restrict__ r1 = r0 + M;
-    auto ell = [&](int m) { const double a = (double)__ldg(r0 + m); return fma(w, (double)__ldg(r1 + m) - a, a); };  // eq.28
+    const double e0a = (double)__ldg(r0), e0b = (double)__ldg(r0 + M);
     const double lr = log(r);
-    if (lr < ell(0)) return exp(T.ln_xi_min);  // below the first column (R6)
-    int lo = 0, hi = M - 1;                    // ell(lo) <= lr; answer = max{m: ell(m) <= lr}
-    while (hi - lo > 1) {                      // eq.29
-        const int mid = (lo + hi) >> 1;
-        if (ell(mid) <= lr) lo = mid; else hi = mid;
-    }
-    if (ell(hi) <= lr) lo = hi;
-    const int ms = min(lo, M - 2);
-    const double step = -T.ln_xi_min / (double)(M - 1);       // ln xi_{m+1} - ln xi_m
+    if (lr < fma(w, e0b - e0a, e0a)) return exp(T.ln_xi_min);  // below the first column (R6)
+    double a, b;
+    const int ms = search_row(T, k, w, lr, &a, &b);            // eq.29
+    const double step = -T.ln_xi_min / (double)(M - 1);        // ln xi_{m+1} - ln xi_m
     const double lx0 = T.ln_xi_min + step * (double)ms;
-    const double a = ell(ms), b = ell(ms + 1);
     if (!(b > a)) return exp(lx0);
-    return exp(fma((lr - a) / (b - a), step, lx0));           // eq.30
+    return exp(fma((lr - a) / (b - a), step, lx0));            // eq.30
 }
 
 // eqs.24-26 on r' = min(r, 1-r): xi = chi_-/chi_gamma in [0, 1/2]
@@ -209,42 +286,60 @@ __device__ __forceinline__ double bw_sample_xi(const Table2D<R>& T, double ln_ch
     int k; double w;
     row_bracket(T, ln_chi, &k, &w);
     const int M = T.n_xi;
-    const R* __restrict__ r0 = T.P + (size_t)k * M;
-    const R* __restrict__ r1 = r0 + M;
-    auto P = [&](int m) { const double a = (double)__ldg(r0 + m); return fma(w, (double)__ldg(r1 + m) - a, a); };  // eq.24
-    int lo = 0, hi = M - 1;  // P(0) = 0 <= r'
-    while (hi - lo > 1) {    // eq.25
-        const int mid = (lo + hi) >> 1;
-        if (P(mid) <= rp) lo = mid; else hi = mid;
-    }
-    if (P(hi) <= rp) lo = hi;
-    const int ms = min(lo, M - 2);
+    double a, b;
+    const int ms = search_row(T, k, w, rp, &a, &b);            // eq.25 (P(0) = 0 <= r')
     const double step = 0.5 / (double)(M - 1);
     const double x0 = step * (double)ms;
-    const double a = P(ms), b = P(ms + 1);
     if (!(b > a)) return x0;
-    return fma((rp - a) / (b - a), step, x0);  // eq.26
+    return fma((rp - a) / (b - a), step, x0);                  // eq.26
 }
 
-// ---- 128-bit streaming loads / stores -------------------------------------------------
+// ---- 128-bit streaming loads / stores with L2 eviction policies -------------------------------
+// The particle arrays are read once per step: they go through L2 as evict-first, so that what is re-used
+// (the CDF tables, the guides, the staged records) stays resident in the 126 MB L2.
+__device__ __forceinline__ unsigned long long l2_policy_evict_first() {
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ unsigned long long l2_policy_evict_last() {
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+
 template <typename T, int V> struct alignas(sizeof(T) * V) Vec { T v[V]; };
 
+// read-only streaming load (never written during the kernel)
 template <typename T, int V>
-__device__ __forceinline__ Vec<T, V> ld_stream(const T* p) {
-    static_assert(sizeof(T) * V == 16 || sizeof(T) * V == 32, "16- or 32-byte vectors");
+__device__ __forceinline__ Vec<T, V> ld_stream(const T* p, unsigned long long policy) {
+    static_assert(sizeof(T) * V == 16, "128-bit vectors");
     Vec<T, V> r;
-    if constexpr (sizeof(T) * V == 16) {
-        uint32_t a, b, c, d;
-        asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
-                     : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "l"(p));
-        uint32_t* o = reinterpret_cast<uint32_t*>(&r);
-        o[0] = a; o[1] = b; o[2] = c; o[3] = d;
-    } else {
-        const Vec<T, V / 2> lo = ld_stream<T, V / 2>(p), hi = ld_stream<T, V / 2>(p + V / 2);
+    uint32_t a, b, c, d;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "l"(p), "l"(policy));
+    uint32_t* o = reinterpret_cast<uint32_t*>(&r);
+    o[0] = a; o[1] = b; o[2] = c; o[3] = d;
+    return r;
+}
+// the same without .nc, for arrays the kernel also writes (tau)
+template <typename T, int V>
+__device__ __forceinline__ Vec<T, V> ld_stream_rw(const T* p, unsigned long long policy) {
+    static_assert(sizeof(T) * V == 16 || sizeof(T) * V == 32, "128- or 256-bit vectors");
+    Vec<T, V> r;
+    uint32_t* o = reinterpret_cast<uint32_t*>(&r);
 #pragma unroll
-        for (int i = 0; i < V / 2; ++i) { r.v[i] = lo.v[i]; r.v[V / 2 + i] = hi.v[i]; }
+    for (int h = 0; h < (int)(sizeof(T) * V / 16); ++h) {
+        uint32_t a, b, c, d;
+        asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;"
+                     : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "l"(reinterpret_cast<const char*>(p) + 16 * h), "l"(policy) : "memory");
+        o[4 * h] = a; o[4 * h + 1] = b; o[4 * h + 2] = c; o[4 * h + 3] = d;
     }
     return r;
+}
+__device__ __forceinline__ void st_policy(uint4* p, const uint4& v, unsigned long long policy) {
+    asm volatile("st.global.L2::cache_hint.v4.u32 [%0], {%1,%2,%3,%4}, %5;"
+                 ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(policy) : "memory");
 }
 
 }  // namespace pxq
