@@ -27,9 +27,9 @@ METRIC = "QED MC step particles/sec (fp64/fp32) at 1 B200; achieved HBM GB/s vs 
 UNIT = "particles/s"
 SEED = 2
 BYTES_PER_PARTICLE_EVOLVE = 88  # 9 reads + tau read + tau write, fp64
-# dram__bytes_read.sum + dram__bytes_write.sum of one step_kernel launch (16 Mi particles), ncu --set full;
-# see profiles/.  None until measured.
-STEP_DRAM_TRAFFIC_BYTES = None
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the evolve pass (16 Mi particles), ncu --set full:
+# profiles/r1b_evolve_emit_full.md
+EVOLVE_DRAM_TRAFFIC_BYTES = 1343862000 + 157025000
 
 
 def parse():
@@ -162,6 +162,7 @@ def run_ours(args):
     import torch.distributed as dist
 
     import paper_2110_00256_b200 as q
+    from paper_2110_00256_b200 import sharding
     from paper_2110_00256_b200 import workloads as w
 
     rank = int(os.environ.get("RANK", "0"))
@@ -173,7 +174,7 @@ def run_ours(args):
     dev = torch.device("cuda", local)
     n = args.particles
     seed = SEED + 1000 * rank      # every rank owns an independent shard (weak scaling, no data-path collective)
-    id_base = rank * n
+    id_base, _ = sharding.shard_range(rank, world, world * n)   # contiguous global particle ids per rank
     cap = n // 8
 
     ctx = q.Context(local)
@@ -220,21 +221,26 @@ def run_ours(args):
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(args.steps)]
+    while not sampler.samples and not sampler.reasons and sampler.is_alive():
+        time.sleep(0.001)          # NVML is up before the timed region starts
+    ctx.set_option("time_kernels", 1)  # CUDA events around the evolve pass and the event pass, on this stream
+    ctx.get_timing()
     start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
     start.record()
     for k in range(args.steps):
-        ev[k][0].record()
-        step(args.warmup + k)      # one launch: step_kernel<double,double,LEPTON>
-        ev[k][1].record()
+        step(args.warmup + k)      # evolve_kernel<..., EMIT> + tile_sums + tile_scan + event_kernel
     stop.record()
     barrier()
     sampler.stop_flag = True
     sampler.join()
     ms_total = start.elapsed_time(stop)
-    ms_kernel = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
+    ms_evolve, ms_events, n_timed = ctx.get_timing()
+    ctx.set_option("time_kernels", 0)
+    ms_evolve /= max(n_timed, 1)
+    ms_events /= max(n_timed, 1)
     fired_last = ctx.read_count(n_out)
-    # the two-kernel path (evolve, then generate_photons) on the same state, for the per-kernel split
+    # the two-call path (evolve_optical_depth, then generate_photons) on the same state, for comparison
     split = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(5)]
     for k in range(5):
         s = args.warmup + args.steps + k
@@ -245,12 +251,9 @@ def run_ours(args):
         ctx.generate_photons(p, f[:3], f[3:], tau, seed, s, id_base, cap, ph_p, ph_tau, ph_parent, n_out)
         split[k][2].record()
     barrier()
-    ms_evolve = float(np.mean([e[0].elapsed_time(e[1]) for e in split[1:]]))
-    ms_events = float(np.mean([e[1].elapsed_time(e[2]) for e in split[1:]]))
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_evolve2 = float(np.mean([e[0].elapsed_time(e[1]) for e in split[1:]]))
+    ms_events2 = float(np.mean([e[1].elapsed_time(e[2]) for e in split[1:]]))
+    ms_total = sharding.max_over_ranks(ms_total, dev)
     value = world * n * args.steps / (ms_total * 1e-3)
 
     # ---- end to end through the C ABI with HOST buffers (copies inside the timed region) -------------
@@ -266,10 +269,7 @@ def run_ours(args):
         fired_e2e = ctx.step_host(q.LEPTON, p_e2e, f[:3], f[3:], tau_pin, dt, seed, 10_001 + k, id_base, cap, sec_pin)
     barrier()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = sharding.max_over_ranks(e2e_s, dev)
     e2e_value = world * n * args.e2e_steps / e2e_s
     h2d = 10 * n * 8
     d2h = 4 * n * 8 + 8 + min(fired_e2e, cap) * 4 * 8
@@ -279,10 +279,10 @@ def run_ours(args):
             dist.destroy_process_group()
         return
     peaks, peak_kind = measured_peaks()
-    # algorithmic bytes of one fused launch: evolve's 88 B per particle + per fired parent 3 reals of momentum
-    # rewritten, tau rewritten, photon (3 reals + tau) and parent index written = 72 B
-    step_bytes = BYTES_PER_PARTICLE_EVOLVE * n + 72 * fired_last
-    achieved = step_bytes / (ms_kernel * 1e-3) / 1e9
+    # dominant kernel: the evolve pass (evolve_kernel<double,double,LEPTON,2,EMIT>): 88 algorithmic bytes per particle
+    # (SURVEY.md 8(d)); the 80-byte records it stages for the ~5 % that fire are not counted as algorithmic
+    evolve_bytes = BYTES_PER_PARTICLE_EVOLVE * n
+    achieved = evolve_bytes / (ms_evolve * 1e-3) / 1e9
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -294,15 +294,17 @@ def run_ours(args):
                        n_sets, 6 * n * 8 >> 20, 4 * n * 8 >> 20),
                    "parallelism": "independent shards per GPU" if world > 1 else "single GPU",
                    "table_build_s": table_build_s},
-        "roofline": {"bound": "hbm", "kernel": "step_kernel<double,double,LEPTON>", "achieved": achieved,
+        "roofline": {"bound": "hbm", "kernel": "evolve_kernel<double,double,LEPTON,U=2,EMIT> (evolve pass of qed_step)",
+                     "achieved": achieved,
                      "peak": peaks["hbm_gbs"], "peak_kind": peak_kind + " (MEASURED_PEAKS.json hbm_gbs, copy)",
                      "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
-                     "traffic": STEP_DRAM_TRAFFIC_BYTES, "algorithmic_bytes_per_launch": step_bytes,
-                     "ms_per_launch": ms_kernel},
-        "kernels_ms": {"fused_step": ms_kernel, "two_kernel_path": {"evolve": ms_evolve, "events": ms_events}},
+                     "traffic": EVOLVE_DRAM_TRAFFIC_BYTES, "algorithmic_bytes_per_launch": evolve_bytes,
+                     "ms_per_launch": ms_evolve, "share_of_step": ms_evolve * args.steps / ms_total},
+        "kernels_ms": {"qed_step": {"evolve_pass": ms_evolve, "event_pass": ms_events},
+                       "two_call_path": {"evolve_optical_depth": ms_evolve2, "generate_photons": ms_events2}},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": args.e2e_steps},
-        "gpu_launches": args.steps,
+        "gpu_launches": 4 * args.steps,
         "clocks": sampler.summary(),
     }
     if not args.no_cpu_baseline and world == 1:

@@ -79,8 +79,14 @@ const char* picsarqed_last_error(const picsarqed_ctx* ctx);
 /* bit 0: library was compiled for sm_100a; returns the CUDA runtime version in the upper bits */
 int picsarqed_version(void);
 /* Tuning knobs (integers): "evolve_unroll" in {0 (default), 1, 2, 4} = independent 128-bit
- * loads per array per thread in the evolve kernel; "evolve_ctas_per_sm" (0 = occupancy limit). */
+ * loads per array per thread in the evolve kernel; "evolve_ctas_per_sm" (0 = occupancy limit);
+ * "event_config" 0..7 = (threads, chunks per tile) of the event kernel; "time_kernels" 0/1. */
 int picsarqed_set_option(picsarqed_ctx* ctx, const char* name, long long value);
+/* With "time_kernels" = 1 every qed_step brackets its evolve pass and its event pass (offsets scan +
+ * event kernel) with CUDA events on the context's stream.  get_timing synchronises, writes the
+ * accumulated milliseconds host_ms[0] (evolve pass) and host_ms[1] (event pass) and the number of
+ * qed_step calls they cover, and resets the accumulation. */
+int picsarqed_get_timing(picsarqed_ctx* ctx, double* host_ms, long long* host_calls);
 
 /* ---- tables -------------------------------------------------------------------------
  * build_tables: integrates on the GPU, in fp64,

@@ -52,6 +52,7 @@ _SIGNATURES = {
     "picsarqed_destroy": (_i, [_vp]),
     "picsarqed_last_error": (C.c_char_p, [_vp]),
     "picsarqed_set_option": (_i, [_vp, C.c_char_p, _i64]),
+    "picsarqed_get_timing": (_i, [_vp, C.POINTER(_d), C.POINTER(_i64)]),
     "picsarqed_build_tables": (_i, [_vp, C.POINTER(_CParams), _d]),
     "picsarqed_export_tables": (_i, [_vp, _i, _vp, C.c_size_t]),
     "picsarqed_import_tables": (_i, [_vp, C.POINTER(_CParams), _vp, _vp, _vp, _vp]),
@@ -138,6 +139,13 @@ class Context:
     # ---- options / tables ---------------------------------------------------------------
     def set_option(self, name, value):
         self._check(lib().picsarqed_set_option(self._h, name.encode(), int(value)))
+
+    def get_timing(self):
+        """(evolve-pass ms, event-pass ms, calls) accumulated by qed_step since the last call ("time_kernels" = 1)"""
+        ms = (_d * 2)()
+        calls = _i64(0)
+        self._check(lib().picsarqed_get_timing(self._h, ms, C.byref(calls)))
+        return float(ms[0]), float(ms[1]), int(calls.value)
 
     def build_tables(self, params, rel_tol=0.0):
         cp = params._c()

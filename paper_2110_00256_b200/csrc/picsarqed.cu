@@ -40,6 +40,8 @@ struct picsarqed_ctx {
     int evolve_unroll = 0;       // 0 = default per dtype
     int evolve_ctas_per_sm = 0;  // 0 = occupancy
     int event_config = 0;        // shape of event_kernel: see launch_event_pass
+    int time_kernels = 0;        // qed_step brackets its evolve pass and its event pass with CUDA events
+    std::vector<cudaEvent_t> timing_events;  // triples (start, after evolve, after events), not yet read
     // per-chunk scratch of the event path: staged records, counts, output offsets (see events.cuh)
     void* rec = nullptr;
     size_t rec_bytes = 0;
@@ -267,6 +269,7 @@ int picsarqed_destroy(picsarqed_ctx* c) {
     cudaFree(c->guide[0]);
     cudaFree(c->guide[1]);
     cudaFree(c->d_scalar);
+    for (cudaEvent_t e : c->timing_events) cudaEventDestroy(e);
     cudaFree(c->d_counts);
     delete c;
     return PICSARQED_OK;
@@ -280,10 +283,30 @@ int picsarqed_set_option(picsarqed_ctx* c, const char* name, long long value) {
         c->evolve_unroll = (int)value;
     else if (!std::strcmp(name, "evolve_ctas_per_sm") && value >= 0 && value <= 32)
         c->evolve_ctas_per_sm = (int)value;
+    else if (!std::strcmp(name, "time_kernels") && (value == 0 || value == 1))
+        c->time_kernels = (int)value;
     else if (!std::strcmp(name, "event_config") && value >= 0 && value <= 7)
         c->event_config = (int)value;
     else
         return fail(c, PICSARQED_ERR_INVALID, std::string("unknown option or bad value: ") + name);
+    return PICSARQED_OK;
+}
+
+int picsarqed_get_timing(picsarqed_ctx* c, double* host_ms, long long* host_calls) {
+    if (!c || !host_ms || !host_calls) return PICSARQED_ERR_INVALID;
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    host_ms[0] = host_ms[1] = 0.0;
+    *host_calls = (long long)(c->timing_events.size() / 3);
+    for (size_t k = 0; k + 2 < c->timing_events.size(); k += 3) {
+        float a = 0.f, b = 0.f;
+        cudaEventElapsedTime(&a, c->timing_events[k], c->timing_events[k + 1]);
+        cudaEventElapsedTime(&b, c->timing_events[k + 1], c->timing_events[k + 2]);
+        host_ms[0] += a;
+        host_ms[1] += b;
+    }
+    for (cudaEvent_t e : c->timing_events) cudaEventDestroy(e);
+    c->timing_events.clear();
     return PICSARQED_OK;
 }
 
@@ -493,9 +516,21 @@ int launch_step(picsarqed_ctx* c, long long n, void* const* p, const void* const
     sv.cnt = cs.cnt;
     const void* a9[9] = {p[0], p[1], p[2], eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]};
     constexpr int U = kChunk / (32 * (16 / (int)sizeof(R)));  // fp64: 2, fp32: 1
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    if (c->time_kernels) {
+        for (int k = 0; k < 3; ++k) PXQ_CUDA(c, cudaEventCreate(&ev[k]));
+        PXQ_CUDA(c, cudaEventRecord(ev[0], c->stream));
+    }
     if (int rc = launch_evolve_u<R, TR, SPECIES, U, true>(c, n, a9, dt, tau, nullptr, sv)) return rc;
-    return launch_event_pass<R, TR, SPECIES>(c, n, cs, p, eb, tau, seed, step, id_base, capacity, out_p, out_tau, parent,
-                                             d_n_out);
+    if (c->time_kernels) PXQ_CUDA(c, cudaEventRecord(ev[1], c->stream));
+    if (int rc = launch_event_pass<R, TR, SPECIES>(c, n, cs, p, eb, tau, seed, step, id_base, capacity, out_p, out_tau,
+                                                   parent, d_n_out))
+        return rc;
+    if (c->time_kernels) {
+        PXQ_CUDA(c, cudaEventRecord(ev[2], c->stream));
+        for (int k = 0; k < 3; ++k) c->timing_events.push_back(ev[k]);
+    }
+    return PICSARQED_OK;
 }
 
 // dispatch on (dtype, tau_dtype); fp64 particles with fp32 optical depth is not offered
