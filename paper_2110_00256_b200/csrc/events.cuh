@@ -234,11 +234,24 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
     __shared__ unsigned char list[CHUNKS][kChunk];  // re-scanned chunks: local indices of the fired particles
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const long long first_chunk = (long long)blockIdx.x * CHUNKS;
     const long long n_chunks = (a.n + kChunk - 1) / kChunk;
-    const bool real = lane < CHUNKS && first_chunk + lane < n_chunks;
-    const unsigned short flags = real ? a.stage_cnt[first_chunk + lane] : (unsigned short)0;
-    const unsigned long long excl = a.tile_offset[blockIdx.x];            // output slot of the tile's first event
+    const long long n_tiles = (n_chunks + CHUNKS - 1) / CHUNKS;
+    // Persistent CTAs stride over the tiles.  The warps of a CTA walk the same tiles in the same order but do
+    // not wait for one another (no barrier on the common path): a warp whose slice of a tile holds no event is
+    // already loading the next tile.  The loads of the next tile are issued before the current one is processed.
+    auto load_flags = [&](long long tile) -> unsigned short {
+        const long long ch = tile * CHUNKS + lane;
+        return (tile < n_tiles && lane < CHUNKS && ch < n_chunks) ? a.stage_cnt[ch] : (unsigned short)0;
+    };
+    long long tile = blockIdx.x;
+    unsigned short flags_next = load_flags(tile);
+    unsigned long long excl_next = tile < n_tiles ? a.tile_offset[tile] : 0ull;
+    for (; tile < n_tiles; tile += gridDim.x) {
+    const long long first_chunk = tile * CHUNKS;
+    const unsigned short flags = flags_next;
+    const unsigned long long excl = excl_next;                            // output slot of the tile's first event
+    flags_next = load_flags(tile + gridDim.x);
+    excl_next = tile + gridDim.x < n_tiles ? a.tile_offset[tile + gridDim.x] : 0ull;
     const unsigned int cnt = flags & kStageCountMask;
     unsigned int incl = cnt;                                             // offsets of the chunks inside the tile
 #pragma unroll
@@ -248,10 +261,11 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
     }
     const unsigned int off_lane = incl - cnt;
     const unsigned int total = __shfl_sync(0xffffffffu, incl, 31);
-    if (total == 0) return;
+    if (total == 0) continue;
     const unsigned int rescan_mask =
         __ballot_sync(0xffffffffu, cnt > 0 && (cnt > (unsigned)kStageCap || (flags & kStageNoRecords) != 0));
     if (rescan_mask) {  // chunks without records: find their fired particles again (tau < 0), in index order
+        __syncthreads();  // (every warp is done with the list of the previous tile that needed one)
         for (int j = warp; j < CHUNKS; j += WARPS) {
             if (!((rescan_mask >> j) & 1u)) continue;
             const long long cbase = (first_chunk + j) * kChunk;
@@ -305,6 +319,7 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
                                               : bw_event_compute<R, TR>(a, i, px, py, pz, ex, ey, ez, bx, by, bz);
         event_commit<R, TR, KIND>(a, i, slot, out);
     }
+    }  // tiles
 }
 
 }  // namespace pxq

@@ -470,23 +470,32 @@ int launch_event_pass(picsarqed_ctx* c, long long n, const ChunkScratch& cs, voi
     ev.stage_rec = cs.rec;
     ev.stage_cnt = cs.cnt;
     ev.tile_offset = cs.off;
-    static const int kChunksOf[8] = {24, 32, 24, 16, 12, 20, 8, 32};  // must match the switch below
+    static const int kChunksOf[8] = {24, 32, 24, 16, 12, 24, 24, 32};  // must match the switch below
     const int chunks = kChunksOf[c->event_config];
     const long long n_tiles = (cs.n_chunks + chunks - 1) / chunks;
-    const unsigned grid = (unsigned)n_tiles;
     const int sum_grid = (int)std::max<long long>(1, std::min<long long>((n_tiles + 7) / 8, (long long)c->num_sms * 8));
     tile_sums_kernel<TR><<<sum_grid, 256, 0, c->stream>>>(cs.cnt, cs.n_chunks, chunks, n_tiles, (const TR*)tau, n, cs.sum);
     tile_scan_kernel<<<1, kScanThreads, 0, c->stream>>>(cs.sum, n_tiles, cs.off, d_n_out);
+#define PXQ_LAUNCH_EVENTS(T, CH, MB)                                                                         \
+    do {                                                                                                     \
+        auto kern = event_kernel<R, TR, KIND, T, CH, MB>;                                                    \
+        int per_sm = 0;                                                                                      \
+        PXQ_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, T, 0));                     \
+        const unsigned grid = (unsigned)std::max<long long>(                                                 \
+            1, std::min<long long>(n_tiles, (long long)c->num_sms * std::max(per_sm, 1)));                   \
+        kern<<<grid, T, 0, c->stream>>>(ev);                                                                 \
+    } while (0)
     switch (c->event_config) {
-        case 1: event_kernel<R, TR, KIND, 256, 32, 3><<<grid, 256, 0, c->stream>>>(ev); break;
-        case 2: event_kernel<R, TR, KIND, 256, 24, 4><<<grid, 256, 0, c->stream>>>(ev); break;
-        case 3: event_kernel<R, TR, KIND, 256, 16, 4><<<grid, 256, 0, c->stream>>>(ev); break;
-        case 4: event_kernel<R, TR, KIND, 128, 12, 8><<<grid, 128, 0, c->stream>>>(ev); break;
-        case 5: event_kernel<R, TR, KIND, 256, 20, 4><<<grid, 256, 0, c->stream>>>(ev); break;
-        case 6: event_kernel<R, TR, KIND, 128, 8, 8><<<grid, 128, 0, c->stream>>>(ev); break;
-        case 7: event_kernel<R, TR, KIND, 384, 32, 2><<<grid, 384, 0, c->stream>>>(ev); break;
-        default: event_kernel<R, TR, KIND, 256, 24, 3><<<grid, 256, 0, c->stream>>>(ev); break;
+        case 1: PXQ_LAUNCH_EVENTS(256, 32, 3); break;
+        case 2: PXQ_LAUNCH_EVENTS(256, 24, 4); break;
+        case 3: PXQ_LAUNCH_EVENTS(256, 16, 4); break;
+        case 4: PXQ_LAUNCH_EVENTS(128, 12, 8); break;
+        case 5: PXQ_LAUNCH_EVENTS(256, 24, 5); break;
+        case 6: PXQ_LAUNCH_EVENTS(256, 24, 6); break;
+        case 7: PXQ_LAUNCH_EVENTS(384, 32, 2); break;
+        default: PXQ_LAUNCH_EVENTS(256, 24, 3); break;
     }
+#undef PXQ_LAUNCH_EVENTS
     PXQ_CUDA(c, cudaGetLastError());
     return PICSARQED_OK;
 }
