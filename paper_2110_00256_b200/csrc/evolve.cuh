@@ -99,11 +99,28 @@ __device__ __forceinline__ auto decrement_one(R pxr, R pyr, R pzr, R exr, R eyr,
         // eq.8 with T from eq.23; Erber form outside; gamma_gamma <= 2 cannot decay (R12)
         if (!(g2 > 4.0) || !(c2 > 0.0)) return (A)0;
         if (c2 < T.chi_min * T.chi_min || c2 > T.chi_max * T.chi_max) {
-            const double chi = sqrt(c2);
-            const double x = 4.0 / (3.0 * chi);
-            const double lk = ln_bessel_k13_scaled(x);                 // ln K_{1/3}(x) + x
-            const double d = rate_dt * 0.16 * exp(2.0 * (lk - x)) * inv_g;  // chi T = 0.16 K^2
-            return (A)d;
+            // chi T = 0.16 K_{1/3}(x)^2, x = 4/(3 chi) (eq.10 with the argument of DESIGN.md R2)
+            if (c2 < 1.7777e-4) return (A)0;  // x > 100: K^2 < e^-200, the decrement is below 1e-80 of any optical depth
+            double k2;                        // K_{1/3}(x)^2
+            if (c2 > 7.2e2) {                 // x < 0.05
+                // ascending series (DLMF 10.27.4, 10.25.2), four terms: relative error < (x^2/4)^4 < 2e-13.
+                // K = (pi/sqrt3) (sm/h - sp h), h = (x/2)^(1/3); with y = x^2/4 = 4/(9 chi^2): h^2 = cbrt(y)
+                // (coefficients 1/(k (k -+ nu)) are written as constants: no divisions in the series)
+                const double y = (4.0 / 9.0) / c2;
+                constexpr double am1 = 1.0 / (1.0 * (1.0 - 1.0 / 3.0)), am2 = 1.0 / (2.0 * (2.0 - 1.0 / 3.0)),
+                                 am3 = 1.0 / (3.0 * (3.0 - 1.0 / 3.0));
+                constexpr double ap1 = 1.0 / (1.0 * (1.0 + 1.0 / 3.0)), ap2 = 1.0 / (2.0 * (2.0 + 1.0 / 3.0)),
+                                 ap3 = 1.0 / (3.0 * (3.0 + 1.0 / 3.0));
+                const double sm = (1.0 / 1.3541179394264004) * fma(y * am1, fma(y * am2, fma(y, am3, 1.0), 1.0), 1.0);
+                const double sp = (1.0 / 0.8929795115692492) * fma(y * ap1, fma(y * ap2, fma(y, ap3, 1.0), 1.0), 1.0);
+                const double h2 = cbrt(y);
+                const double k = sm - sp * h2;  // K h sqrt3/pi
+                k2 = (1.5707963267948966 / 0.8660254037844386) * (1.5707963267948966 / 0.8660254037844386) * k * k / h2;
+            } else {
+                const double x = 4.0 / (3.0 * sqrt(c2));
+                k2 = exp(2.0 * (ln_bessel_k13_scaled(x) - x));
+            }
+            return (A)(rate_dt * 0.16 * k2 * inv_g);
         }
         lc = fmin(fmax(lc, ln_min), ln_max);
         const A L = lookup_ln<R, A>(tab, T.n, lc, ln_min, inv_delta);
