@@ -83,17 +83,17 @@ __device__ __forceinline__ auto decrement_one(R pxr, R pyr, R pzr, R exr, R eyr,
     const double px = pxr, py = pyr, pz = pzr;
     const double p2 = fma(px, px, fma(py, py, pz * pz));
     const double g2 = SPECIES == 0 ? 1.0 + p2 : p2;
-    const double inv_g = rsqrt(g2);       // 1/gamma (lepton) or 1/gamma_gamma (photon)
+    const double inv_g = g2 > 1e-300 ? rsqrt_fast(g2) : 0.0;  // 1/gamma (lepton) or 1/gamma_gamma (photon)
     const double g = g2 * inv_g;
     const double c2 = chi_squared<SPECIES>(px, py, pz, exr, eyr, ezr, bxr, byr, bzr, g, p2);
     A lc;
-    if constexpr (sizeof(R) == 8) lc = 0.5 * log(c2); else lc = 0.5f * logf((float)c2);
+    if constexpr (sizeof(R) == 8) lc = 0.5 * log_pos(c2); else lc = 0.5f * logf((float)c2);
     const A ln_min = (A)T.ln_min, ln_max = (A)T.ln_max, inv_delta = (A)T.inv_delta;
     if (SPECIES == 0) {
         // eq.15 with G from eq.27; first/last value outside the table
-        lc = fmin(fmax(lc, ln_min), ln_max);
+        lc = lc < ln_min ? ln_min : (lc > ln_max ? ln_max : lc);
         const A L = lookup_ln<R, A>(tab, T.n, lc, ln_min, inv_delta);
-        if constexpr (sizeof(R) == 8) return rate_dt * exp(L) * inv_g;
+        if constexpr (sizeof(R) == 8) return rate_dt * exp_fast(L) * inv_g;
         else return (float)rate_dt * expf(L) * (float)inv_g;
     } else {
         // eq.8 with T from eq.23; Erber form outside; gamma_gamma <= 2 cannot decay (R12)
@@ -122,9 +122,9 @@ __device__ __forceinline__ auto decrement_one(R pxr, R pyr, R pzr, R exr, R eyr,
             }
             return (A)(rate_dt * 0.16 * k2 * inv_g);
         }
-        lc = fmin(fmax(lc, ln_min), ln_max);
+        lc = lc < ln_min ? ln_min : (lc > ln_max ? ln_max : lc);
         const A L = lookup_ln<R, A>(tab, T.n, lc, ln_min, inv_delta);
-        if constexpr (sizeof(R) == 8) return rate_dt * exp(L + lc) * inv_g;
+        if constexpr (sizeof(R) == 8) return rate_dt * exp_fast(L + lc) * inv_g;
         else return (float)rate_dt * expf(L + lc) * (float)inv_g;
     }
 }

@@ -93,6 +93,77 @@ template <> __device__ __forceinline__ float draw_tau<float>(uint32_t a, uint32_
     return -logf(uniform_open<float>(a, b));
 }
 
+// ---- lean fp64 elementary functions for the streaming kernel ------------------------------------
+// The CUDA library log/exp cost ~85 / ~50 instructions per call (special cases, constant moves); in the evolve
+// kernel they were 45 % of all instructions (profiles/r1b_step_full.md).  These versions assume what holds
+// there -- log of a positive normal number (anything else takes the library path), exp of a finite argument --
+// and keep the error at the 1e-16 level: a few ulp, far inside the 1e-9 tolerance on the optical depth.
+__device__ __forceinline__ double rcp_fast(double x) {        // 1/x for normal x, ~1 ulp
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));     // ~20 bits
+    r = fma(fma(-x, r, 1.0), r, r);                           // ~40 bits
+    return fma(fma(-x, r, 1.0), r, r);                        // ~80 bits -> rounded
+}
+__device__ __forceinline__ double rsqrt_fast(double x) {      // 1/sqrt(x) for normal x > 0, ~1 ulp
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));   // ~20 bits
+    const double hx = 0.5 * x;
+    y = fma(fma(-hx * y, y, 0.5), y, y);
+    return fma(fma(-hx * y, y, 0.5), y, y);
+}
+__device__ __forceinline__ double log_pos(double x) {
+    int hi = __double2hiint(x);
+    const int lo = __double2loint(x);
+    if ((unsigned)(hi - 0x00100000) >= 0x7fe00000u) return log(x);  // zero, denormal, inf, nan, negative
+    int e = (hi >> 20) - 1023;
+    hi = (hi & 0x000fffff) | 0x3ff00000;                     // mantissa in [1, 2)
+    if (hi >= 0x3ff6a09e) { hi -= 0x00100000; e += 1; }      // -> [sqrt(1/2), sqrt(2))
+    const double m = __hiloint2double(hi, lo);
+    const double num = m - 1.0, den = m + 1.0;
+    const double r = rcp_fast(den);
+    double s = num * r;
+    s = fma(fma(-s, den, num), r, s);                        // s = (m-1)/(m+1), |s| <= 0.1716
+    const double s2 = s * s;
+    // ln m = 2 atanh(s) = 2 s (1 + s^2/3 + s^4/5 + ... + s^18/19); the first dropped term is < 3e-17
+    double p = 1.0 / 19.0;
+    p = fma(p, s2, 1.0 / 17.0);
+    p = fma(p, s2, 1.0 / 15.0);
+    p = fma(p, s2, 1.0 / 13.0);
+    p = fma(p, s2, 1.0 / 11.0);
+    p = fma(p, s2, 1.0 / 9.0);
+    p = fma(p, s2, 1.0 / 7.0);
+    p = fma(p, s2, 1.0 / 5.0);
+    p = fma(p, s2, 1.0 / 3.0);
+    const double two_s = s + s;
+    const double lnm = fma(two_s * s2, p, two_s);
+    const double ed = (double)e;
+    return fma(ed, 6.93147180369123816490e-01, fma(ed, 1.90821492927058770002e-10, lnm));  // e ln2 (hi + lo)
+}
+__device__ __forceinline__ double exp_fast(double x) {
+    if (!(x > -707.0)) return x < 0.0 ? 0.0 : x;             // underflow (or nan)
+    x = x > 709.0 ? 709.0 : x;
+    const double t = fma(x, 1.4426950408889634074, 6755399441055744.0);  // k = rint(x log2 e) in the low word
+    const int k = __double2loint(t);
+    const double kd = t - 6755399441055744.0;
+    double r = fma(kd, -6.93147180369123816490e-01, x);
+    r = fma(kd, -1.90821492927058770002e-10, r);             // |r| <= 0.3466
+    double p = 1.0 / 6227020800.0;                           // Taylor to r^13/13!: remainder < 2e-17
+    p = fma(p, r, 1.0 / 479001600.0);
+    p = fma(p, r, 1.0 / 39916800.0);
+    p = fma(p, r, 1.0 / 3628800.0);
+    p = fma(p, r, 1.0 / 362880.0);
+    p = fma(p, r, 1.0 / 40320.0);
+    p = fma(p, r, 1.0 / 5040.0);
+    p = fma(p, r, 1.0 / 720.0);
+    p = fma(p, r, 1.0 / 120.0);
+    p = fma(p, r, 1.0 / 24.0);
+    p = fma(p, r, 1.0 / 6.0);
+    p = fma(p, r, 0.5);
+    p = fma(p, r, 1.0);
+    p = fma(p, r, 1.0);
+    return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));  // p 2^k, k in [-1021, 1023]
+}
+
 // ---- chi^2 --------------------------------------------------------------------------
 // eq.2 / eq.3: chi^2 = |g e + p x b|^2 - (p.e)^2.  Taken literally the two terms cancel by
 // up to gamma^2 when e has a component along p, so it is evaluated in the equivalent form
@@ -103,7 +174,7 @@ template <int SPECIES>
 __device__ __forceinline__ double chi_squared(double px, double py, double pz, double ex, double ey, double ez,
                                               double bx, double by, double bz, double g, double p2) {
     const double d = fma(px, ex, fma(py, ey, pz * ez));  // p.e
-    const double q = p2 > 0.0 ? 1.0 / p2 : 0.0;
+    const double q = p2 > 1e-300 ? rcp_fast(p2) : 0.0;
     const double t = d * q;
     const double fx = fma(-t, px, ex), fy = fma(-t, py, ey), fz = fma(-t, pz, ez);  // e_perp
     const double cx = fma(py, bz, -pz * by), cy = fma(pz, bx, -px * bz), cz = fma(px, by, -py * bx);

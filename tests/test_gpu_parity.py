@@ -403,3 +403,26 @@ def test_fused_step_repeated_launches(qed, ctx):
         assert k == int((sec_tau != -7.0).sum().item()) and bool((sec_tau[:k] > 0).all())  # dense, nothing past the count
         assert bool((tau >= 0).all())                                                      # every fired parent was re-drawn
     assert sum(counts) > 0
+
+
+@pytest.mark.parametrize("species", [LEPTON, PHOTON])
+def test_evolve_decrement_accuracy_fp64(orc, qed, ctx, mid_tables, species):
+    """the decrement itself (tau_old = 0), far tighter than the 1e-9 of the north star: the kernel uses its own lean
+    log/exp/rcp/rsqrt, whose errors must stay at the few-ulp level; the bound is the conditioning of the lookup"""
+    import torch
+    n = 50000
+    p, e, b = qed.workloads.config1(seed=41, n=n, species=species)
+    dt = 1e-17
+    tau = torch.zeros(n, dtype=torch.float64, device="cuda")
+    ctx.evolve_optical_depth(species, to_dev(p), to_dev(e), to_dev(b), dt, tau)
+    o = orc.evolve_optical_depth(mid_tables, species, F64, p, e, b, dt, np.zeros(n))
+    d_gpu, d_orc = -tau.cpu().numpy(), o["decr"]
+    ln_chi = np.log(np.maximum(orc.chi(species, p, e, b), 1e-300))
+    ok = d_orc > 1e-80   # below: photons far under the T table, where the kernel returns exactly 0 (K^2 < e^-200)
+    rel = np.abs(d_gpu[ok] - d_orc[ok]) / d_orc[ok]
+    from parity_common import uncancelled_scale
+    chi_cond = uncancelled_scale(species, p, e, b)[ok] / np.exp(ln_chi[ok])       # conditioning of eq.2 itself
+    bound = 2.2e-16 * (32 + np.abs(o["slope"][ok]) * (8 + 2 * np.abs(ln_chi[ok]) + 8 * chi_cond) + 4 * np.abs(o["lnval"][ok]))
+    bad = np.nonzero(rel > bound)[0]
+    assert bad.size == 0, (rel[bad[:5]], bound[bad[:5]])
+    assert np.all(d_gpu[~ok] <= 1.0000001 * d_orc[~ok])
