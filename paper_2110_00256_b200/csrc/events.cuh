@@ -53,11 +53,9 @@ struct EventOut {
 // ---- photon emission by one lepton ------------------------------
 template <typename R, typename TR>
 __device__ __forceinline__ EventOut<R, TR> qs_event_compute(const EventArgs<R, TR>& a, long long i, double px, double py,
-                                                            double pz, double ex, double ey, double ez, double bx,
-                                                            double by, double bz) {
+                                                            double pz, double c2) {
     const double p2 = fma(px, px, fma(py, py, pz * pz));
     const double g = sqrt(1.0 + p2);
-    const double c2 = chi_squared<0>(px, py, pz, ex, ey, ez, bx, by, bz, g, p2);
     const unsigned long long id = a.id_base + (unsigned long long)i;
     const Words4 w = qed_words(a.seed, id, a.step, 1, 0);
     const Words4 wc = qed_words(a.seed, id, a.step, 2, 0);
@@ -87,11 +85,9 @@ __device__ __forceinline__ EventOut<R, TR> qs_event_compute(const EventArgs<R, T
 // ---- pair production by one photon -----------------------------
 template <typename R, typename TR>
 __device__ __forceinline__ EventOut<R, TR> bw_event_compute(const EventArgs<R, TR>& a, long long i, double px, double py,
-                                                            double pz, double ex, double ey, double ez, double bx,
-                                                            double by, double bz) {
+                                                            double pz, double c2) {
     const double p2 = fma(px, px, fma(py, py, pz * pz));
     const double g = sqrt(p2);                  // gamma_gamma = |p|
-    const double c2 = chi_squared<1>(px, py, pz, ex, ey, ez, bx, by, bz, g, p2);
     const unsigned long long id = a.id_base + (unsigned long long)i;
     const Words4 w = qed_words(a.seed, id, a.step, 1, 1);
     const Words4 wc = qed_words(a.seed, id, a.step, 2, 1);
@@ -117,6 +113,14 @@ __device__ __forceinline__ EventOut<R, TR> bw_event_compute(const EventArgs<R, T
     o.parent_p[0] = o.parent_p[1] = o.parent_p[2] = (R)0;   // photon removed: p = 0, tau = +inf
     o.parent_tau = (TR)INFINITY;
     return o;
+}
+
+// chi^2 of a parent gathered from the particle arrays (chunks without staged records)
+template <int KIND>
+__device__ __forceinline__ double event_c2(double px, double py, double pz, double ex, double ey, double ez, double bx,
+                                           double by, double bz) {
+    double inv_g, g2;
+    return chi_squared_of<KIND>(px, py, pz, ex, ey, ez, bx, by, bz, &inv_g, &g2);
 }
 
 template <typename R, typename TR, int KIND>
@@ -297,26 +301,25 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
         if (e >= total || slot >= a.capacity) continue;  // capacity rule (R16): later parents untouched
         const unsigned int r = e - off_j;
         const long long cbase = (first_chunk + j) * kChunk;
-        double px, py, pz, ex, ey, ez, bx, by, bz;
+        const bool staged = !((rescan_mask >> j) & 1u);
+        double px, py, pz, c2;
         long long i;
-        if ((rescan_mask >> j) & 1u) {
-            i = cbase + list[j][r];
-            px = a.p[0][i]; py = a.p[1][i]; pz = a.p[2][i];
-            ex = a.e[0][i]; ey = a.e[1][i]; ez = a.e[2][i];
-            bx = a.b[0][i]; by = a.b[1][i]; bz = a.b[2][i];
-        } else {
-            constexpr int NV = StageRecord<R>::kVecs;
+        if (staged) {
             const uint4* src = reinterpret_cast<const uint4*>(
                 a.stage_rec + ((first_chunk + j) * (long long)kStageCap + r) * StageRecord<R>::kBytes);
-            uint4 raw[NV];
+            union { uint4 raw[StageRecord<R>::kVecs]; StageRecord<R> rec; } u;
 #pragma unroll
-            for (int k = 0; k < NV; ++k) raw[k] = __ldg(src + k);
-            const R* w = reinterpret_cast<const R*>(raw);
-            px = w[0]; py = w[1]; pz = w[2]; ex = w[3]; ey = w[4]; ez = w[5]; bx = w[6]; by = w[7]; bz = w[8];
-            i = cbase + *reinterpret_cast<const unsigned int*>(&w[9]);
+            for (int k = 0; k < StageRecord<R>::kVecs; ++k) u.raw[k] = __ldg(src + k);
+            px = u.rec.p[0]; py = u.rec.p[1]; pz = u.rec.p[2];
+            c2 = u.rec.c2;
+            i = cbase + u.rec.idx;
+        } else {
+            i = cbase + list[j][r];
+            px = a.p[0][i]; py = a.p[1][i]; pz = a.p[2][i];
+            c2 = event_c2<KIND>(px, py, pz, a.e[0][i], a.e[1][i], a.e[2][i], a.b[0][i], a.b[1][i], a.b[2][i]);
         }
-        const EventOut<R, TR> out = KIND == 0 ? qs_event_compute<R, TR>(a, i, px, py, pz, ex, ey, ez, bx, by, bz)
-                                              : bw_event_compute<R, TR>(a, i, px, py, pz, ex, ey, ez, bx, by, bz);
+        const EventOut<R, TR> out = KIND == 0 ? qs_event_compute<R, TR>(a, i, px, py, pz, c2)
+                                              : bw_event_compute<R, TR>(a, i, px, py, pz, c2);
         event_commit<R, TR, KIND>(a, i, slot, out);
     }
     }  // tiles

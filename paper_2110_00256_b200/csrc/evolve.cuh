@@ -41,13 +41,20 @@ constexpr unsigned short kStageCountMask = 0x7FFFu;
 constexpr unsigned short kStageNoRecords = 0x8000u;
 constexpr unsigned short kStageUnknown = 0xFFFFu;
 
-// one staged record: px,py,pz, ex,ey,ez, bx,by,bz of a particle that fired + its index inside the chunk,
-// padded to a multiple of 16 bytes (fp64: 80 B, fp32: 48 B) so that records move as 128-bit vectors
-template <typename R> struct StageRecord {
-    static constexpr int kWords = sizeof(R) == 8 ? 10 : 12;          // in units of R
-    static constexpr int kBytes = kWords * (int)sizeof(R);
-    static constexpr int kVecs = kBytes / 16;
+// one staged record: what event generation needs of a particle that fired -- its momentum, chi^2 (computed by the
+// evolve pass anyway) and its index inside the chunk.  Sizes are multiples of 16 bytes so that records move as
+// 128-bit vectors.  (Also staging the fields, 80 B, and letting the evolve pass re-draw the parent's optical depth
+// were both measured: each made the evolve pass slower by more than the event pass gained.)
+template <typename R> struct StageRecord;
+template <> struct alignas(16) StageRecord<double> {
+    double p[3]; double c2; unsigned idx; unsigned pad[3];
+    static constexpr int kBytes = 48, kVecs = 3;
 };
+template <> struct alignas(16) StageRecord<float> {
+    float p[3]; unsigned idx; double c2; double pad;
+    static constexpr int kBytes = 32, kVecs = 2;
+};
+static_assert(sizeof(StageRecord<double>) == 48 && sizeof(StageRecord<float>) == 32, "record layout");
 
 // ---- TMA bulk copy of a 1D table into shared memory ------------------------------------
 __device__ __forceinline__ void stage_table_tma(void* smem_dst, const void* gmem_src, unsigned bytes,
@@ -78,14 +85,12 @@ __device__ __forceinline__ void stage_table_tma(void* smem_dst, const void* gmem
 // Returns the decrement dN/dt * dt in the particle arithmetic type A (float or double).
 template <typename R, int SPECIES>
 __device__ __forceinline__ auto decrement_one(R pxr, R pyr, R pzr, R exr, R eyr, R ezr, R bxr, R byr, R bzr,
-                                              const R* tab, const Table1D<R>& T, double rate_dt) -> R {
+                                              const R* tab, const Table1D<R>& T, double rate_dt,
+                                              double* c2_out = nullptr) -> R {
     typedef R A;
-    const double px = pxr, py = pyr, pz = pzr;
-    const double p2 = fma(px, px, fma(py, py, pz * pz));
-    const double g2 = SPECIES == 0 ? 1.0 + p2 : p2;
-    const double inv_g = g2 > 1e-300 ? rsqrt_fast(g2) : 0.0;  // 1/gamma (lepton) or 1/gamma_gamma (photon)
-    const double g = g2 * inv_g;
-    const double c2 = chi_squared<SPECIES>(px, py, pz, exr, eyr, ezr, bxr, byr, bzr, g, p2);
+    double inv_g, g2;
+    const double c2 = chi_squared_of<SPECIES>(pxr, pyr, pzr, exr, eyr, ezr, bxr, byr, bzr, &inv_g, &g2);
+    if (c2_out) *c2_out = c2;
     A lc;
     if constexpr (sizeof(R) == 8) lc = 0.5 * log_pos(c2); else lc = 0.5f * logf((float)c2);
     const A ln_min = (A)T.ln_min, ln_max = (A)T.ln_max, inv_delta = (A)T.inv_delta;
@@ -135,7 +140,7 @@ __device__ __forceinline__ auto decrement_one(R pxr, R pyr, R pzr, R exr, R eyr,
 // EMIT: also append the nine reals of every particle that fired to the staging segment of its 128-particle
 // chunk, in index order (warp ballot/popc; no CTA barrier), for staged_event_kernel.  Requires U*32*V == kChunk.
 template <typename R, typename TR, int SPECIES, int U, bool EMIT>
-__global__ void __launch_bounds__(kEvolveThreads)
+__global__ void __launch_bounds__(kEvolveThreads, U <= 2 ? 2 : 1)
 evolve_kernel(const EvolveArgs<R, TR> a) {
     constexpr int V = 16 / sizeof(R);
     constexpr int TILE = kEvolveThreads * V * U;
@@ -176,20 +181,20 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                 t[u] = ld_stream_rw<TR, V>(a.tau + i, pol_stream);
             }
             unsigned int fired_bits = 0;
+            double c2s[EMIT ? U * V : 1];
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const long long i = base + (long long)warp * WCH + (u * 32 + lane) * V;
 #pragma unroll
                 for (int v = 0; v < V; ++v) {
                     const R d = decrement_one<R, SPECIES>(q[0][u].v[v], q[1][u].v[v], q[2][u].v[v], q[3][u].v[v],
                                                           q[4][u].v[v], q[5][u].v[v], q[6][u].v[v], q[7][u].v[v],
-                                                          q[8][u].v[v], tab, a.tab, a.rate_dt);
+                                                          q[8][u].v[v], tab, a.tab, a.rate_dt,
+                                                          EMIT ? &c2s[EMIT ? u * V + v : 0] : nullptr);
                     const TR tn = t[u].v[v] - (TR)d;
                     t[u].v[v] = tn;
                     fired += tn < (TR)0 ? 1u : 0u;
                     if (EMIT && tn < (TR)0) fired_bits |= 1u << (u * V + v);
                 }
-                *reinterpret_cast<Vec<TR, V>*>(a.tau + i) = t[u];
             }
             if constexpr (EMIT) {
                 // rank inside the warp's chunk, in index order (u, lane, v): ballot / popc
@@ -211,19 +216,21 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                 if (lane == 0)
                     a.stage_cnt[chunk] = (unsigned short)(total <= (unsigned)kStageCap ? total : (total | kStageNoRecords));
                 if (total > 0 && total <= (unsigned)kStageCap) {  // (overflow: the event kernel re-scans the chunk)
-                    // records are assembled in this warp's shared-memory buffer (scattered 8-byte writes are
-                    // cheap there) and leave as one coalesced stream of 128-bit stores
-                    constexpr int W = StageRecord<R>::kWords;
-                    R* wbuf = reinterpret_cast<R*>(smem_raw + a.table_bytes) + warp * (kStageCap * W);
+                    // records are assembled in this warp's shared-memory buffer (scattered writes are cheap there)
+                    // and leave as one coalesced stream of 128-bit stores
+                    StageRecord<R>* wbuf = reinterpret_cast<StageRecord<R>*>(smem_raw + a.table_bytes) + warp * kStageCap;
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
                         unsigned int r = rank_u[u];
 #pragma unroll
                         for (int v = 0; v < V; ++v) {
                             if ((fired_bits >> (u * V + v)) & 1u) {
-#pragma unroll
-                                for (int c = 0; c < 9; ++c) wbuf[r * W + c] = q[c][u].v[v];
-                                *reinterpret_cast<unsigned int*>(&wbuf[r * W + 9]) = (unsigned)((u * 32 + lane) * V + v);
+                                StageRecord<R>& rec = wbuf[r];
+                                rec.p[0] = q[0][u].v[v];
+                                rec.p[1] = q[1][u].v[v];
+                                rec.p[2] = q[2][u].v[v];
+                                rec.c2 = c2s[u * V + v];
+                                rec.idx = (unsigned)((u * 32 + lane) * V + v);
                                 ++r;
                             }
                         }
@@ -235,6 +242,11 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                     for (unsigned int k = lane; k < nvec; k += 32) st_policy(dst + k, src[k], pol_keep);
                     __syncwarp();
                 }
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const long long i = base + (long long)warp * WCH + (u * 32 + lane) * V;
+                *reinterpret_cast<Vec<TR, V>*>(a.tau + i) = t[u];
             }
         } else {  // ragged last tile: scalar, guarded
             if constexpr (EMIT) {  // its chunks are re-scanned by the event kernel

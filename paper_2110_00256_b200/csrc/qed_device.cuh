@@ -184,6 +184,19 @@ __device__ __forceinline__ double chi_squared(double px, double py, double pz, d
     return c2;
 }
 
+// chi^2 with g and 1/g from one fast reciprocal square root: the one routine both passes use, so that the
+// evolve pass and the event pass see bit-identical chi for the same particle
+template <int SPECIES>
+__device__ __forceinline__ double chi_squared_of(double px, double py, double pz, double ex, double ey, double ez,
+                                                 double bx, double by, double bz, double* inv_g_out, double* g2_out) {
+    const double p2 = fma(px, px, fma(py, py, pz * pz));
+    const double g2 = SPECIES == 0 ? 1.0 + p2 : p2;
+    const double inv_g = g2 > 1e-300 ? rsqrt_fast(g2) : 0.0;  // 1/gamma (lepton) or 1/gamma_gamma (photon)
+    *inv_g_out = inv_g;
+    *g2_out = g2;
+    return chi_squared<SPECIES>(px, py, pz, ex, ey, ez, bx, by, bz, g2 * inv_g, p2);
+}
+
 // ---- K_{1/3}(x), only for the Erber branch outside the T table -------------------------
 // returns ln K_{1/3}(x) + x  (exponentially scaled, so chi_gamma -> 0 does not underflow)
 __device__ __noinline__ double ln_bessel_k13_scaled(double x) {
