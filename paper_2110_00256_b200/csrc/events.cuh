@@ -193,37 +193,53 @@ __global__ void __launch_bounds__(256) tile_sums_kernel(unsigned short* __restri
     }
 }
 
-// tile_scan_kernel: one CTA scans the tile sums, 1024 at a time (coalesced), carrying the running total;
-// tile_offset[t] = number of events before tile t, *d_total = number of events.
+// tile_scan_kernel: one CTA scans the tile sums, 4096 per round (four consecutive sums per thread: 128-bit
+// loads), carrying the running total; tile_offset[t] = number of events before tile t, *d_total = their number.
 constexpr int kScanThreads = 1024;
+constexpr int kScanItems = 4;
 
 __global__ void __launch_bounds__(kScanThreads) tile_scan_kernel(const unsigned int* __restrict__ tile_sum, long long n_tiles,
                                                                  unsigned long long* __restrict__ tile_offset,
                                                                  unsigned long long* __restrict__ d_total) {
-    __shared__ unsigned long long warp_sum[kScanThreads / 32];
-    __shared__ unsigned long long s_carry;
+    __shared__ unsigned long long warp_sum[2][kScanThreads / 32];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_carry = 0;
-    __syncthreads();
-    for (long long base = 0; base < n_tiles; base += kScanThreads) {
-        const long long t = base + tid;
-        const unsigned long long v = t < n_tiles ? tile_sum[t] : 0ull;
-        unsigned long long incl = v;
+    unsigned long long carry = 0;  // (the same value in every thread)
+    int round = 0;
+    for (long long base = 0; base < n_tiles; base += kScanThreads * kScanItems, ++round) {
+        const long long t0 = base + (long long)tid * kScanItems;
+        unsigned int v[kScanItems];
+        if (t0 + kScanItems <= n_tiles) {
+            const uint4 q = *reinterpret_cast<const uint4*>(tile_sum + t0);  // t0 is a multiple of 4: 16-byte aligned
+            v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
+        } else {
+#pragma unroll
+            for (int k = 0; k < kScanItems; ++k) v[k] = t0 + k < n_tiles ? tile_sum[t0 + k] : 0u;
+        }
+        const unsigned long long s = (unsigned long long)v[0] + v[1] + v[2] + v[3];
+        unsigned long long incl = s;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
             const unsigned long long o = __shfl_up_sync(0xffffffffu, incl, d);
             if (lane >= d) incl += o;
         }
-        if (lane == 31) warp_sum[warp] = incl;
-        __syncthreads();
-        unsigned long long before = s_carry;
-        for (int w = 0; w < warp; ++w) before += warp_sum[w];
-        if (t < n_tiles) tile_offset[t] = before + incl - v;
-        __syncthreads();
-        if (tid == kScanThreads - 1) s_carry = before + incl;
-        __syncthreads();
+        if (lane == 31) warp_sum[round & 1][warp] = incl;
+        __syncthreads();  // (double-buffered: one barrier per round)
+        unsigned long long before = carry, all = 0;
+#pragma unroll 8
+        for (int w = 0; w < kScanThreads / 32; ++w) {
+            const unsigned long long ws = warp_sum[round & 1][w];
+            if (w < warp) before += ws;
+            all += ws;
+        }
+        unsigned long long run = before + incl - s;
+#pragma unroll
+        for (int k = 0; k < kScanItems; ++k) {
+            if (t0 + k < n_tiles) tile_offset[t0 + k] = run;
+            run += v[k];
+        }
+        carry += all;
     }
-    if (tid == 0) *d_total = s_carry;
+    if (tid == 0) *d_total = carry;
 }
 
 // ---- level 3: the events ---------------------------------------------------------------------
