@@ -8,8 +8,8 @@
 //  Compaction in three levels, all deterministic:
 //   1. warp ballot/popc ranks the fired particles of a 128-particle chunk and counts them
 //      (inside the evolve pass for picsarqed_qed_step, count_chunks_kernel for generate_*);
-//   2. tile_sums_kernel + tile_scan_kernel: the chunk counts are summed per tile and one CTA
-//      scans the tile sums (block-level scan) into exclusive output offsets and the total;
+//   2. tile_scan_kernel: one CTA sums the chunk counts per tile and scans the tile sums
+//      (block-level scan) into exclusive output offsets and the total;
 //   3. event_kernel: a tile of consecutive chunks per CTA; event e of the tile is handled by
 //      thread e, its output slot is tile_offset + e.  Tiles are independent: no
 //      ticket, no look-back, no barrier on the common path.
@@ -156,51 +156,19 @@ __global__ void __launch_bounds__(256) count_chunks_kernel(const TR* __restrict_
 }
 
 // ---- level 2: output offsets of the tiles (block-level scan) -------------------------------------
-// tile_sums_kernel: one warp per tile of `chunks_per_tile` chunks (<= 32): lane j reads the count of chunk j
-// (coalesced), chunks not counted yet (ragged tail of the evolve pass) are counted from tau and fixed up in
-// place, a warp reduction gives the tile's number of events.
-template <typename TR>
-__global__ void __launch_bounds__(256) tile_sums_kernel(unsigned short* __restrict__ cnt, long long n_chunks,
-                                                        int chunks_per_tile, long long n_tiles,
-                                                        const TR* __restrict__ tau, long long n,
-                                                        unsigned int* __restrict__ tile_sum) {
-    const int lane = threadIdx.x & 31;
-    const long long warps = (long long)gridDim.x * (blockDim.x / 32);
-    for (long long t = (long long)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); t < n_tiles; t += warps) {
-        const long long ch = t * chunks_per_tile + lane;
-        const bool real = lane < chunks_per_tile && ch < n_chunks;
-        unsigned int c = real ? cnt[ch] : 0u;
-        unsigned int unknown = __ballot_sync(0xffffffffu, real && c == kStageUnknown);
-        while (unknown) {  // rare: count the chunk from tau (tau < 0, R1), the whole warp on one chunk
-            const int j = __ffs(unknown) - 1;
-            unknown &= unknown - 1;
-            const long long cb = (t * chunks_per_tile + j) * kChunk;
-            unsigned int k = 0;
-#pragma unroll
-            for (int r4 = 0; r4 < kChunk / 32; ++r4) {
-                const long long i = cb + r4 * 32 + lane;
-                k += __popc(__ballot_sync(0xffffffffu, i < n && tau[i] < (TR)0));
-            }
-            if (lane == j) {
-                c = k | kStageNoRecords;
-                cnt[ch] = (unsigned short)c;
-            }
-        }
-        unsigned int s = c & kStageCountMask;
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
-        if (lane == 0) tile_sum[t] = s;
-    }
-}
-
-// tile_scan_kernel: one CTA scans the tile sums, 4096 per round (four consecutive sums per thread: 128-bit
-// loads), carrying the running total; tile_offset[t] = number of events before tile t, *d_total = their number.
+// tile_scan_kernel: one CTA sums the chunk counts of every tile (128-bit loads of eight 16-bit counts) and scans
+// the tile sums, 4096 tiles per round (four consecutive tiles per thread), carrying the running total;
+// tile_offset[t] = number of events before tile t, *d_total = their number.
 constexpr int kScanThreads = 1024;
 constexpr int kScanItems = 4;
 
+// cnt != nullptr: the tile sums are computed here as well (chunk counts summed per tile, 128-bit loads when a tile
+// is a multiple of 8 chunks); every chunk has been counted.  cnt == nullptr: they are read from tile_sum.
 __global__ void __launch_bounds__(kScanThreads) tile_scan_kernel(const unsigned int* __restrict__ tile_sum, long long n_tiles,
                                                                  unsigned long long* __restrict__ tile_offset,
-                                                                 unsigned long long* __restrict__ d_total) {
+                                                                 unsigned long long* __restrict__ d_total,
+                                                                 const unsigned short* __restrict__ cnt, long long n_chunks,
+                                                                 int chunks_per_tile) {
     __shared__ unsigned long long warp_sum[2][kScanThreads / 32];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     unsigned long long carry = 0;  // (the same value in every thread)
@@ -208,7 +176,26 @@ __global__ void __launch_bounds__(kScanThreads) tile_scan_kernel(const unsigned 
     for (long long base = 0; base < n_tiles; base += kScanThreads * kScanItems, ++round) {
         const long long t0 = base + (long long)tid * kScanItems;
         unsigned int v[kScanItems];
-        if (t0 + kScanItems <= n_tiles) {
+        if (cnt != nullptr) {
+#pragma unroll
+            for (int k = 0; k < kScanItems; ++k) {
+                const long long c0 = (t0 + k) * chunks_per_tile;
+                unsigned int sum = 0;
+                if (t0 + k < n_tiles) {
+                    if ((chunks_per_tile & 7) == 0 && c0 + chunks_per_tile <= n_chunks) {
+                        for (int c = 0; c < chunks_per_tile; c += 8) {  // 8 counts per 128-bit load, two per word
+                            const uint4 q = *reinterpret_cast<const uint4*>(cnt + c0 + c);
+                            const unsigned int w4[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) sum += (w4[j] & kStageCountMask) + ((w4[j] >> 16) & kStageCountMask);
+                        }
+                    } else {
+                        for (long long c = c0; c < min(c0 + (long long)chunks_per_tile, n_chunks); ++c) sum += cnt[c] & kStageCountMask;
+                    }
+                }
+                v[k] = sum;
+            }
+        } else if (t0 + kScanItems <= n_tiles) {
             const uint4 q = *reinterpret_cast<const uint4*>(tile_sum + t0);  // t0 is a multiple of 4: 16-byte aligned
             v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
         } else {

@@ -36,10 +36,9 @@ struct EvolveArgs {
 constexpr int kChunk = 128;                 // particles one warp handles per tile: the unit of record staging
 constexpr int kStageCap = 24;               // records per chunk segment (mean at 5 % firing: 6.4)
 // stage_cnt[chunk]: bits 0..14 = number of particles of the chunk that fired; bit 15 = the chunk has no staged
-// records (segment overflow, or counted by count_chunks_kernel); 0xFFFF = not counted yet (ragged tail)
+// records (segment overflow, ragged last tile, or counted by count_chunks_kernel)
 constexpr unsigned short kStageCountMask = 0x7FFFu;
 constexpr unsigned short kStageNoRecords = 0x8000u;
-constexpr unsigned short kStageUnknown = 0xFFFFu;
 
 // one staged record: what event generation needs of a particle that fired -- its momentum, chi^2 (computed by the
 // evolve pass anyway) and its index inside the chunk.  Sizes are multiples of 16 bytes so that records move as
@@ -248,18 +247,27 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                 const long long i = base + (long long)warp * WCH + (u * 32 + lane) * V;
                 *reinterpret_cast<Vec<TR, V>*>(a.tau + i) = t[u];
             }
-        } else {  // ragged last tile: scalar, guarded
-            if constexpr (EMIT) {  // its chunks are re-scanned by the event kernel
-                const long long c0 = base / kChunk, c1 = (a.n + kChunk - 1) / kChunk;
-                for (long long c = c0 + threadIdx.x; c < c1; c += kEvolveThreads) a.stage_cnt[c] = kStageUnknown;
-            }
-            for (long long i = base + threadIdx.x; i < a.n; i += kEvolveThreads) {
-                const R d = decrement_one<R, SPECIES>(a.p[0][i], a.p[1][i], a.p[2][i], a.e[0][i], a.e[1][i],
-                                                      a.e[2][i], a.b[0][i], a.b[1][i], a.b[2][i], tab, a.tab,
-                                                      a.rate_dt);
-                const TR tn = a.tau[i] - (TR)d;
-                a.tau[i] = tn;
-                fired += tn < (TR)0 ? 1u : 0u;
+        } else {  // ragged last tile: one warp per 128-particle chunk, scalar guarded accesses
+            const long long c1 = (a.n + kChunk - 1) / kChunk;
+            for (long long c = base / kChunk + warp; c < c1; c += kEvolveThreads / 32) {
+                unsigned int k = 0;
+#pragma unroll 1
+                for (int r4 = 0; r4 < kChunk / 32; ++r4) {
+                    const long long i = c * kChunk + r4 * 32 + lane;
+                    bool f = false;
+                    if (i < a.n) {
+                        const R d = decrement_one<R, SPECIES>(a.p[0][i], a.p[1][i], a.p[2][i], a.e[0][i], a.e[1][i],
+                                                              a.e[2][i], a.b[0][i], a.b[1][i], a.b[2][i], tab, a.tab,
+                                                              a.rate_dt);
+                        const TR tn = a.tau[i] - (TR)d;
+                        a.tau[i] = tn;
+                        f = tn < (TR)0;
+                    }
+                    k += __popc(__ballot_sync(0xffffffffu, f));
+                }
+                if (lane == 0) fired += k;
+                // no records for these chunks: the event kernel finds their particles again from tau
+                if (EMIT && lane == 0) a.stage_cnt[c] = (unsigned short)(k | kStageNoRecords);
             }
         }
     }

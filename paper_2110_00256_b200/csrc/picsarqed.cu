@@ -474,9 +474,7 @@ int launch_event_pass(picsarqed_ctx* c, long long n, const ChunkScratch& cs, voi
     static const int kChunksOf[8] = {24, 32, 24, 16, 12, 24, 24, 32};  // must match the switch below
     const int chunks = kChunksOf[c->event_config];
     const long long n_tiles = (cs.n_chunks + chunks - 1) / chunks;
-    const int sum_grid = (int)std::max<long long>(1, std::min<long long>((n_tiles + 7) / 8, (long long)c->num_sms * 8));
-    tile_sums_kernel<TR><<<sum_grid, 256, 0, c->stream>>>(cs.cnt, cs.n_chunks, chunks, n_tiles, (const TR*)tau, n, cs.sum);
-    tile_scan_kernel<<<1, kScanThreads, 0, c->stream>>>(cs.sum, n_tiles, cs.off, d_n_out);
+    tile_scan_kernel<<<1, kScanThreads, 0, c->stream>>>(nullptr, n_tiles, cs.off, d_n_out, cs.cnt, cs.n_chunks, chunks);
 #define PXQ_LAUNCH_EVENTS(T, CH, MB)                                                                         \
     do {                                                                                                     \
         auto kern = event_kernel<R, TR, KIND, T, CH, MB>;                                                    \
