@@ -139,11 +139,11 @@ __device__ __forceinline__ void event_commit(const EventArgs<R, TR>& a, long lon
 // ---- level 1 for generate_*: count the fired particles of every chunk --------------------------
 // one warp per chunk: tau < 0 (R1) -> ballot/popc.  No records are staged on this path.
 template <typename TR>
-__global__ void __launch_bounds__(256) count_chunks_kernel(const TR* __restrict__ tau, long long n, long long n_chunks,
-                                                           unsigned short* __restrict__ cnt) {
+__global__ void __launch_bounds__(256) count_chunks_kernel(const TR* __restrict__ tau, long long n, long long first_chunk,
+                                                           long long n_chunks, unsigned short* __restrict__ cnt) {
     const int lane = threadIdx.x & 31;
     const long long warps = (long long)gridDim.x * (blockDim.x / 32);
-    for (long long ch = (long long)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); ch < n_chunks; ch += warps) {
+    for (long long ch = first_chunk + (long long)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); ch < n_chunks; ch += warps) {
         unsigned int k = 0;
 #pragma unroll
         for (int r4 = 0; r4 < kChunk / 32; ++r4) {

@@ -36,7 +36,7 @@ struct EvolveArgs {
 constexpr int kChunk = 128;                 // particles one warp handles per tile: the unit of record staging
 constexpr int kStageCap = 24;               // records per chunk segment (mean at 5 % firing: 6.4)
 // stage_cnt[chunk]: bits 0..14 = number of particles of the chunk that fired; bit 15 = the chunk has no staged
-// records (segment overflow, ragged last tile, or counted by count_chunks_kernel)
+// records (segment overflow, or counted by count_chunks_kernel: generate_* calls and the ragged last tile)
 constexpr unsigned short kStageCountMask = 0x7FFFu;
 constexpr unsigned short kStageNoRecords = 0x8000u;
 
@@ -139,7 +139,7 @@ __device__ __forceinline__ auto decrement_one(R pxr, R pyr, R pzr, R exr, R eyr,
 // EMIT: also append the nine reals of every particle that fired to the staging segment of its 128-particle
 // chunk, in index order (warp ballot/popc; no CTA barrier), for staged_event_kernel.  Requires U*32*V == kChunk.
 template <typename R, typename TR, int SPECIES, int U, bool EMIT>
-__global__ void __launch_bounds__(kEvolveThreads, U <= 2 ? 2 : 1)
+__global__ void __launch_bounds__(kEvolveThreads, U > 2 ? 1 : ((sizeof(R) == 4 && U == 1 && SPECIES == 0) ? 3 : 2))
 evolve_kernel(const EvolveArgs<R, TR> a) {
     constexpr int V = 16 / sizeof(R);
     constexpr int TILE = kEvolveThreads * V * U;
@@ -247,27 +247,14 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                 const long long i = base + (long long)warp * WCH + (u * 32 + lane) * V;
                 *reinterpret_cast<Vec<TR, V>*>(a.tau + i) = t[u];
             }
-        } else {  // ragged last tile: one warp per 128-particle chunk, scalar guarded accesses
-            const long long c1 = (a.n + kChunk - 1) / kChunk;
-            for (long long c = base / kChunk + warp; c < c1; c += kEvolveThreads / 32) {
-                unsigned int k = 0;
-#pragma unroll 1
-                for (int r4 = 0; r4 < kChunk / 32; ++r4) {
-                    const long long i = c * kChunk + r4 * 32 + lane;
-                    bool f = false;
-                    if (i < a.n) {
-                        const R d = decrement_one<R, SPECIES>(a.p[0][i], a.p[1][i], a.p[2][i], a.e[0][i], a.e[1][i],
-                                                              a.e[2][i], a.b[0][i], a.b[1][i], a.b[2][i], tab, a.tab,
-                                                              a.rate_dt);
-                        const TR tn = a.tau[i] - (TR)d;
-                        a.tau[i] = tn;
-                        f = tn < (TR)0;
-                    }
-                    k += __popc(__ballot_sync(0xffffffffu, f));
-                }
-                if (lane == 0) fired += k;
-                // no records for these chunks: the event kernel finds their particles again from tau
-                if (EMIT && lane == 0) a.stage_cnt[c] = (unsigned short)(k | kStageNoRecords);
+        } else {  // ragged last tile: scalar, guarded (qed_step counts its chunks afterwards: count_chunks_kernel)
+            for (long long i = base + threadIdx.x; i < a.n; i += kEvolveThreads) {
+                const R d = decrement_one<R, SPECIES>(a.p[0][i], a.p[1][i], a.p[2][i], a.e[0][i], a.e[1][i],
+                                                      a.e[2][i], a.b[0][i], a.b[1][i], a.b[2][i], tab, a.tab,
+                                                      a.rate_dt);
+                const TR tn = a.tau[i] - (TR)d;
+                a.tau[i] = tn;
+                fired += tn < (TR)0 ? 1u : 0u;
             }
         }
     }

@@ -507,7 +507,7 @@ int launch_events(picsarqed_ctx* c, long long n, void* const* p, const void* con
     ChunkScratch cs;
     if (int rc = chunk_scratch<R>(c, n, &cs)) return rc;
     const int grid = (int)std::max<long long>(1, std::min<long long>((cs.n_chunks + 7) / 8, (long long)c->num_sms * 8));
-    count_chunks_kernel<TR><<<grid, 256, 0, c->stream>>>((const TR*)tau, n, cs.n_chunks, cs.cnt);
+    count_chunks_kernel<TR><<<grid, 256, 0, c->stream>>>((const TR*)tau, n, 0, cs.n_chunks, cs.cnt);
     return launch_event_pass<R, TR, KIND>(c, n, cs, p, eb, tau, seed, step, id_base, capacity, out_p, out_tau, parent,
                                           d_n_out);
 }
@@ -530,6 +530,9 @@ int launch_step(picsarqed_ctx* c, long long n, void* const* p, const void* const
         PXQ_CUDA(c, cudaEventRecord(ev[0], c->stream));
     }
     if (int rc = launch_evolve_u<R, TR, SPECIES, U, true>(c, n, a9, dt, tau, nullptr, sv)) return rc;
+    constexpr long long kTile = (long long)kEvolveThreads * (16 / (int)sizeof(R)) * U;
+    if (n % kTile)  // the ragged last tile stages no records: count its chunks from the updated tau
+        count_chunks_kernel<TR><<<1, 256, 0, c->stream>>>((const TR*)tau, n, (n / kTile) * kTile / kChunk, cs.n_chunks, cs.cnt);
     if (c->time_kernels) PXQ_CUDA(c, cudaEventRecord(ev[1], c->stream));
     if (int rc = launch_event_pass<R, TR, SPECIES>(c, n, cs, p, eb, tau, seed, step, id_base, capacity, out_p, out_tau,
                                                    parent, d_n_out))
