@@ -74,6 +74,8 @@ def lib():
             _dp, _dp, _dp, _dp, _i64p, _dp)
         sig("orc_generate_pairs", i64, tp, i, i, i64, *([_dp] * 10), u64, u64, _u64p, i64,
             *([_dp] * 8), _i64p, _dp)
+        sig("orc_schwinger_prefactor", d)
+        sig("orc_schwinger_rate", None, i64, *([_dp] * 7))
         sig("orc_qs_sample_xi", d, tp, d, d)
         sig("orc_bw_sample_xi", d, tp, d, d)
         _lib = L
@@ -331,3 +333,19 @@ def qs_sample_xi(tables, chi_v, r):
 def bw_sample_xi(tables, chi_v, rp):
     ct = tables._c()
     return lib().orc_bw_sample_xi(C.byref(ct), chi_v, rp)
+
+
+def schwinger_prefactor():
+    return lib().orc_schwinger_prefactor()
+
+
+def schwinger_rate(e, b):
+    """pairs per m^3 per s (eq.19) for fields in units of E_s"""
+    arrs = [_f64(a) for a in (*e, *b)]
+    n = arrs[0].size
+    out = np.empty(n)
+    lib().orc_schwinger_rate(n, *[_p(a) for a in arrs], _p(out))
+    return out
+
+
+__all__ += ["schwinger_prefactor", "schwinger_rate"]

@@ -716,6 +716,41 @@ int64_t orc_generate_pairs(const OrcTables* t, int dtype, int tau_dtype, int64_t
     return n_out;
 }
 
+// ---- Schwinger pair production rate per unit volume (eqs.19-22), SURVEY.md 8(f)-3 ----
+// Fields in units of E_s (e = E/E_s, b = cB/E_s).  Invariants F = (e^2 - b^2)/2, G = e.b (eqs.21-22, in E_s^2),
+// epsilon = sqrt(sqrt(F^2+G^2) + F), eta = sqrt(sqrt(F^2+G^2) - F) (eq.20), and eq.19 taken literally in
+// binary128 (the difference under the second root cancels when F >> abs(G)):
+//     d^2N/dt dV = q_e^2 E_s^2/(4 pi^2 hbar^2 c) * epsilon eta coth(pi eta/epsilon) exp(-pi/epsilon)   [1/(m^3 s)]
+// eta -> 0 is the removable limit eta coth(pi eta/epsilon) -> epsilon/pi; epsilon = 0 gives 0.
+static real schwinger_prefactor() {
+    const real es = M_ELECTRON * M_ELECTRON * C_LIGHT * C_LIGHT * C_LIGHT / (Q_ELEM * hbar());
+    return Q_ELEM * Q_ELEM * es * es / (4 * PI_L * PI_L * hbar() * hbar() * C_LIGHT);
+}
+double orc_schwinger_prefactor() { return (double)schwinger_prefactor(); }
+void orc_schwinger_rate(int64_t n, const double* ex, const double* ey, const double* ez, const double* bx,
+                        const double* by, const double* bz, double* rate_out) {
+    const __float128 PIq = 4 * atanq((__float128)1);
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        const __float128 e2 = (__float128)ex[i] * ex[i] + (__float128)ey[i] * ey[i] + (__float128)ez[i] * ez[i];
+        const __float128 b2 = (__float128)bx[i] * bx[i] + (__float128)by[i] * by[i] + (__float128)bz[i] * bz[i];
+        const __float128 F = (e2 - b2) / 2;
+        const __float128 G = (__float128)ex[i] * bx[i] + (__float128)ey[i] * by[i] + (__float128)ez[i] * bz[i];
+        const __float128 root = sqrtq(F * F + G * G);
+        __float128 eps2 = root + F, eta2 = root - F;
+        if (eps2 < 0) eps2 = 0;
+        if (eta2 < 0) eta2 = 0;
+        const __float128 eps = sqrtq(eps2), eta = sqrtq(eta2);
+        __float128 r = 0;
+        if (eps > 0) {
+            const __float128 x = PIq * eta / eps;
+            const __float128 eta_coth = x > (__float128)1e-12 ? eta * (coshq(x) / sinhq(x)) : eps / PIq;  // removable limit
+            r = eps * eta_coth * expq(-PIq / eps);
+        }
+        rate_out[i] = (double)((__float128)schwinger_prefactor() * r);
+    }
+}
+
 // the inverse-CDF maps alone (for the distribution pins)
 double orc_qs_sample_xi(const OrcTables* t, double chi, double r) {
     return (double)qs_sample_xi(t, chi, r);

@@ -334,3 +334,48 @@ def test_inverse_cdf_closed_form_tables(orc):
     assert orc.qs_sample_xi(t, 0.5, 1e-3) == 1e-6      # r < P(xi_min) = 1e-2
     for r in (0.0, 0.01, 0.26, 0.5):
         assert orc.bw_sample_xi(t, 3.0, r) == pytest.approx(r, abs=1e-15)
+
+
+# ----------------------------------------------------------------------------- Schwinger rate
+def test_schwinger_rate_closed_forms(orc):
+    """PAPER.md:171-183 eqs.19-22: prefactor from CODATA, pure-E textbook limit, E parallel B, null fields"""
+    hbar = 6.62607015e-34 / (2 * math.pi)
+    m, c = 9.1093837015e-31, 299792458.0
+    C = m ** 4 * c ** 5 / (4 * math.pi ** 2 * hbar ** 4)   # q^2 E_s^2/(4 pi^2 hbar^2 c) with E_s = m^2 c^3/(q hbar)
+    assert orc.schwinger_prefactor() == pytest.approx(C, rel=1e-13)
+    z = np.zeros(4)
+    ev = np.array([1.0, 0.3, 0.1, 0.05])
+    # pure electric field: (qE)^2/(4 pi^3 hbar^2 c) exp(-pi E_s/E), the leading term of Schwinger's formula
+    r = orc.schwinger_rate([ev, z, z], [z, z, z])
+    assert np.allclose(r, C * ev ** 2 / math.pi * np.exp(-math.pi / ev), rtol=1e-14)
+    # E parallel B: epsilon = E/E_s, eta = cB/E_s exactly (F = (e^2-b^2)/2, G = e b)
+    bv = np.array([0.5, 0.3, 0.02, 0.4])
+    r = orc.schwinger_rate([z, ev, z], [z, bv, z])
+    assert np.allclose(r, C * ev * bv / np.tanh(math.pi * bv / ev) * np.exp(-math.pi / ev), rtol=1e-13)
+    # pure magnetic field, and a plane wave (e perpendicular to b, equal norms: F = G = 0): no pairs
+    assert np.all(orc.schwinger_rate([z, z, z], [bv, z, z]) == 0)
+    assert np.all(orc.schwinger_rate([ev, z, z], [z, ev, z]) == 0)
+    # weak-field values are representable far below double underflow of exp(-pi/eps) * C? (C ~ 3e56)
+    assert orc.schwinger_rate([np.array([0.005])] + [np.zeros(1)] * 2, [np.zeros(1)] * 3)[0] == pytest.approx(
+        C * 0.005 ** 2 / math.pi * math.exp(-math.pi / 0.005), rel=1e-12)
+
+
+def test_schwinger_rate_is_lorentz_invariant(orc):
+    """the rate depends on the fields only through the invariants F and G: rotations, boosts, G -> -G"""
+    rng = np.random.default_rng(11)
+    n = 200
+    e = rng.normal(size=(3, n)) * 0.3
+    b = rng.normal(size=(3, n)) * 0.3
+    r0 = orc.schwinger_rate(list(e), list(b))
+    # rotation
+    q, _ = np.linalg.qr(rng.normal(size=(3, 3)))
+    assert np.allclose(orc.schwinger_rate(list(q @ e), list(q @ b)), r0, rtol=1e-12)
+    # boost along x with velocity beta: parallel components unchanged, e_perp' = g (e + beta x b), b_perp' = g (b - beta x e)
+    beta = 0.6
+    g = 1 / math.sqrt(1 - beta * beta)
+    e2 = np.array([e[0], g * (e[1] - beta * b[2]), g * (e[2] + beta * b[1])])
+    b2 = np.array([b[0], g * (b[1] + beta * e[2]), g * (b[2] - beta * e[1])])
+    assert np.allclose(orc.schwinger_rate(list(e2), list(b2)), r0, rtol=1e-11)
+    # parity: b -> -b flips the sign of G only
+    assert np.allclose(orc.schwinger_rate(list(e), list(-b)), r0, rtol=1e-13)
+    assert np.all(r0 >= 0) and np.any(r0 > 0)
