@@ -113,6 +113,14 @@ int picsarqed_chi(picsarqed_ctx* ctx, int species, int dtype, long long n,
                   const void* ex, const void* ey, const void* ez,
                   const void* bx, const void* by, const void* bz, void* chi_out);
 
+/* ---- Schwinger pair production (eqs.19-22) -----------------
+ * rate_out[i] (device, fp64 whatever `dtype`) = d^2N/dt dV in pairs per m^3 per s for the fields of cell i:
+ * q_e^2 E_s^2/(4 pi^2 hbar^2 c) eps eta coth(pi eta/eps) exp(-pi/eps), eps, eta from the invariants
+ * F = (e^2 - b^2)/2 and G = e.b (fields in units of E_s).  Pairs are created at rest. */
+int picsarqed_schwinger_rate(picsarqed_ctx* ctx, int dtype, long long n,
+                             const void* ex, const void* ey, const void* ez,
+                             const void* bx, const void* by, const void* bz, double* rate_out);
+
 /* ---- optical depth ----------------------------------------------
  * tau[i] = -ln U(seed, id_base+i, step 0, purpose 0, species): a draw from p(x) = exp(-x). */
 int picsarqed_init_optical_depth(picsarqed_ctx* ctx, int species, int tau_dtype, long long n,

@@ -57,6 +57,7 @@ _SIGNATURES = {
     "picsarqed_export_tables": (_i, [_vp, _i, _vp, C.c_size_t]),
     "picsarqed_import_tables": (_i, [_vp, C.POINTER(_CParams), _vp, _vp, _vp, _vp]),
     "picsarqed_chi": (_i, [_vp, _i, _i, _i64] + [_vp] * 10),
+    "picsarqed_schwinger_rate": (_i, [_vp, _i, _i64] + [_vp] * 7),
     "picsarqed_init_optical_depth": (_i, [_vp, _i, _i, _i64, _u64, _u64, _vp]),
     "picsarqed_evolve_optical_depth": (_i, [_vp, _i, _i, _i, _i64] + [_vp] * 9 + [_d, _vp, _vp]),
     "picsarqed_generate_photons": (_i, [_vp, _i, _i, _i64] + [_vp] * 10 + [_u64, _u64, _u64, _i64] + [_vp] * 6),
@@ -180,6 +181,16 @@ class Context:
             out = torch.empty(n, dtype=dt, device=p[0].device)
         ptrs = [_dev(t, dt) for t in (*p, *e, *b, out)]
         self._check(lib().picsarqed_chi(self._h, species, _code(dt), n, *ptrs))
+        return out
+
+    def schwinger_rate(self, e, b, out=None):
+        """pairs per m^3 per s (fp64) for fields in units of E_s (picsarqed_schwinger_rate)"""
+        d = e[0].dtype
+        n = e[0].numel()
+        if out is None:
+            out = torch.empty(n, dtype=torch.float64, device=e[0].device)
+        self._check(lib().picsarqed_schwinger_rate(self._h, _code(d), n, *[_dev(t, d) for t in (*e, *b)],
+                                                   _dev(out, torch.float64)))
         return out
 
     def init_optical_depth(self, species, tau, seed, id_base=0):

@@ -323,6 +323,67 @@ __global__ void __launch_bounds__(256) chi_kernel(const R* __restrict__ px, cons
         out[i] = one(px[i], py[i], pz[i], ex[i], ey[i], ez[i], bx[i], by[i], bz[i]);
 }
 
+// ---- Schwinger pair-production rate per unit volume (eqs.19-22) ----------
+// rate[i] = q_e^2 E_s^2/(4 pi^2 hbar^2 c) eps eta coth(pi eta/eps) exp(-pi/eps) in 1/(m^3 s), with
+// F = (e^2 - b^2)/2, G = e.b, eps^2 = sqrt(F^2+G^2) + F, eta^2 = sqrt(F^2+G^2) - F.  The smaller of eps^2, eta^2 is
+// taken as G^2 over the larger one (the literal difference cancels when abs(F) >> abs(G)).  Output is fp64 for
+// either input type: the values span e^-600 .. 1e56.
+constexpr double kSchwingerPrefactor =
+    kElectronMass * kElectronMass * kElectronMass * kElectronMass * kLightSpeed * kLightSpeed * kLightSpeed *
+    kLightSpeed * kLightSpeed /
+    (4.0 * kPi * kPi * (kPlanck / (2.0 * kPi)) * (kPlanck / (2.0 * kPi)) * (kPlanck / (2.0 * kPi)) * (kPlanck / (2.0 * kPi)));
+
+constexpr double kLnSchwingerPrefactor = 130.17295285072183;  // ln(kSchwingerPrefactor) (the parity test would show a slip)
+
+__device__ __forceinline__ double schwinger_rate_one(double ex, double ey, double ez, double bx, double by, double bz) {
+    const double e2 = fma(ex, ex, fma(ey, ey, ez * ez)), b2 = fma(bx, bx, fma(by, by, bz * bz));
+    const double F = 0.5 * (e2 - b2), G = fma(ex, bx, fma(ey, by, ez * bz));
+    const double s1 = fma(F, F, G * G);
+    if (!(s1 > 1e-280)) return 0.0;                       // null field: eps = eta = 0
+    const double big = s1 * rsqrt_fast(s1) + fabs(F);     // the larger of eps^2, eta^2
+    const double small = G * G * rcp_fast(big);
+    const double eps2 = F >= 0.0 ? big : small, eta2 = F >= 0.0 ? small : big;
+    if (!(eps2 > 1e-280)) return 0.0;                     // exp(-pi/eps) = 0
+    const double inv_eps = rsqrt_fast(eps2);
+    const double eps = eps2 * inv_eps;
+    const double eta = eta2 > 1e-280 ? eta2 * rsqrt_fast(eta2) : 0.0;
+    const double x = kPi * eta * inv_eps;
+    double eta_coth;                                      // eta coth(x); x coth x = 1 + x^2/3 - ... at x -> 0
+    if (x > 1e-4) {
+        const double q = exp_fast(-2.0 * x);
+        eta_coth = eta * (1.0 + q) * rcp_fast(1.0 - q);
+    } else {
+        eta_coth = eps * (1.0 / kPi) * fma(x * x, 1.0 / 3.0, 1.0);
+    }
+    // the prefactor (~3e56) goes into the exponent: exp(-pi/eps) alone underflows long before the rate does
+    return eps * eta_coth * exp_fast(kLnSchwingerPrefactor - kPi * inv_eps);
+}
+
+template <typename R>
+__global__ void __launch_bounds__(256) schwinger_kernel(const R* __restrict__ ex, const R* __restrict__ ey,
+                                                        const R* __restrict__ ez, const R* __restrict__ bx,
+                                                        const R* __restrict__ by, const R* __restrict__ bz,
+                                                        double* __restrict__ out, long long n) {
+    constexpr int V = 16 / sizeof(R);
+    const long long nvec = n / V;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const unsigned long long pol = l2_policy_evict_first();
+    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < nvec; j += stride) {
+        const long long i = j * V;
+        const Vec<R, V> a0 = ld_stream<R, V>(ex + i, pol), a1 = ld_stream<R, V>(ey + i, pol), a2 = ld_stream<R, V>(ez + i, pol),
+                        a3 = ld_stream<R, V>(bx + i, pol), a4 = ld_stream<R, V>(by + i, pol), a5 = ld_stream<R, V>(bz + i, pol);
+#pragma unroll
+        for (int v = 0; v < V; v += 2) {
+            double2 o;
+            o.x = schwinger_rate_one(a0.v[v], a1.v[v], a2.v[v], a3.v[v], a4.v[v], a5.v[v]);
+            o.y = schwinger_rate_one(a0.v[v + 1], a1.v[v + 1], a2.v[v + 1], a3.v[v + 1], a4.v[v + 1], a5.v[v + 1]);
+            *reinterpret_cast<double2*>(out + i + v) = o;
+        }
+    }
+    for (long long i = nvec * V + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+        out[i] = schwinger_rate_one(ex[i], ey[i], ez[i], bx[i], by[i], bz[i]);
+}
+
 // ---- tau = -ln U, purpose 0, step 0 -------------------------------
 template <typename TR>
 __global__ void __launch_bounds__(256) init_tau_kernel(TR* __restrict__ tau, long long n, unsigned long long seed,

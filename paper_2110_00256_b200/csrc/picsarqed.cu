@@ -579,6 +579,28 @@ int picsarqed_chi(picsarqed_ctx* c, int species, int dtype, long long n, const v
     return fail(c, PICSARQED_ERR_DTYPE, "bad dtype");
 }
 
+int picsarqed_schwinger_rate(picsarqed_ctx* c, int dtype, long long n, const void* ex, const void* ey, const void* ez,
+                             const void* bx, const void* by, const void* bz, double* rate_out) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (n < 0) return fail(c, PICSARQED_ERR_INVALID, "bad n");
+    if (n == 0) return PICSARQED_OK;
+    const void* a[7] = {ex, ey, ez, bx, by, bz, rate_out};
+    if (int rc = check_arrays(c, a, 7)) return rc;
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    if (dtype == PICSARQED_F64)
+        schwinger_kernel<double><<<stream_grid(c, (n + 1) / 2, 256), 256, 0, c->stream>>>(
+            (const double*)ex, (const double*)ey, (const double*)ez, (const double*)bx, (const double*)by,
+            (const double*)bz, rate_out, n);
+    else if (dtype == PICSARQED_F32)
+        schwinger_kernel<float><<<stream_grid(c, (n + 3) / 4, 256), 256, 0, c->stream>>>(
+            (const float*)ex, (const float*)ey, (const float*)ez, (const float*)bx, (const float*)by, (const float*)bz,
+            rate_out, n);
+    else
+        return fail(c, PICSARQED_ERR_DTYPE, "bad dtype");
+    PXQ_CUDA(c, cudaGetLastError());
+    return PICSARQED_OK;
+}
+
 int picsarqed_init_optical_depth(picsarqed_ctx* c, int species, int tau_dtype, long long n, unsigned long long seed,
                                  unsigned long long id_base, void* tau) {
     if (!c) return PICSARQED_ERR_INVALID;

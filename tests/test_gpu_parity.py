@@ -426,3 +426,44 @@ def test_evolve_decrement_accuracy_fp64(orc, qed, ctx, mid_tables, species):
     bad = np.nonzero(rel > bound)[0]
     assert bad.size == 0, (rel[bad[:5]], bound[bad[:5]])
     assert np.all(d_gpu[~ok] <= 1.0000001 * d_orc[~ok])
+
+
+# ----------------------------------------------------------------------------- Schwinger rate
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("n", [100003, 5, 1])
+def test_schwinger_rate(orc, qed, ctx, dtype, n):
+    """PAPER.md eqs.19-22 against the oracle's binary128 evaluation.  Tolerance on ln(rate): the rate is
+    exp(-pi/eps) of the field invariants, so a rounding of the invariants F, G is amplified by (2 + pi/eps) kappa,
+    kappa = d ln(eps^2) per unit relative rounding (order 1 for E parallel B, infinite for a plane wave)."""
+    rng = np.random.default_rng(3)
+    amp = np.exp(rng.uniform(np.log(0.02), np.log(2.0), n))
+    e = [np.ascontiguousarray((amp * rng.normal(size=n)).astype(dtype)) for _ in range(3)]
+    b = [np.ascontiguousarray((amp * rng.normal(size=n)).astype(dtype)) for _ in range(3)]
+    if n > 100:  # special geometries: pure E, pure B, plane wave, E parallel B
+        for k in range(3):
+            b[k][0] = 0
+            e[k][1] = 0
+        e[0][2], e[1][2], e[2][2], b[0][2], b[1][2], b[2][2] = 0.3, 0, 0, 0, 0.3, 0
+        e[0][3], e[1][3], e[2][3], b[0][3], b[1][3], b[2][3] = 0.4, 0, 0, 0.25, 0, 0
+    got = ctx.schwinger_rate(to_dev(e), to_dev(b)).cpu().numpy()
+    ref = orc.schwinger_rate(e, b)
+    e64 = [np.asarray(a, np.float64) for a in e]
+    b64 = [np.asarray(a, np.float64) for a in b]
+    e2, b2 = sum(a * a for a in e64), sum(a * a for a in b64)
+    F, G = 0.5 * (e2 - b2), sum(x * y for x, y in zip(e64, b64))
+    root = np.sqrt(F * F + G * G)
+    eps = np.sqrt(np.maximum(root + F, 1e-300))
+    # conditioning of eps^2 = sqrt(F^2+G^2) + F with respect to roundings of F and G of size u (e^2 + b^2)
+    rs = np.maximum(root, 1e-300)
+    kappa = (e2 + b2) * (np.abs(1 + F / rs) + np.abs(G) / rs) / np.maximum(eps * eps, 1e-300)
+    pos = ref > 1e-290
+    assert np.all(got[~pos] <= 1e-280)
+    err = np.abs(np.log(got[pos]) - np.log(ref[pos]))
+    # 4e-13: the kernel carries ln(prefactor) = 130 in the exponent (so that weak fields do not underflow early):
+    # a few roundings of size 130 * 2^-53
+    bound = 4e-13 + 1e-15 * (2 + np.pi / eps[pos]) * kappa[pos]
+    w = int(np.argmax(err / bound))
+    assert np.all(err <= bound), (err[w], bound[w], eps[pos][w], kappa[pos][w], got[pos][w], ref[pos][w])
+    if n > 100:
+        assert got[1] == 0 and got[2] == 0 and got[0] > 0 and got[3] > 0
+        assert np.median(err) < 2e-13
