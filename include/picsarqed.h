@@ -80,7 +80,9 @@ const char* picsarqed_last_error(const picsarqed_ctx* ctx);
 int picsarqed_version(void);
 /* Tuning knobs (integers): "evolve_unroll" in {0 (default), 1, 2, 4} = independent 128-bit
  * loads per array per thread in the evolve kernel; "evolve_ctas_per_sm" (0 = occupancy limit);
- * "event_config" 0..7 = (threads, chunks per tile) of the event kernel; "time_kernels" 0/1. */
+ * "event_config" 0..7 = (threads, chunks per tile) of the event kernel; "time_kernels" 0/1;
+ * "host_slabs" 0..64 = number of slabs step_host pipelines (0 = automatic: slabs of at least
+ * 2^20 particles, at most 32; 1 = copy in, step, copy out, one after the other). */
 int picsarqed_set_option(picsarqed_ctx* ctx, const char* name, long long value);
 /* With "time_kernels" = 1 every qed_step brackets its evolve pass and its event pass (offsets scan +
  * event kernel) with CUDA events on the context's stream.  get_timing synchronises, writes the
@@ -181,10 +183,11 @@ int picsarqed_generate_pairs(picsarqed_ctx* ctx, int dtype, int tau_dtype, long 
  * qed_step == evolve_optical_depth followed by generate_photons (species = lepton; s1_* = photon
  * buffers, s2_* ignored, may be NULL) or generate_pairs (species = photon; s1_* = electron,
  * s2_* = positron buffers), with identical results, ordering, capacity rule and d_n_out, but the
- * evolve pass also stages the nine reals of every particle that fires (it still has them in
- * registers), so the event pass reads dense records instead of re-scanning tau and gathering
- * scattered parents.  The staging buffer (about 14 bytes per particle in fp64) is owned by the
- * context.  This is the call bench.py times. */
+ * evolve pass also stages a record (momentum, chi^2, index) of every particle that fires (it
+ * still has them in registers), so the event pass reads dense records instead of re-scanning tau
+ * and gathering scattered parents.  The staging buffer (24 records of 48 B (fp64) or 32 B (fp32)
+ * per 128 particles, about 9 bytes per particle in fp64) is owned by the context.  This is the
+ * call bench.py times. */
 int picsarqed_qed_step(picsarqed_ctx* ctx, int species, int dtype, int tau_dtype, long long n,
                        void* px, void* py, void* pz, /* in/out */
                        const void* ex, const void* ey, const void* ez,
@@ -202,8 +205,13 @@ int picsarqed_read_count(picsarqed_ctx* ctx, const unsigned long long* d_count,
 
 /* ---- host-buffer convenience path (used for end-to-end timing) -------------------------
  * One full QED step for one species on HOST arrays: copies the nine particle/field arrays
- * and tau to device staging owned by the context, runs qed_step, copies p, tau and the secondaries back.  All pointers are
- * HOST pointers (pinned memory makes the copies asynchronous, but is not required).
+ * and tau to device staging owned by the context, runs qed_step, copies p, tau and the
+ * secondaries back.  The arrays are cut into slabs of whole evolve tiles: slab k+1 is copied in
+ * and slab k-1 copied out (three streams, full-duplex PCIe) while slab k is stepped; the slabs
+ * are chained through device counters so that the results are bit for bit those of ONE qed_step
+ * over the whole arrays (same order of the secondaries, global parent indices, same capacity
+ * rule).  All pointers are HOST pointers (pinned memory makes the copies asynchronous and lets
+ * them overlap; pageable memory works but serialises).
  * sec[0..3] (leptons: photon px,py,pz,tau) or sec[0..7] (photons: el px,py,pz,tau, po
  * px,py,pz,tau) receive min(*h_n_out, capacity) entries each.  Synchronises. */
 int picsarqed_step_host(picsarqed_ctx* ctx, int species, int dtype, int tau_dtype, long long n,

@@ -40,6 +40,10 @@ struct EventArgs {
     const unsigned char* stage_rec;           // staged records (unused for chunks flagged kStageNoRecords)
     const unsigned short* stage_cnt;          // count | flags
     const unsigned long long* tile_offset;    // [n_tiles] number of events before the tile
+    // a call that handles the slab [parent_base, parent_base + n) of a longer array (step_host): its events
+    // follow the *slot_base events of the slabs before it (device word, NULL = 0), parents are numbered globally
+    const unsigned long long* slot_base;
+    long long parent_base;
 };
 
 template <typename R, typename TR>
@@ -130,7 +134,7 @@ __device__ __forceinline__ void event_commit(const EventArgs<R, TR>& a, long lon
     for (int c = 0; c < (KIND == 0 ? 3 : 6); ++c) a.out_p[c][slot] = o.sec[c];
     a.out_tau[0][slot] = o.sec_tau[0];
     if (KIND == 1) a.out_tau[1][slot] = o.sec_tau[1];
-    if (a.parent) a.parent[slot] = i;
+    if (a.parent) a.parent[slot] = a.parent_base + i;
 #pragma unroll
     for (int c = 0; c < 3; ++c) a.p[c][i] = o.parent_p[c];
     a.tau[i] = o.parent_tau;
@@ -156,19 +160,19 @@ __global__ void __launch_bounds__(256) count_chunks_kernel(const TR* __restrict_
 }
 
 // ---- level 2: output offsets of the tiles (block-level scan) -------------------------------------
-// tile_scan_kernel: one CTA sums the chunk counts of every tile (128-bit loads of eight 16-bit counts) and scans
-// the tile sums, 4096 tiles per round (four consecutive tiles per thread), carrying the running total;
-// tile_offset[t] = number of events before tile t, *d_total = their number.
+// tile_scan_kernel: one CTA sums the chunk counts of every tile (128-bit loads of eight 16-bit counts when a tile
+// is a multiple of 8 chunks) and scans the tile sums, 4096 tiles per round (four consecutive tiles per thread),
+// carrying the running total; tile_offset[t] = number of events before tile t, *d_total = *d_base (0 when
+// d_base is NULL) + their number.  d_base chains the slabs of step_host: the events of a slab follow those of
+// the slabs before it in the secondary buffers.
 constexpr int kScanThreads = 1024;
 constexpr int kScanItems = 4;
 
-// cnt != nullptr: the tile sums are computed here as well (chunk counts summed per tile, 128-bit loads when a tile
-// is a multiple of 8 chunks); every chunk has been counted.  cnt == nullptr: they are read from tile_sum.
-__global__ void __launch_bounds__(kScanThreads) tile_scan_kernel(const unsigned int* __restrict__ tile_sum, long long n_tiles,
+__global__ void __launch_bounds__(kScanThreads) tile_scan_kernel(const unsigned short* __restrict__ cnt, long long n_chunks,
+                                                                 int chunks_per_tile, long long n_tiles,
                                                                  unsigned long long* __restrict__ tile_offset,
-                                                                 unsigned long long* __restrict__ d_total,
-                                                                 const unsigned short* __restrict__ cnt, long long n_chunks,
-                                                                 int chunks_per_tile) {
+                                                                 const unsigned long long* d_base,
+                                                                 unsigned long long* d_total) {
     __shared__ unsigned long long warp_sum[2][kScanThreads / 32];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     unsigned long long carry = 0;  // (the same value in every thread)
@@ -176,31 +180,23 @@ __global__ void __launch_bounds__(kScanThreads) tile_scan_kernel(const unsigned 
     for (long long base = 0; base < n_tiles; base += kScanThreads * kScanItems, ++round) {
         const long long t0 = base + (long long)tid * kScanItems;
         unsigned int v[kScanItems];
-        if (cnt != nullptr) {
 #pragma unroll
-            for (int k = 0; k < kScanItems; ++k) {
-                const long long c0 = (t0 + k) * chunks_per_tile;
-                unsigned int sum = 0;
-                if (t0 + k < n_tiles) {
-                    if ((chunks_per_tile & 7) == 0 && c0 + chunks_per_tile <= n_chunks) {
-                        for (int c = 0; c < chunks_per_tile; c += 8) {  // 8 counts per 128-bit load, two per word
-                            const uint4 q = *reinterpret_cast<const uint4*>(cnt + c0 + c);
-                            const unsigned int w4[4] = {q.x, q.y, q.z, q.w};
+        for (int k = 0; k < kScanItems; ++k) {
+            const long long c0 = (t0 + k) * chunks_per_tile;
+            unsigned int sum = 0;
+            if (t0 + k < n_tiles) {
+                if ((chunks_per_tile & 7) == 0 && c0 + chunks_per_tile <= n_chunks) {
+                    for (int c = 0; c < chunks_per_tile; c += 8) {  // 8 counts per 128-bit load, two per word
+                        const uint4 q = *reinterpret_cast<const uint4*>(cnt + c0 + c);
+                        const unsigned int w4[4] = {q.x, q.y, q.z, q.w};
 #pragma unroll
-                            for (int j = 0; j < 4; ++j) sum += (w4[j] & kStageCountMask) + ((w4[j] >> 16) & kStageCountMask);
-                        }
-                    } else {
-                        for (long long c = c0; c < min(c0 + (long long)chunks_per_tile, n_chunks); ++c) sum += cnt[c] & kStageCountMask;
+                        for (int j = 0; j < 4; ++j) sum += (w4[j] & kStageCountMask) + ((w4[j] >> 16) & kStageCountMask);
                     }
+                } else {
+                    for (long long c = c0; c < min(c0 + (long long)chunks_per_tile, n_chunks); ++c) sum += cnt[c] & kStageCountMask;
                 }
-                v[k] = sum;
             }
-        } else if (t0 + kScanItems <= n_tiles) {
-            const uint4 q = *reinterpret_cast<const uint4*>(tile_sum + t0);  // t0 is a multiple of 4: 16-byte aligned
-            v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
-        } else {
-#pragma unroll
-            for (int k = 0; k < kScanItems; ++k) v[k] = t0 + k < n_tiles ? tile_sum[t0 + k] : 0u;
+            v[k] = sum;
         }
         const unsigned long long s = (unsigned long long)v[0] + v[1] + v[2] + v[3];
         unsigned long long incl = s;
@@ -226,7 +222,7 @@ __global__ void __launch_bounds__(kScanThreads) tile_scan_kernel(const unsigned 
         }
         carry += all;
     }
-    if (tid == 0) *d_total = carry;
+    if (tid == 0) *d_total = (d_base ? *d_base : 0ull) + carry;
 }
 
 // ---- level 3: the events ---------------------------------------------------------------------
@@ -250,6 +246,7 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
         const long long ch = tile * CHUNKS + lane;
         return (tile < n_tiles && lane < CHUNKS && ch < n_chunks) ? a.stage_cnt[ch] : (unsigned short)0;
     };
+    const unsigned long long slot_base = a.slot_base ? *a.slot_base : 0ull;
     long long tile = blockIdx.x;
     unsigned short flags_next = load_flags(tile);
     unsigned long long excl_next = tile < n_tiles ? a.tile_offset[tile] : 0ull;
@@ -300,7 +297,7 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
             if (cand < 32 && oc <= e) j = cand;
         }
         const unsigned int off_j = __shfl_sync(0xffffffffu, off_lane, j);
-        const long long slot = (long long)(excl + e);
+        const long long slot = (long long)(slot_base + excl + e);
         if (e >= total || slot >= a.capacity) continue;  // capacity rule (R16): later parents untouched
         const unsigned int r = e - off_j;
         const long long cbase = (first_chunk + j) * kChunk;

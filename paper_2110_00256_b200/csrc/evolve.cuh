@@ -146,8 +146,9 @@ __device__ __forceinline__ auto decrement_one(R pxr, R pyr, R pzr, R exr, R eyr,
 // ---- fused evolve kernel ------------------------------------------------------------
 // V = particles per 128-bit load of R; U = independent vectors per thread per tile.  A warp owns U*32*V
 // contiguous particles of the tile (every load instruction still covers 512 contiguous bytes).
-// EMIT: also append the nine reals of every particle that fired to the staging segment of its 128-particle
-// chunk, in index order (warp ballot/popc; no CTA barrier), for staged_event_kernel.  Requires U*32*V == kChunk.
+// EMIT: also append a record (momentum, chi^2, index in chunk) of every particle that fired to the staging
+// segment of its 128-particle chunk, in index order (warp ballot/popc; no CTA barrier), for event_kernel.
+// Requires U*32*V == kChunk.
 template <typename R, typename TR, int SPECIES, int U, bool EMIT>
 __global__ void __launch_bounds__(kEvolveThreads, U > 2 ? 1 : ((sizeof(R) == 4 && U == 1 && SPECIES == 0) ? 3 : 2))
 evolve_kernel(const EvolveArgs<R, TR> a) {

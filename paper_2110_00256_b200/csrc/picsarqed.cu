@@ -16,6 +16,8 @@
 
 using namespace pxq;
 
+constexpr int kMaxSlabs = 64;
+
 struct picsarqed_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
@@ -48,7 +50,16 @@ struct picsarqed_ctx {
     // host-path staging
     void* stage = nullptr;
     size_t stage_bytes = 0;
-    unsigned long long* d_counts = nullptr;  // 2 device counters
+    // step_host pipeline: slab k is copied in on h2d_stream, stepped on stream, copied out on d2h_stream;
+    // d_counts[k] = events of the slabs before slab k (d_counts[0] = 0), so the secondaries of all slabs land
+    // densely, in parent order, in one buffer
+    unsigned long long* d_counts = nullptr;  // kMaxSlabs + 2 device counters
+    unsigned long long* h_counts = nullptr;  // pinned copy of d_counts
+    cudaStream_t h2d_stream = nullptr, d2h_stream = nullptr;
+    std::vector<cudaEvent_t> slab_events;    // 2 per slab: copied in, stepped
+    int host_slabs = 0;                      // 0 = automatic, k = split step_host into (at most) k slabs
+    const unsigned long long* link_slot_base = nullptr;  // set by step_host around the qed_step of a slab
+    long long link_parent_base = 0;
     double build_ms = 0.0;
 };
 
@@ -245,7 +256,8 @@ int picsarqed_create(picsarqed_ctx** out, int cuda_device, void* cuda_stream) {
     }
     if (e == cudaSuccess) e = cudaMalloc(&c->ticket, sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaMemset(c->ticket, 0, sizeof(unsigned int));
-    if (e == cudaSuccess) e = cudaMalloc(&c->d_counts, 2 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_counts, (kMaxSlabs + 2) * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMallocHost(&c->h_counts, (kMaxSlabs + 2) * sizeof(unsigned long long));
     if (e != cudaSuccess) {
         delete c;
         return PICSARQED_ERR_CUDA;
@@ -271,6 +283,10 @@ int picsarqed_destroy(picsarqed_ctx* c) {
     cudaFree(c->d_scalar);
     for (cudaEvent_t e : c->timing_events) cudaEventDestroy(e);
     cudaFree(c->d_counts);
+    cudaFreeHost(c->h_counts);
+    for (cudaEvent_t e : c->slab_events) cudaEventDestroy(e);
+    if (c->h2d_stream) cudaStreamDestroy(c->h2d_stream);
+    if (c->d2h_stream) cudaStreamDestroy(c->d2h_stream);
     delete c;
     return PICSARQED_OK;
 }
@@ -287,6 +303,8 @@ int picsarqed_set_option(picsarqed_ctx* c, const char* name, long long value) {
         c->time_kernels = (int)value;
     else if (!std::strcmp(name, "event_config") && value >= 0 && value <= 7)
         c->event_config = (int)value;
+    else if (!std::strcmp(name, "host_slabs") && value >= 0 && value <= kMaxSlabs)
+        c->host_slabs = (int)value;
     else
         return fail(c, PICSARQED_ERR_INVALID, std::string("unknown option or bad value: ") + name);
     return PICSARQED_OK;
@@ -420,28 +438,26 @@ int launch_evolve(picsarqed_ctx* c, long long n, const void* const* a, double dt
 }
 
 // per-chunk scratch: [records][counts][offsets]
-struct ChunkScratch { unsigned char* rec; unsigned short* cnt; unsigned long long* off; unsigned int* sum; long long n_chunks; };
+struct ChunkScratch { unsigned char* rec; unsigned short* cnt; unsigned long long* off; long long n_chunks; };
 
 template <typename R>
 int chunk_scratch(picsarqed_ctx* c, long long n, ChunkScratch* out) {
     const long long nchunks = (n + kChunk - 1) / kChunk;
     const size_t rec_sz = ((size_t)nchunks * kStageCap * StageRecord<R>::kBytes + 255) & ~(size_t)255;
     const size_t cnt_sz = ((size_t)nchunks * sizeof(unsigned short) + 255) & ~(size_t)255;
-    // tiles hold at least 8 chunks: n_chunks/8 + 1 tile offsets and tile sums are always enough
+    // tiles hold at least 8 chunks: n_chunks/8 + 1 tile offsets are always enough
     const size_t off_sz = ((size_t)(nchunks / 8 + 2) * sizeof(unsigned long long) + 255) & ~(size_t)255;
-    const size_t sum_sz = ((size_t)(nchunks / 8 + 2) * sizeof(unsigned int) + 255) & ~(size_t)255;
-    if (rec_sz + cnt_sz + off_sz + sum_sz > c->rec_bytes) {  // grow (rare; synchronises)
+    if (rec_sz + cnt_sz + off_sz > c->rec_bytes) {  // grow (rare; synchronises)
         PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
         if (c->rec) cudaFree(c->rec);
         c->rec = nullptr;
         c->rec_bytes = 0;
-        PXQ_CUDA(c, cudaMalloc(&c->rec, rec_sz + cnt_sz + off_sz + sum_sz));
-        c->rec_bytes = rec_sz + cnt_sz + off_sz + sum_sz;
+        PXQ_CUDA(c, cudaMalloc(&c->rec, rec_sz + cnt_sz + off_sz));
+        c->rec_bytes = rec_sz + cnt_sz + off_sz;
     }
     out->rec = static_cast<unsigned char*>(c->rec);
     out->cnt = reinterpret_cast<unsigned short*>(out->rec + rec_sz);
     out->off = reinterpret_cast<unsigned long long*>(out->rec + rec_sz + cnt_sz);
-    out->sum = reinterpret_cast<unsigned int*>(out->rec + rec_sz + cnt_sz + off_sz);
     out->n_chunks = nchunks;
     return PICSARQED_OK;
 }
@@ -471,10 +487,12 @@ int launch_event_pass(picsarqed_ctx* c, long long n, const ChunkScratch& cs, voi
     ev.stage_rec = cs.rec;
     ev.stage_cnt = cs.cnt;
     ev.tile_offset = cs.off;
+    ev.slot_base = c->link_slot_base;
+    ev.parent_base = c->link_parent_base;
     static const int kChunksOf[8] = {24, 32, 24, 16, 12, 24, 24, 32};  // must match the switch below
     const int chunks = kChunksOf[c->event_config];
     const long long n_tiles = (cs.n_chunks + chunks - 1) / chunks;
-    tile_scan_kernel<<<1, kScanThreads, 0, c->stream>>>(nullptr, n_tiles, cs.off, d_n_out, cs.cnt, cs.n_chunks, chunks);
+    tile_scan_kernel<<<1, kScanThreads, 0, c->stream>>>(cs.cnt, cs.n_chunks, chunks, n_tiles, cs.off, c->link_slot_base, d_n_out);
 #define PXQ_LAUNCH_EVENTS(T, CH, MB)                                                                         \
     do {                                                                                                     \
         auto kern = event_kernel<R, TR, KIND, T, CH, MB>;                                                    \
@@ -772,25 +790,71 @@ extern "C" int picsarqed_step_host(picsarqed_ctx* c, int species, int dtype, int
     for (int k = 0; k < n_sec_tau; ++k) d_sec_tau[k] = sec0 + n_sec * sp_bytes + k * st_bytes;
     long long* d_parent = reinterpret_cast<long long*>(sec0 + n_sec * sp_bytes + n_sec_tau * st_bytes);
 
-    const void* h_in[9] = {h_px, h_py, h_pz, h_ex, h_ey, h_ez, h_bx, h_by, h_bz};
-    for (int k = 0; k < 9; ++k) {
+    const void* h_in[10] = {h_px, h_py, h_pz, h_ex, h_ey, h_ez, h_bx, h_by, h_bz, h_tau};
+    for (int k = 0; k < 10; ++k)
         if (!h_in[k]) return fail(c, PICSARQED_ERR_INVALID, "null host array");
-        PXQ_CUDA(c, cudaMemcpyAsync(d[k], h_in[k], (size_t)n * es, cudaMemcpyHostToDevice, c->stream));
-    }
-    if (!h_tau) return fail(c, PICSARQED_ERR_INVALID, "null host tau");
-    PXQ_CUDA(c, cudaMemcpyAsync(d[9], h_tau, (size_t)n * ts, cudaMemcpyHostToDevice, c->stream));
+    void* h_back[4] = {h_px, h_py, h_pz, h_tau};
+    const int back_of[4] = {0, 1, 2, 9};
 
-    int rc = picsarqed_qed_step(c, species, dtype, tau_dtype, n, d[0], d[1], d[2], d[3], d[4], d[5], d[6], d[7], d[8],
-                                d[9], dt, seed, step, id_base, capacity, d_sec_p[0], d_sec_p[1], d_sec_p[2],
-                                d_sec_tau[0], d_sec_p[3], d_sec_p[4], d_sec_p[5], d_sec_tau[1],
-                                h_parent ? d_parent : nullptr, c->d_counts);
-    if (rc) return rc;
-    void* h_p[3] = {h_px, h_py, h_pz};
-    for (int k = 0; k < 3; ++k)
-        PXQ_CUDA(c, cudaMemcpyAsync(h_p[k], d[k], (size_t)n * es, cudaMemcpyDeviceToHost, c->stream));
-    PXQ_CUDA(c, cudaMemcpyAsync(h_tau, d[9], (size_t)n * ts, cudaMemcpyDeviceToHost, c->stream));
-    PXQ_CUDA(c, cudaMemcpyAsync(h_n_out, c->d_counts, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+    // Slabs of whole evolve tiles, at least 1 Mi particles each: while slab k is stepped, slab k+1 is on its way
+    // in and slab k-1 on its way out (PCIe is full duplex; the copies are asynchronous for pinned host memory).
+    // The slabs are stepped in order on one stream and chained through d_counts, so the results (secondaries,
+    // their order, the capacity rule) are those of one qed_step over the whole array.
+    long long slab = n;
+    int n_slabs = 1;
+    {
+        const long long kMinSlab = 1 << 20;
+        int want = c->host_slabs > 0 ? c->host_slabs : (int)std::min<long long>(32, n / kMinSlab);
+        if (want > 1) {
+            slab = ((n + want - 1) / want + 1023) / 1024 * 1024;
+            n_slabs = (int)((n + slab - 1) / slab);
+        }
+    }
+    if (!c->h2d_stream) PXQ_CUDA(c, cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking));
+    if (!c->d2h_stream) PXQ_CUDA(c, cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking));
+    while ((int)c->slab_events.size() < 2 * n_slabs) {
+        cudaEvent_t e;
+        PXQ_CUDA(c, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        c->slab_events.push_back(e);
+    }
+    struct LinkReset {  // the link must not outlive this call, whatever path leaves it
+        picsarqed_ctx* c;
+        ~LinkReset() { c->link_slot_base = nullptr; c->link_parent_base = 0; }
+    } link_reset{c};
+    PXQ_CUDA(c, cudaMemsetAsync(c->d_counts, 0, sizeof(unsigned long long), c->stream));
+    for (int s = 0; s < n_slabs; ++s) {
+        const long long i0 = (long long)s * slab, m = std::min(slab, n - i0);
+        cudaEvent_t copied_in = c->slab_events[2 * s], stepped = c->slab_events[2 * s + 1];
+        for (int k = 0; k < 10; ++k) {
+            const size_t w = k == 9 ? ts : es;
+            PXQ_CUDA(c, cudaMemcpyAsync(static_cast<char*>(d[k]) + (size_t)i0 * w,
+                                        static_cast<const char*>(h_in[k]) + (size_t)i0 * w, (size_t)m * w,
+                                        cudaMemcpyHostToDevice, c->h2d_stream));
+        }
+        PXQ_CUDA(c, cudaEventRecord(copied_in, c->h2d_stream));
+        PXQ_CUDA(c, cudaStreamWaitEvent(c->stream, copied_in, 0));
+        void* ds[10];
+        for (int k = 0; k < 10; ++k) ds[k] = static_cast<char*>(d[k]) + (size_t)i0 * (k == 9 ? ts : es);
+        c->link_slot_base = c->d_counts + s;
+        c->link_parent_base = i0;
+        int rc = picsarqed_qed_step(c, species, dtype, tau_dtype, m, ds[0], ds[1], ds[2], ds[3], ds[4], ds[5], ds[6],
+                                    ds[7], ds[8], ds[9], dt, seed, step, id_base + (unsigned long long)i0, capacity,
+                                    d_sec_p[0], d_sec_p[1], d_sec_p[2], d_sec_tau[0], d_sec_p[3], d_sec_p[4],
+                                    d_sec_p[5], d_sec_tau[1], h_parent ? d_parent : nullptr, c->d_counts + s + 1);
+        if (rc) return rc;
+        PXQ_CUDA(c, cudaEventRecord(stepped, c->stream));
+        PXQ_CUDA(c, cudaStreamWaitEvent(c->d2h_stream, stepped, 0));
+        for (int k = 0; k < 4; ++k) {
+            const size_t w = k == 3 ? ts : es;
+            PXQ_CUDA(c, cudaMemcpyAsync(static_cast<char*>(h_back[k]) + (size_t)i0 * w,
+                                        static_cast<const char*>(d[back_of[k]]) + (size_t)i0 * w, (size_t)m * w,
+                                        cudaMemcpyDeviceToHost, c->d2h_stream));
+        }
+    }
+    PXQ_CUDA(c, cudaMemcpyAsync(c->h_counts, c->d_counts + n_slabs, sizeof(unsigned long long), cudaMemcpyDeviceToHost,
+                                c->stream));
     PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    *h_n_out = c->h_counts[0];
     const size_t m = (size_t)std::min<unsigned long long>(*h_n_out, (unsigned long long)capacity);
     if (m > 0 && h_sec) {
         // order of h_sec: leptons: ph px,py,pz,tau; photons: el px,py,pz,tau, po px,py,pz,tau
@@ -808,6 +872,7 @@ extern "C" int picsarqed_step_host(picsarqed_ctx* c, int species, int dtype, int
         if (h_parent) PXQ_CUDA(c, cudaMemcpyAsync(h_parent, d_parent, m * sizeof(long long), cudaMemcpyDeviceToHost, c->stream));
         PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
     }
+    PXQ_CUDA(c, cudaStreamSynchronize(c->d2h_stream));
     return PICSARQED_OK;
 }
 

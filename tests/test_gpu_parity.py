@@ -406,6 +406,48 @@ def test_fused_step_repeated_launches(qed, ctx):
 
 
 @pytest.mark.parametrize("species", [LEPTON, PHOTON])
+@pytest.mark.parametrize("dtype,tdtype", [(np.float64, np.float64), (np.float32, np.float32), (np.float32, np.float64)])
+def test_step_host_pipeline(orc, qed, ctx, mid_tables, species, dtype, tdtype):
+    """picsarqed_step_host (host buffers, slabs pipelined over three streams and chained through device counters)
+    == one picsarqed_qed_step over the whole array, bit for bit: momenta, optical depths, secondaries, their
+    order, global parent indices, the count and the capacity rule across slab borders.  qed_step itself is held
+    to the oracle on these inputs by test_fused_step."""
+    import torch
+    pdt = torch.float64 if dtype == np.float64 else torch.float32
+    tdt = torch.float64 if tdtype == np.float64 else torch.float32
+    nsec = 1 if species == LEPTON else 2
+    try:
+        for n in (3 * 4096 + 77, 8192, 300):
+            p, e, b = qed.workloads.config1(seed=33, n=n, species=species, dtype=dtype)
+            tables = _tables_for(mid_tables, dtype)
+            dt = qed.workloads.choose_dt(orc.rate(tables, species, p, e, b), 0.2)
+            tau0 = orc.init_optical_depth(species, code(tdtype), n, 6).astype(tdtype)
+            for cap in (n, max(1, n // 40)):
+                f = _run_fused(qed, ctx, species, dtype, tdtype, p, e, b, tau0, dt, 78, 3, 987654321, cap)
+                m = min(f["n_fired"], cap)
+                assert f["n_fired"] > cap or cap == n
+                for slabs in (0, 1, 3, 7):
+                    ctx.set_option("host_slabs", slabs)
+                    hp = [torch.from_numpy(np.ascontiguousarray(x)).pin_memory() for x in p]
+                    he = [torch.from_numpy(np.ascontiguousarray(x)).pin_memory() for x in e]
+                    hb = [torch.from_numpy(np.ascontiguousarray(x)).pin_memory() for x in b]
+                    htau = torch.from_numpy(tau0.copy()).pin_memory()
+                    sec = [torch.full((cap,), -7.0, dtype=tdt if k % 4 == 3 else pdt).pin_memory() for k in range(4 * nsec)]
+                    parent = torch.full((cap,), -1, dtype=torch.int64).pin_memory()
+                    fired = ctx.step_host(species, hp, he, hb, htau, dt, 78, 3, 987654321, cap, sec, parent)
+                    assert fired == f["n_fired"], (n, cap, slabs)
+                    assert _same(htau.numpy(), f["tau"]) and all(_same(x.numpy(), y) for x, y in zip(hp, f["p"]))
+                    assert _same(parent.numpy()[:m], f["parent"][:m]) and bool((parent[m:] == -1).all())
+                    for s_ in range(nsec):
+                        for k in range(3):
+                            assert _same(sec[4 * s_ + k].numpy()[:m], f["sec_p"][s_][k][:m])
+                        assert _same(sec[4 * s_ + 3].numpy()[:m], f["sec_tau"][s_][:m])
+                        assert bool((sec[4 * s_ + 3][m:] == -7.0).all())
+    finally:
+        ctx.set_option("host_slabs", 0)
+
+
+@pytest.mark.parametrize("species", [LEPTON, PHOTON])
 def test_evolve_decrement_accuracy_fp64(orc, qed, ctx, mid_tables, species):
     """the decrement itself (tau_old = 0), far tighter than the 1e-9 of the north star: the kernel uses its own lean
     log/exp/rcp/rsqrt, whose errors must stay at the few-ulp level; the bound is the conditioning of the lookup"""
