@@ -28,8 +28,9 @@ UNIT = "particles/s"
 SEED = 2
 BYTES_PER_PARTICLE_EVOLVE = 88  # 9 reads + tau read + tau write, fp64
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the evolve pass (16 Mi particles), ncu --set full:
-# profiles/r1b_evolve_emit_full.md
-EVOLVE_DRAM_TRAFFIC_BYTES = 1343862000 + 157025000
+# profiles/r1c_step_full.md (1.343656 GB read = the 80 B/particle of inputs; 109 MB written: part of the 134 MB of
+# new tau is still dirty in L2 when the kernel ends, plus the staged records)
+EVOLVE_DRAM_TRAFFIC_BYTES = 1343656000 + 109172224
 
 
 def parse():
@@ -280,7 +281,7 @@ def run_ours(args):
         return
     peaks, peak_kind = measured_peaks()
     # dominant kernel: the evolve pass (evolve_kernel<double,double,LEPTON,2,EMIT>): 88 algorithmic bytes per particle
-    # (SURVEY.md 8(d)); the 80-byte records it stages for the ~5 % that fire are not counted as algorithmic
+    # (SURVEY.md 8(d)); the 48-byte records it stages for the ~5 % that fire are not counted as algorithmic
     evolve_bytes = BYTES_PER_PARTICLE_EVOLVE * n
     achieved = evolve_bytes / (ms_evolve * 1e-3) / 1e9
     line = {
