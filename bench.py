@@ -42,7 +42,7 @@ def parse():
     ap.add_argument("--particles", type=int, default=1 << 24, help="particles per GPU (default 16 Mi = config 2)")
     ap.add_argument("--field-sets", type=int, default=4, help="distinct per-step field sets kept in HBM")
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--cpu-sample", type=int, default=1 << 21, help="particles in the oracle timing sample")
+    ap.add_argument("--cpu-sample", type=int, default=1 << 23, help="particles in the oracle timing sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -141,7 +141,7 @@ def run_reference(args):
     dt = w.choose_dt(oracle.rate(oracle_tables_from(tp, tables), 0, p0, e0, b0), 0.05)  # the 5 % rule
     for _ in range(max(0, min(args.warmup, 1))):
         time_oracle(tp, tables, min(n, 1 << 16), 1, dt)
-    # bound the run: at ~1.5e6 particle-steps/s a 2 Mi sample takes ~1.5 s per step
+    # bound the run: at ~4e6 particle-steps/s an 8 Mi sample takes ~2 s per step
     steps_run = min(steps, 8)
     value, sec, threads = time_oracle(tp, tables, n, steps_run, dt)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps_run,
@@ -311,7 +311,7 @@ def run_ours(args):
     if not args.no_cpu_baseline and world == 1:
         tables = [ctx.export_tables(k) for k in range(4)]
         ns = min(args.cpu_sample, n)
-        steps_cpu = 4
+        steps_cpu = 6  # 8 Mi x 6 particle-steps: 10-15 s on 16 host cores
         v, sec, threads = time_oracle(tp_kwargs, tables, ns, steps_cpu, dt)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
                                 "sample": "first %d particles of the workload x %d steps (evolve + photon emission), "
