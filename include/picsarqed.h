@@ -223,6 +223,67 @@ int picsarqed_step_host(picsarqed_ctx* ctx, int species, int dtype, int tau_dtyp
                         unsigned long long id_base, long long capacity,
                         void* const* h_sec, long long* h_parent, unsigned long long* h_n_out);
 
+/* ---- closed loop in a uniform field ----------------
+ * The paper validates the library inside a PIC code on populations in static uniform fields
+ * (Ridgers cases (i), (iii)): leptons are pushed, every species takes its QED step, the
+ * secondaries join the populations, photons below an energy threshold are dropped at creation,
+ * energy spectra are compared (Fig.6).  These calls are the pieces around qed_step that this
+ * needs; cascade_step strings them together.  Units as everywhere: p in m_e c, e = E/E_s,
+ * b = cB/E_s, dt in seconds. */
+
+/* Boris push of n leptons of charge sign `charge_sign` (-1 electron, +1 positron) by dt in the
+ * uniform fields e[3], b[3] (HOST arrays of three doubles): half kick, rotation with
+ * t = s b dt/(2 tau_C gamma^-), half kick; du/dt = s (e + u x b/gamma)/tau_C, tau_C = hbar/(m_e c^2)
+ * (R19).  px, py, pz: device, in/out.  fp64 arithmetic whatever `dtype`. */
+int picsarqed_boris_push_uniform(picsarqed_ctx* ctx, int dtype, long long n, void* px, void* py, void* pz,
+                                 int charge_sign, const double* e, const double* b, double dt);
+
+/* Ordered, filtering append (R20, R22): of the first m = min(*d_count, m_max) entries
+ * of the source arrays s_* (device; *d_count is a device counter such as qed_step's d_n_out),
+ * those with sqrt(px^2+py^2+pz^2) >= min_energy (photons below the threshold are
+ * discarded right after creation; min_energy = 0 keeps everything) are copied, in order, to
+ * d_*[dst_n ...] (device arrays of dst_capacity entries).  *d_new_n (device, 8 bytes) receives
+ * dst_n + number kept; entries that would land at or past dst_capacity are not written, so the
+ * caller detects overflow by *d_new_n > dst_capacity. */
+int picsarqed_append_secondaries(picsarqed_ctx* ctx, int dtype, int tau_dtype, long long m_max,
+                                 const void* s_px, const void* s_py, const void* s_pz, const void* s_tau,
+                                 const unsigned long long* d_count, double min_energy,
+                                 void* d_px, void* d_py, void* d_pz, void* d_tau,
+                                 long long dst_n, long long dst_capacity, unsigned long long* d_new_n);
+
+/* Energy spectrum (Fig.6; R23): adds to hist[nbins] (device, 64-bit counters, NOT
+ * zeroed here) the number of particles per logarithmic bin of [e_min, e_max) of the kinetic energy
+ * gamma - 1 (leptons) or gamma_gamma = |p| (photons); bin = floor((ln E - ln e_min) nbins /
+ * (ln e_max - ln e_min)) in fp64.  Dead entries (p = 0) and energies outside the range are not
+ * counted.  1 <= nbins <= 8192. */
+int picsarqed_energy_spectrum(picsarqed_ctx* ctx, int species, int dtype, long long n,
+                              const void* px, const void* py, const void* pz,
+                              double e_min, double e_max, int nbins, unsigned long long* hist);
+
+/* One species of the closed loop: device structure of arrays with room for `capacity` entries, the
+ * first n in use.  Positions never change (a photon that decayed stays as p = 0, tau = +inf), so the
+ * Philox id of a particle is id_base + position for its lifetime (R21). */
+typedef struct picsarqed_species_arrays {
+    void *px, *py, *pz, *tau;
+    long long n;        /* in/out */
+    long long capacity;
+    unsigned long long id_base;
+} picsarqed_species_arrays;
+
+/* One time step of the closed loop in the order of DESIGN.md R20: push electrons (s = -1) and
+ * positrons (+1); qed_step of electrons, positrons, photons in the uniform field (each on the
+ * entries that existed when the step began); append the photons of the electrons, then those of
+ * the positrons (min_energy = photon_min_energy), and the pairs.  Updates n of the three species
+ * (one 24-byte device-to-host read per step) and writes the event counts (electrons, positrons,
+ * photons) to h_events[3] if it is not NULL.  Scratch (constant field arrays, secondary buffers) is
+ * owned by the context.  PICSARQED_ERR_INVALID if a species would exceed its capacity (its n is
+ * then clipped to the capacity and the entries that did not fit are lost). */
+int picsarqed_cascade_step(picsarqed_ctx* ctx, int dtype, int tau_dtype,
+                           picsarqed_species_arrays* electrons, picsarqed_species_arrays* positrons,
+                           picsarqed_species_arrays* photons, const double* e, const double* b, double dt,
+                           unsigned long long seed, unsigned long long step, double photon_min_energy,
+                           int push, unsigned long long* h_events);
+
 #ifdef __cplusplus
 }
 #endif

@@ -5,5 +5,5 @@
 """
 from . import workloads  # noqa: F401
 from .binding import (F32, F64, LEPTON, PHOTON, TAB_BW_P, TAB_LNG, TAB_LNT, TAB_QS_LNP, Context,  # noqa: F401
-                      PicsarQedError, TableParams, lib)
+                      PicsarQedError, Species, TableParams, lib)
 from .build import build, lib_path  # noqa: F401

@@ -19,6 +19,11 @@ TAB_LNG, TAB_QS_LNP, TAB_LNT, TAB_BW_P = 0, 1, 2, 3
 _vp, _u64, _i64, _i, _d = C.c_void_p, C.c_uint64, C.c_longlong, C.c_int, C.c_double
 
 
+class _CSpecies(C.Structure):
+    _fields_ = [("px", _vp), ("py", _vp), ("pz", _vp), ("tau", _vp), ("n", _i64), ("capacity", _i64),
+                ("id_base", _u64)]
+
+
 class _CParams(C.Structure):
     _fields_ = [("qs_chi_min", _d), ("qs_chi_max", _d), ("qs_n_chi", _i), ("qs_xi_min", _d),
                 ("qs_n_xi", _i), ("bw_chi_min", _d), ("bw_chi_max", _d), ("bw_n_chi", _i),
@@ -66,6 +71,11 @@ _SIGNATURES = {
     "picsarqed_read_count": (_i, [_vp, _vp, C.POINTER(_u64)]),
     "picsarqed_step_host": (_i, [_vp, _i, _i, _i, _i64] + [_vp] * 10 + [_d, _u64, _u64, _u64, _i64, _vp, _vp,
                                                                      C.POINTER(_u64)]),
+    "picsarqed_boris_push_uniform": (_i, [_vp, _i, _i64, _vp, _vp, _vp, _i, C.POINTER(_d), C.POINTER(_d), _d]),
+    "picsarqed_append_secondaries": (_i, [_vp, _i, _i, _i64] + [_vp] * 5 + [_d] + [_vp] * 4 + [_i64, _i64, _vp]),
+    "picsarqed_energy_spectrum": (_i, [_vp, _i, _i, _i64, _vp, _vp, _vp, _d, _d, _i, _vp]),
+    "picsarqed_cascade_step": (_i, [_vp, _i, _i, C.POINTER(_CSpecies), C.POINTER(_CSpecies), C.POINTER(_CSpecies),
+                                    C.POINTER(_d), C.POINTER(_d), _d, _u64, _u64, _d, _i, C.POINTER(_u64)]),
 }
 
 _lib = None
@@ -255,3 +265,53 @@ class Context:
             tau.data_ptr(), float(dt), seed, step, id_base, capacity, C.cast(sec_ptrs, _vp),
             parent.data_ptr() if parent is not None else None, C.byref(n_out)))
         return int(n_out.value)
+
+    # ---- closed loop in a uniform field ------------------------------
+    def boris_push_uniform(self, p, charge_sign, e, b, dt):
+        d = p[0].dtype
+        self._check(lib().picsarqed_boris_push_uniform(
+            self._h, _code(d), p[0].numel(), *[_dev(t, d) for t in p], int(charge_sign), (_d * 3)(*e), (_d * 3)(*b),
+            float(dt)))
+
+    def append_secondaries(self, m_max, src_p, src_tau, count, min_energy, dst_p, dst_tau, dst_n, new_n):
+        """ordered, filtering append of the first min(count, m_max) source entries to dst[dst_n:]"""
+        d = src_p[0].dtype
+        self._check(lib().picsarqed_append_secondaries(
+            self._h, _code(d), _code(src_tau.dtype), m_max, *[_dev(t, d) for t in src_p], _dev(src_tau),
+            _dev(count, torch.int64), float(min_energy), *[_dev(t, d) for t in dst_p], _dev(dst_tau, src_tau.dtype),
+            dst_n, dst_tau.numel(), _dev(new_n, torch.int64)))
+
+    def energy_spectrum(self, species, p, e_min, e_max, hist):
+        d = p[0].dtype
+        self._check(lib().picsarqed_energy_spectrum(
+            self._h, species, _code(d), p[0].numel(), *[_dev(t, d) for t in p], float(e_min), float(e_max),
+            hist.numel(), _dev(hist, torch.int64)))
+
+    def cascade_step(self, pops, e, b, dt, seed, step, photon_min_energy=0.0, push=True):
+        """one time step of the closed loop; pops: dict electrons / positrons / photons -> Species.
+        Returns the event counts (electrons, positrons, photons)."""
+        cs = {k: pops[k]._c() for k in ("electrons", "positrons", "photons")}
+        d, td = pops["electrons"].p[0].dtype, pops["electrons"].tau.dtype
+        ev = (_u64 * 3)()
+        rc = lib().picsarqed_cascade_step(
+            self._h, _code(d), _code(td), C.byref(cs["electrons"]), C.byref(cs["positrons"]), C.byref(cs["photons"]),
+            (_d * 3)(*e), (_d * 3)(*b), float(dt), seed, step, float(photon_min_energy), int(bool(push)), ev)
+        for k in cs:
+            pops[k].n = int(cs[k].n)
+        self._check(rc)
+        return tuple(int(v) for v in ev)
+
+
+class Species:
+    """device structure of arrays with room for `capacity` entries, the first n in use (picsarqed_species_arrays)"""
+
+    def __init__(self, capacity, dtype, tau_dtype, id_base, device="cuda"):
+        self.p = [torch.zeros(capacity, dtype=dtype, device=device) for _ in range(3)]
+        self.tau = torch.zeros(capacity, dtype=tau_dtype, device=device)
+        self.n = 0
+        self.capacity = capacity
+        self.id_base = id_base
+
+    def _c(self):
+        return _CSpecies(self.p[0].data_ptr(), self.p[1].data_ptr(), self.p[2].data_ptr(), self.tau.data_ptr(), self.n,
+                         self.capacity, self.id_base)

@@ -1,0 +1,180 @@
+// =====================================================================================
+//  cascade.cuh -- the closed loop in a uniform field:
+//  what surrounds the QED step when secondaries are fed back.
+//    boris_kernel        leptons pushed in uniform e, b (R19)                       HBM, 48/24 B per particle
+//    keep_count_kernel   \  ordered, filtering append of the new secondaries to a species'
+//    append_kernel       /  arrays: photons below the energy threshold are discarded at
+//                           creation (R22); order is kept (ballot/popc + the
+//                           block scan of events.cuh)
+//    spectrum_kernel     energy histogram over logarithmic bins (Fig.6, R23)                   HBM, 24/12 B per particle
+//    fill_kernel         constant field arrays for the QED step
+// =====================================================================================
+#pragma once
+#include "qed_device.cuh"
+#include "evolve.cuh"
+
+namespace pxq {
+
+constexpr double kInvTauC = kElectronMass * kLightSpeed * kLightSpeed / (kPlanck / (2.0 * kPi));  // m c^2/hbar, 1/s
+
+// ---- Boris push in a uniform field (R19) ---------------------------------------------------------------
+// ke = s dt/(2 tau_C) e, kb = s dt/(2 tau_C) b (host, fp64).  Arithmetic in fp64 registers whatever R.
+struct BorisArgs {
+    double ke[3], kb[3];
+};
+
+__device__ __forceinline__ void boris_one(double& ux, double& uy, double& uz, const BorisArgs& a) {
+    const double mx = ux + a.ke[0], my = uy + a.ke[1], mz = uz + a.ke[2];            // half electric kick
+    const double inv_g = rsqrt_fast(1.0 + fma(mx, mx, fma(my, my, mz * mz)));        // 1/gamma^-
+    const double tx = a.kb[0] * inv_g, ty = a.kb[1] * inv_g, tz = a.kb[2] * inv_g;    // rotation vector
+    const double px = mx + (my * tz - mz * ty);                                       // u' = u^- + u^- x t
+    const double py = my + (mz * tx - mx * tz);
+    const double pz = mz + (mx * ty - my * tx);
+    const double f = 2.0 * rcp_fast(1.0 + fma(tx, tx, fma(ty, ty, tz * tz)));
+    const double sx = f * tx, sy = f * ty, sz = f * tz;
+    ux = mx + (py * sz - pz * sy) + a.ke[0];                                          // u^+ = u^- + u' x s, second half kick
+    uy = my + (pz * sx - px * sz) + a.ke[1];
+    uz = mz + (px * sy - py * sx) + a.ke[2];
+}
+
+template <typename R>
+__global__ void __launch_bounds__(256) boris_kernel(R* __restrict__ px, R* __restrict__ py, R* __restrict__ pz, long long n,
+                                                    const BorisArgs a) {
+    constexpr int V = 16 / sizeof(R);
+    const long long nvec = n / V;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const unsigned long long pol = l2_policy_evict_first();
+    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < nvec; j += stride) {
+        Vec<R, V> x = ld_stream_rw<R, V>(px + j * V, pol), y = ld_stream_rw<R, V>(py + j * V, pol),
+                  z = ld_stream_rw<R, V>(pz + j * V, pol);
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            double ux = x.v[v], uy = y.v[v], uz = z.v[v];
+            boris_one(ux, uy, uz, a);
+            x.v[v] = (R)ux; y.v[v] = (R)uy; z.v[v] = (R)uz;
+        }
+        *reinterpret_cast<Vec<R, V>*>(px + j * V) = x;
+        *reinterpret_cast<Vec<R, V>*>(py + j * V) = y;
+        *reinterpret_cast<Vec<R, V>*>(pz + j * V) = z;
+    }
+    for (long long i = nvec * V + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        double ux = px[i], uy = py[i], uz = pz[i];
+        boris_one(ux, uy, uz, a);
+        px[i] = (R)ux; py[i] = (R)uy; pz[i] = (R)uz;
+    }
+}
+
+// ---- ordered, filtering append (R20, R22) -----------------------------------------------------------
+// keep(i) = !(|p_i| < min_energy), |p| = sqrt((px^2 + py^2) + pz^2) with every operation rounded separately
+// (no fma): the decision is then the one an fp64 evaluation of the same expression takes anywhere.
+template <typename R>
+__device__ __forceinline__ bool keep_entry(const R* px, const R* py, const R* pz, long long i, double min_energy) {
+    const double x = px[i], y = py[i], z = pz[i];
+    const double g = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)), __dmul_rn(z, z)));
+    return !(g < min_energy);
+}
+
+// level 1: one warp per 128-entry chunk of the source; m = min(*d_count, m_max) valid entries
+template <typename R>
+__global__ void __launch_bounds__(256) keep_count_kernel(const R* __restrict__ px, const R* __restrict__ py,
+                                                         const R* __restrict__ pz, const unsigned long long* d_count,
+                                                         long long m_max, double min_energy, long long n_chunks,
+                                                         unsigned short* __restrict__ cnt) {
+    const int lane = threadIdx.x & 31;
+    const long long m = (long long)min((unsigned long long)m_max, *d_count);
+    const long long warps = (long long)gridDim.x * (blockDim.x / 32);
+    for (long long ch = (long long)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); ch < n_chunks; ch += warps) {
+        unsigned int k = 0;
+#pragma unroll
+        for (int r4 = 0; r4 < kChunk / 32; ++r4) {
+            const long long i = ch * kChunk + r4 * 32 + lane;
+            const bool f = i < m && keep_entry(px, py, pz, i, min_energy);
+            k += __popc(__ballot_sync(0xffffffffu, f));
+        }
+        if (lane == 0) cnt[ch] = (unsigned short)k;
+    }
+}
+
+constexpr int kAppendChunksPerTile = 8;
+
+// level 3 (level 2 is tile_scan_kernel with kAppendChunksPerTile): entry i of the source that is kept goes to
+// dst[dst_n + (number of kept entries before i)]; entries past dst_capacity are dropped, *d_new_n = dst_n + kept
+// tells (the caller checks it against the capacity)
+template <typename R, typename TR>
+struct AppendArgs {
+    const R* s_p[3];
+    const TR* s_tau;
+    R* d_p[3];
+    TR* d_tau;
+    const unsigned long long* d_count;
+    long long m_max, dst_n, dst_capacity, n_chunks;
+    const unsigned long long* d_dst_n;   // not NULL: the destination starts at *d_dst_n instead of dst_n
+    double min_energy;
+    const unsigned short* cnt;
+    const unsigned long long* tile_offset;
+    const unsigned long long* d_kept;
+    unsigned long long* d_new_n;
+};
+
+template <typename R, typename TR>
+__global__ void __launch_bounds__(256) append_kernel(const AppendArgs<R, TR> a) {
+    const int lane = threadIdx.x & 31;
+    const long long m = (long long)min((unsigned long long)a.m_max, *a.d_count);
+    const long long dst_n = a.d_dst_n ? (long long)*a.d_dst_n : a.dst_n;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *a.d_new_n = (unsigned long long)dst_n + *a.d_kept;
+    const long long warps = (long long)gridDim.x * (blockDim.x / 32);
+    for (long long ch = (long long)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); ch < a.n_chunks; ch += warps) {
+        const long long tile = ch / kAppendChunksPerTile;
+        const int in_tile = (int)(ch - tile * kAppendChunksPerTile);
+        const unsigned int c = lane < in_tile ? a.cnt[tile * kAppendChunksPerTile + lane] : 0u;   // chunks before this one
+        long long slot = dst_n + (long long)a.tile_offset[tile] + __reduce_add_sync(0xffffffffu, c);
+#pragma unroll
+        for (int r4 = 0; r4 < kChunk / 32; ++r4) {
+            const long long i = ch * kChunk + r4 * 32 + lane;
+            const bool f = i < m && keep_entry(a.s_p[0], a.s_p[1], a.s_p[2], i, a.min_energy);
+            const unsigned int bal = __ballot_sync(0xffffffffu, f);
+            const long long d = slot + __popc(bal & ((1u << lane) - 1u));
+            if (f && d < a.dst_capacity) {
+#pragma unroll
+                for (int k = 0; k < 3; ++k) a.d_p[k][d] = a.s_p[k][i];
+                a.d_tau[d] = a.s_tau[i];
+            }
+            slot += __popc(bal);
+        }
+    }
+}
+
+// ---- energy spectrum (R23) --------------------------------------------------------------------------
+// bin = floor((ln E - ln e_min) * scale), scale = nbins/(ln e_max - ln e_min), in fp64; E = gamma - 1 =
+// p^2/(gamma + 1) for leptons, |p| for photons; p = 0 (dead) and out-of-range energies are skipped.
+// Shared-memory counters per CTA (nbins <= kSpectrumMaxBins), flushed with one atomic per non-empty bin.
+constexpr int kSpectrumMaxBins = 8192;
+
+template <typename R, int SPECIES>
+__global__ void __launch_bounds__(256) spectrum_kernel(const R* __restrict__ px, const R* __restrict__ py,
+                                                       const R* __restrict__ pz, long long n, double ln_min, double scale,
+                                                       int nbins, unsigned long long* __restrict__ hist) {
+    extern __shared__ unsigned int bins[];
+    for (int k = threadIdx.x; k < nbins; k += blockDim.x) bins[k] = 0u;
+    __syncthreads();
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const double x = px[i], y = py[i], z = pz[i];
+        const double p2 = __dadd_rn(__dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)), __dmul_rn(z, z));
+        if (!(p2 > 0.0)) continue;
+        const double en = SPECIES == 0 ? p2 / (__dsqrt_rn(1.0 + p2) + 1.0) : __dsqrt_rn(p2);
+        const double pos = (log(en) - ln_min) * scale;
+        if (pos >= 0.0 && pos < (double)nbins) atomicAdd(&bins[(int)floor(pos)], 1u);
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < nbins; k += blockDim.x)
+        if (bins[k]) atomicAdd(&hist[k], (unsigned long long)bins[k]);
+}
+
+template <typename R>
+__global__ void __launch_bounds__(256) fill_kernel(R* __restrict__ out, long long n, R value) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) out[i] = value;
+}
+
+}  // namespace pxq

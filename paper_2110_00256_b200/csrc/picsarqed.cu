@@ -13,6 +13,7 @@
 #include "evolve.cuh"
 #include "events.cuh"
 #include "tables.cuh"
+#include "cascade.cuh"
 
 using namespace pxq;
 
@@ -60,6 +61,14 @@ struct picsarqed_ctx {
     int host_slabs = 0;                      // 0 = automatic, k = split step_host into (at most) k slabs
     const unsigned long long* link_slot_base = nullptr;  // set by step_host around the qed_step of a slab
     long long link_parent_base = 0;
+    // closed loop (cascade_step): constant field arrays + secondary buffers, device counters and their pinned copy
+    void* cas = nullptr;
+    size_t cas_bytes = 0;
+    long long cas_field_n = 0;          // entries of the six field arrays that hold cas_field[]
+    double cas_field[6] = {0, 0, 0, 0, 0, 0};
+    int cas_field_dtype = -1;
+    unsigned long long* d_cas = nullptr;  // 16 counters
+    unsigned long long* h_cas = nullptr;
     double build_ms = 0.0;
 };
 
@@ -258,6 +267,8 @@ int picsarqed_create(picsarqed_ctx** out, int cuda_device, void* cuda_stream) {
     if (e == cudaSuccess) e = cudaMemset(c->ticket, 0, sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaMalloc(&c->d_counts, (kMaxSlabs + 2) * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_counts, (kMaxSlabs + 2) * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_cas, 16 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMallocHost(&c->h_cas, 16 * sizeof(unsigned long long));
     if (e != cudaSuccess) {
         delete c;
         return PICSARQED_ERR_CUDA;
@@ -284,6 +295,9 @@ int picsarqed_destroy(picsarqed_ctx* c) {
     for (cudaEvent_t e : c->timing_events) cudaEventDestroy(e);
     cudaFree(c->d_counts);
     cudaFreeHost(c->h_counts);
+    cudaFree(c->cas);
+    cudaFree(c->d_cas);
+    cudaFreeHost(c->h_cas);
     for (cudaEvent_t e : c->slab_events) cudaEventDestroy(e);
     if (c->h2d_stream) cudaStreamDestroy(c->h2d_stream);
     if (c->d2h_stream) cudaStreamDestroy(c->d2h_stream);
@@ -570,6 +584,44 @@ int launch_step(picsarqed_ctx* c, long long n, void* const* p, const void* const
         else if ((dtype) == PICSARQED_F32 && (tau_dtype) == PICSARQED_F64) { typedef float R; typedef double TR; CALL; } \
         else return fail(ctx, PICSARQED_ERR_DTYPE, "unsupported (dtype, tau_dtype) combination");                \
     } while (0)
+
+// ordered, filtering append: per-chunk keep counts -> tile offsets -> scatter (cascade.cuh).  d_dst_n (device) overrides
+// dst_n when not NULL: the second append of a step starts where the first one ended.
+template <typename R, typename TR>
+int launch_append(picsarqed_ctx* c, long long m_max, const void* const* s_p, const void* s_tau,
+                  const unsigned long long* d_count, double min_energy, void* const* d_p, void* d_tau, long long dst_n,
+                  const unsigned long long* d_dst_n, long long dst_capacity, unsigned long long* d_kept,
+                  unsigned long long* d_new_n) {
+    ChunkScratch cs;
+    if (int rc = chunk_scratch<R>(c, m_max, &cs)) return rc;
+    const int grid = (int)std::max<long long>(1, std::min<long long>((cs.n_chunks + 7) / 8, (long long)c->num_sms * 8));
+    keep_count_kernel<R><<<grid, 256, 0, c->stream>>>((const R*)s_p[0], (const R*)s_p[1], (const R*)s_p[2], d_count, m_max,
+                                                       min_energy, cs.n_chunks, cs.cnt);
+    const long long n_tiles = (cs.n_chunks + kAppendChunksPerTile - 1) / kAppendChunksPerTile;
+    tile_scan_kernel<<<1, kScanThreads, 0, c->stream>>>(cs.cnt, cs.n_chunks, kAppendChunksPerTile, n_tiles, cs.off, nullptr,
+                                                        d_kept);
+    AppendArgs<R, TR> a;
+    for (int k = 0; k < 3; ++k) {
+        a.s_p[k] = (const R*)s_p[k];
+        a.d_p[k] = (R*)d_p[k];
+    }
+    a.s_tau = (const TR*)s_tau;
+    a.d_tau = (TR*)d_tau;
+    a.d_count = d_count;
+    a.m_max = m_max;
+    a.dst_n = dst_n;
+    a.d_dst_n = d_dst_n;
+    a.dst_capacity = dst_capacity;
+    a.n_chunks = cs.n_chunks;
+    a.min_energy = min_energy;
+    a.cnt = cs.cnt;
+    a.tile_offset = cs.off;
+    a.d_kept = d_kept;
+    a.d_new_n = d_new_n;
+    append_kernel<R, TR><<<grid, 256, 0, c->stream>>>(a);
+    PXQ_CUDA(c, cudaGetLastError());
+    return PICSARQED_OK;
+}
 
 int check_arrays(picsarqed_ctx* c, const void* const* a, int count) {
     for (int k = 0; k < count; ++k)
@@ -909,5 +961,208 @@ extern "C" int picsarqed_build_tables(picsarqed_ctx* c, const picsarqed_table_pa
     if (int rc = build_guides(c)) return rc;
     PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
     c->have_tables = true;
+    return PICSARQED_OK;
+}
+
+// =====================================================================================
+//  closed loop in a uniform field (cascade.cuh)
+// =====================================================================================
+extern "C" int picsarqed_boris_push_uniform(picsarqed_ctx* c, int dtype, long long n, void* px, void* py, void* pz,
+                                            int charge_sign, const double* e, const double* b, double dt) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (n < 0 || (charge_sign != 1 && charge_sign != -1) || !e || !b)
+        return fail(c, PICSARQED_ERR_INVALID, "bad n, charge_sign, e or b");
+    if (dtype != PICSARQED_F64 && dtype != PICSARQED_F32) return fail(c, PICSARQED_ERR_DTYPE, "bad dtype");
+    if (n == 0) return PICSARQED_OK;
+    const void* a[3] = {px, py, pz};
+    if (int rc = check_arrays(c, a, 3)) return rc;
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    BorisArgs args;
+    const double k = charge_sign * dt * kInvTauC * 0.5;
+    for (int j = 0; j < 3; ++j) {
+        args.ke[j] = k * e[j];
+        args.kb[j] = k * b[j];
+    }
+    if (dtype == PICSARQED_F64)
+        boris_kernel<double><<<stream_grid(c, (n + 1) / 2, 256), 256, 0, c->stream>>>((double*)px, (double*)py, (double*)pz, n, args);
+    else
+        boris_kernel<float><<<stream_grid(c, (n + 3) / 4, 256), 256, 0, c->stream>>>((float*)px, (float*)py, (float*)pz, n, args);
+    PXQ_CUDA(c, cudaGetLastError());
+    return PICSARQED_OK;
+}
+
+extern "C" int picsarqed_append_secondaries(picsarqed_ctx* c, int dtype, int tau_dtype, long long m_max, const void* s_px,
+                                            const void* s_py, const void* s_pz, const void* s_tau,
+                                            const unsigned long long* d_count, double min_energy, void* d_px, void* d_py,
+                                            void* d_pz, void* d_tau, long long dst_n, long long dst_capacity,
+                                            unsigned long long* d_new_n) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (m_max < 0 || dst_n < 0 || dst_capacity < dst_n || !d_count || !d_new_n || !(min_energy >= 0.0))
+        return fail(c, PICSARQED_ERR_INVALID, "bad m_max, dst_n, dst_capacity, min_energy, d_count or d_new_n");
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    if (m_max == 0) {
+        const unsigned long long v = (unsigned long long)dst_n;
+        PXQ_CUDA(c, cudaMemcpyAsync(d_new_n, &v, sizeof(v), cudaMemcpyHostToDevice, c->stream));
+        PXQ_CUDA(c, cudaStreamSynchronize(c->stream));  // (v lives on this stack frame)
+        return PICSARQED_OK;
+    }
+    const void* chk[8] = {s_px, s_py, s_pz, s_tau, d_px, d_py, d_pz, d_tau};
+    if (int rc = check_arrays(c, chk, 8)) return rc;
+    const void* s_p[3] = {s_px, s_py, s_pz};
+    void* d_p[3] = {d_px, d_py, d_pz};
+    PXQ_DISPATCH_RT(c, dtype, tau_dtype,
+                    return (launch_append<R, TR>(c, m_max, s_p, s_tau, d_count, min_energy, d_p, d_tau, dst_n, nullptr,
+                                                 dst_capacity, c->d_cas + 15, d_new_n)));
+}
+
+extern "C" int picsarqed_energy_spectrum(picsarqed_ctx* c, int species, int dtype, long long n, const void* px,
+                                         const void* py, const void* pz, double e_min, double e_max, int nbins,
+                                         unsigned long long* hist) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (n < 0 || (species != 0 && species != 1) || !(e_min > 0.0) || !(e_max > e_min) || nbins < 1 ||
+        nbins > kSpectrumMaxBins || !hist)
+        return fail(c, PICSARQED_ERR_INVALID, "bad n, species, energy range, nbins or hist");
+    if (dtype != PICSARQED_F64 && dtype != PICSARQED_F32) return fail(c, PICSARQED_ERR_DTYPE, "bad dtype");
+    if (n == 0) return PICSARQED_OK;
+    const void* a[3] = {px, py, pz};
+    if (int rc = check_arrays(c, a, 3)) return rc;
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    const double ln_min = std::log(e_min), scale = nbins / (std::log(e_max) - std::log(e_min));
+    const int grid = (int)std::max<long long>(1, std::min<long long>((n + 255) / 256, (long long)c->num_sms * 4));
+    const size_t smem = (size_t)nbins * sizeof(unsigned int);
+#define PXQ_SPECTRUM(R, S)                                                                                     \
+    spectrum_kernel<R, S><<<grid, 256, smem, c->stream>>>((const R*)px, (const R*)py, (const R*)pz, n, ln_min, \
+                                                          scale, nbins, hist)
+    if (dtype == PICSARQED_F64) {
+        if (species == 0) PXQ_SPECTRUM(double, 0); else PXQ_SPECTRUM(double, 1);
+    } else {
+        if (species == 0) PXQ_SPECTRUM(float, 0); else PXQ_SPECTRUM(float, 1);
+    }
+#undef PXQ_SPECTRUM
+    PXQ_CUDA(c, cudaGetLastError());
+    return PICSARQED_OK;
+}
+
+extern "C" int picsarqed_cascade_step(picsarqed_ctx* c, int dtype, int tau_dtype, picsarqed_species_arrays* el,
+                                      picsarqed_species_arrays* po, picsarqed_species_arrays* ph, const double* e,
+                                      const double* b, double dt, unsigned long long seed, unsigned long long step,
+                                      double photon_min_energy, int push, unsigned long long* h_events) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (!el || !po || !ph || !e || !b || !(photon_min_energy >= 0.0))
+        return fail(c, PICSARQED_ERR_INVALID, "null species, e or b, or bad photon_min_energy");
+    if ((dtype != 0 && dtype != 1) || (tau_dtype != 0 && tau_dtype != 1) || (dtype == 1 && tau_dtype == 0))
+        return fail(c, PICSARQED_ERR_DTYPE, "unsupported (dtype, tau_dtype) combination");
+    picsarqed_species_arrays* sp[3] = {el, po, ph};
+    for (int k = 0; k < 3; ++k)
+        if (sp[k]->n < 0 || sp[k]->capacity < sp[k]->n) return fail(c, PICSARQED_ERR_INVALID, "species: bad n or capacity");
+    if (!c->have_tables) return fail(c, PICSARQED_ERR_NO_TABLES, "no tables: call build_tables or import_tables");
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    const size_t es = dtype ? 8 : 4, ts = tau_dtype ? 8 : 4;
+    auto pad = [](size_t x) { return (x + 255) & ~(size_t)255; };
+    const long long n_e = el->n, n_p = po->n, n_g = ph->n;
+    const long long n_max = std::max(n_e, std::max(n_p, n_g));
+    // scratch: six constant field arrays of n_field entries; secondary buffers (photons of the electrons, photons of
+    // the positrons, electrons and positrons of the photons), 3 momenta + tau each
+    auto need_for = [&](long long nf, long long ne, long long np, long long ng) {
+        return 6 * pad((size_t)nf * es) + (3 * pad((size_t)ne * es) + pad((size_t)ne * ts)) +
+               (3 * pad((size_t)np * es) + pad((size_t)np * ts)) + 2 * (3 * pad((size_t)ng * es) + pad((size_t)ng * ts));
+    };
+    long long n_field = std::max<long long>(c->cas_field_n, n_max);
+    if (need_for(n_field, n_e, n_p, n_g) > c->cas_bytes) {  // grow with headroom: populations rise step after step
+        n_field = n_max + n_max / 2 + 1024;
+        const size_t want = need_for(n_field, n_e + n_e / 2 + 1024, n_p + n_p / 2 + 1024, n_g + n_g / 2 + 1024);
+        PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+        if (c->cas) cudaFree(c->cas);
+        c->cas = nullptr;
+        c->cas_bytes = 0;
+        c->cas_field_n = 0;
+        PXQ_CUDA(c, cudaMalloc(&c->cas, want));
+        c->cas_bytes = want;
+    }
+    char* base = static_cast<char*>(c->cas);
+    void* f[6];
+    for (int k = 0; k < 6; ++k) f[k] = base + k * pad((size_t)n_field * es);
+    char* q = base + 6 * pad((size_t)n_field * es);
+    auto carve = [&](long long m, void** p4) {  // 3 momenta + tau of m entries
+        for (int k = 0; k < 3; ++k) { p4[k] = q; q += pad((size_t)m * es); }
+        p4[3] = q;
+        q += pad((size_t)m * ts);
+    };
+    void *ph_e[4], *ph_p[4], *pair_e[4], *pair_p[4];
+    carve(n_e, ph_e);
+    carve(n_p, ph_p);
+    carve(n_g, pair_e);
+    carve(n_g, pair_p);
+    const double fv[6] = {e[0], e[1], e[2], b[0], b[1], b[2]};
+    bool same = c->cas_field_dtype == dtype && c->cas_field_n >= n_field;
+    for (int k = 0; k < 6; ++k) same = same && c->cas_field[k] == fv[k];
+    if (!same && n_field > 0) {
+        for (int k = 0; k < 6; ++k) {
+            const int grid = stream_grid(c, n_field, 256);
+            if (dtype) fill_kernel<double><<<grid, 256, 0, c->stream>>>((double*)f[k], n_field, fv[k]);
+            else fill_kernel<float><<<grid, 256, 0, c->stream>>>((float*)f[k], n_field, (float)fv[k]);
+            c->cas_field[k] = fv[k];
+        }
+        PXQ_CUDA(c, cudaGetLastError());
+        c->cas_field_n = n_field;
+        c->cas_field_dtype = dtype;
+    }
+    // d_cas: [0..2] events of electrons, positrons, photons; [3] photons before the appends, [4] after the first,
+    // [5] after the second; [6] electrons, [7] positrons after the pairs; [15] scratch (kept count of an append)
+    PXQ_CUDA(c, cudaMemsetAsync(c->d_cas, 0, 16 * sizeof(unsigned long long), c->stream));
+    if (push) {
+        if (int rc = picsarqed_boris_push_uniform(c, dtype, n_e, el->px, el->py, el->pz, -1, e, b, dt)) return rc;
+        if (int rc = picsarqed_boris_push_uniform(c, dtype, n_p, po->px, po->py, po->pz, +1, e, b, dt)) return rc;
+    }
+    if (n_e > 0)
+        if (int rc = picsarqed_qed_step(c, 0, dtype, tau_dtype, n_e, el->px, el->py, el->pz, f[0], f[1], f[2], f[3], f[4], f[5],
+                                        el->tau, dt, seed, step, el->id_base, n_e, ph_e[0], ph_e[1], ph_e[2], ph_e[3],
+                                        nullptr, nullptr, nullptr, nullptr, nullptr, c->d_cas + 0))
+            return rc;
+    if (n_p > 0)
+        if (int rc = picsarqed_qed_step(c, 0, dtype, tau_dtype, n_p, po->px, po->py, po->pz, f[0], f[1], f[2], f[3], f[4], f[5],
+                                        po->tau, dt, seed, step, po->id_base, n_p, ph_p[0], ph_p[1], ph_p[2], ph_p[3],
+                                        nullptr, nullptr, nullptr, nullptr, nullptr, c->d_cas + 1))
+            return rc;
+    if (n_g > 0)
+        if (int rc = picsarqed_qed_step(c, 1, dtype, tau_dtype, n_g, ph->px, ph->py, ph->pz, f[0], f[1], f[2], f[3], f[4], f[5],
+                                        ph->tau, dt, seed, step, ph->id_base, n_g, pair_e[0], pair_e[1], pair_e[2],
+                                        pair_e[3], pair_p[0], pair_p[1], pair_p[2], pair_p[3], nullptr, c->d_cas + 2))
+            return rc;
+    // feed back (R20): photons of the electrons, then of the positrons; then the pairs
+    c->h_cas[0] = (unsigned long long)n_g;  // (pinned; not read back before the synchronize below)
+    for (int k = 3; k <= 5; ++k)
+        PXQ_CUDA(c, cudaMemcpyAsync(c->d_cas + k, c->h_cas, 8, cudaMemcpyHostToDevice, c->stream));
+    void* ph_dst[3] = {ph->px, ph->py, ph->pz};
+    void* el_dst[3] = {el->px, el->py, el->pz};
+    void* po_dst[3] = {po->px, po->py, po->pz};
+    // (an append never reads and writes the same counter: every block reads its start while block 0 writes the end)
+#define PXQ_APPEND(SRC, M, CNT, THR, DST, DTAU, DSTN, DSTN_PTR, CAP, OUT)                                              \
+    do {                                                                                                               \
+        if ((M) > 0) {                                                                                                 \
+            PXQ_DISPATCH_RT(c, dtype, tau_dtype, {                                                                     \
+                if (int rc = launch_append<R, TR>(c, (M), SRC, SRC[3], (CNT), (THR), DST, DTAU, (DSTN), (DSTN_PTR),    \
+                                                  (CAP), c->d_cas + 15, (OUT)))                                        \
+                    return rc;                                                                                         \
+            });                                                                                                        \
+        }                                                                                                              \
+    } while (0)
+    PXQ_APPEND(ph_e, n_e, c->d_cas + 0, photon_min_energy, ph_dst, ph->tau, 0, c->d_cas + 3, ph->capacity, c->d_cas + 4);
+    PXQ_APPEND(ph_p, n_p, c->d_cas + 1, photon_min_energy, ph_dst, ph->tau, 0, c->d_cas + 4, ph->capacity, c->d_cas + 5);
+    PXQ_APPEND(pair_e, n_g, c->d_cas + 2, 0.0, el_dst, el->tau, n_e, nullptr, el->capacity, c->d_cas + 6);
+    PXQ_APPEND(pair_p, n_g, c->d_cas + 2, 0.0, po_dst, po->tau, n_p, nullptr, po->capacity, c->d_cas + 7);
+#undef PXQ_APPEND
+    PXQ_CUDA(c, cudaMemcpyAsync(c->h_cas, c->d_cas, 8 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+    PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (h_events)
+        for (int k = 0; k < 3; ++k) h_events[k] = c->h_cas[k];
+    const long long new_n[3] = {n_g > 0 ? (long long)c->h_cas[6] : n_e, n_g > 0 ? (long long)c->h_cas[7] : n_p,
+                                (long long)(n_p > 0 ? c->h_cas[5] : c->h_cas[4])};
+    bool overflow = false;
+    for (int k = 0; k < 3; ++k) {
+        overflow = overflow || new_n[k] > sp[k]->capacity;
+        sp[k]->n = std::min(new_n[k], sp[k]->capacity);
+    }
+    if (overflow) return fail(c, PICSARQED_ERR_INVALID, "cascade_step: a species exceeded its capacity");
     return PICSARQED_OK;
 }
