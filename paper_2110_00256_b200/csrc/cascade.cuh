@@ -82,6 +82,7 @@ __global__ void __launch_bounds__(256) keep_count_kernel(const R* __restrict__ p
                                                          unsigned short* __restrict__ cnt) {
     const int lane = threadIdx.x & 31;
     const long long m = (long long)min((unsigned long long)m_max, *d_count);
+    n_chunks = min(n_chunks, (m + kChunk - 1) / kChunk);   // only the chunks that hold entries (the scan does the same)
     const long long warps = (long long)gridDim.x * (blockDim.x / 32);
     for (long long ch = (long long)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); ch < n_chunks; ch += warps) {
         unsigned int k = 0;
@@ -123,7 +124,8 @@ __global__ void __launch_bounds__(256) append_kernel(const AppendArgs<R, TR> a) 
     const long long dst_n = a.d_dst_n ? (long long)*a.d_dst_n : a.dst_n;
     if (blockIdx.x == 0 && threadIdx.x == 0) *a.d_new_n = (unsigned long long)dst_n + *a.d_kept;
     const long long warps = (long long)gridDim.x * (blockDim.x / 32);
-    for (long long ch = (long long)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); ch < a.n_chunks; ch += warps) {
+    const long long n_chunks = min(a.n_chunks, (m + kChunk - 1) / kChunk);
+    for (long long ch = (long long)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); ch < n_chunks; ch += warps) {
         const long long tile = ch / kAppendChunksPerTile;
         const int in_tile = (int)(ch - tile * kAppendChunksPerTile);
         const unsigned int c = lane < in_tile ? a.cnt[tile * kAppendChunksPerTile + lane] : 0u;   // chunks before this one
@@ -150,6 +152,16 @@ __global__ void __launch_bounds__(256) append_kernel(const AppendArgs<R, TR> a) 
 // Shared-memory counters per CTA (nbins <= kSpectrumMaxBins), flushed with one atomic per non-empty bin.
 constexpr int kSpectrumMaxBins = 8192;
 
+template <int SPECIES>
+__device__ __forceinline__ void spectrum_one(double x, double y, double z, double ln_min, double scale, int nbins,
+                                             unsigned int* bins) {
+    const double p2 = __dadd_rn(__dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)), __dmul_rn(z, z));
+    if (!(p2 > 0.0)) return;
+    const double en = SPECIES == 0 ? p2 / (__dsqrt_rn(1.0 + p2) + 1.0) : __dsqrt_rn(p2);
+    const double pos = (log(en) - ln_min) * scale;
+    if (pos >= 0.0 && pos < (double)nbins) atomicAdd(&bins[(int)floor(pos)], 1u);
+}
+
 template <typename R, int SPECIES>
 __global__ void __launch_bounds__(256) spectrum_kernel(const R* __restrict__ px, const R* __restrict__ py,
                                                        const R* __restrict__ pz, long long n, double ln_min, double scale,
@@ -157,15 +169,30 @@ __global__ void __launch_bounds__(256) spectrum_kernel(const R* __restrict__ px,
     extern __shared__ unsigned int bins[];
     for (int k = threadIdx.x; k < nbins; k += blockDim.x) bins[k] = 0u;
     __syncthreads();
+    constexpr int V = 16 / sizeof(R);
+    const long long nvec = n / V;
     const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        const double x = px[i], y = py[i], z = pz[i];
-        const double p2 = __dadd_rn(__dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)), __dmul_rn(z, z));
-        if (!(p2 > 0.0)) continue;
-        const double en = SPECIES == 0 ? p2 / (__dsqrt_rn(1.0 + p2) + 1.0) : __dsqrt_rn(p2);
-        const double pos = (log(en) - ln_min) * scale;
-        if (pos >= 0.0 && pos < (double)nbins) atomicAdd(&bins[(int)floor(pos)], 1u);
+    const unsigned long long pol = l2_policy_evict_first();
+    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < nvec; j += 2 * stride) {
+        // two 128-bit loads per array per thread in flight
+        const long long j2 = j + stride;
+        Vec<R, V> x0 = ld_stream<R, V>(px + j * V, pol), y0 = ld_stream<R, V>(py + j * V, pol),
+                  z0 = ld_stream<R, V>(pz + j * V, pol);
+        Vec<R, V> x1 = x0, y1 = y0, z1 = z0;
+        if (j2 < nvec) {
+            x1 = ld_stream<R, V>(px + j2 * V, pol);
+            y1 = ld_stream<R, V>(py + j2 * V, pol);
+            z1 = ld_stream<R, V>(pz + j2 * V, pol);
+        }
+#pragma unroll
+        for (int v = 0; v < V; ++v) spectrum_one<SPECIES>(x0.v[v], y0.v[v], z0.v[v], ln_min, scale, nbins, bins);
+        if (j2 < nvec) {
+#pragma unroll
+            for (int v = 0; v < V; ++v) spectrum_one<SPECIES>(x1.v[v], y1.v[v], z1.v[v], ln_min, scale, nbins, bins);
+        }
     }
+    for (long long i = nvec * V + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+        spectrum_one<SPECIES>(px[i], py[i], pz[i], ln_min, scale, nbins, bins);
     __syncthreads();
     for (int k = threadIdx.x; k < nbins; k += blockDim.x)
         if (bins[k]) atomicAdd(&hist[k], (unsigned long long)bins[k]);

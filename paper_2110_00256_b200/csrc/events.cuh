@@ -164,7 +164,8 @@ __global__ void __launch_bounds__(256) count_chunks_kernel(const TR* __restrict_
 // is a multiple of 8 chunks) and scans the tile sums, 4096 tiles per round (four consecutive tiles per thread),
 // carrying the running total; tile_offset[t] = number of events before tile t, *d_total = *d_base (0 when
 // d_base is NULL) + their number.  d_base chains the slabs of step_host: the events of a slab follow those of
-// the slabs before it in the secondary buffers.
+// the slabs before it in the secondary buffers.  d_entries (not NULL: the append of cascade.cuh) = device count of
+// the entries that exist: only the chunks that hold them are read.
 constexpr int kScanThreads = 1024;
 constexpr int kScanItems = 4;
 
@@ -172,8 +173,14 @@ __global__ void __launch_bounds__(kScanThreads) tile_scan_kernel(const unsigned 
                                                                  int chunks_per_tile, long long n_tiles,
                                                                  unsigned long long* __restrict__ tile_offset,
                                                                  const unsigned long long* d_base,
-                                                                 unsigned long long* d_total) {
+                                                                 unsigned long long* d_total,
+                                                                 const unsigned long long* d_entries) {
     __shared__ unsigned long long warp_sum[2][kScanThreads / 32];
+    if (d_entries) {
+        const unsigned long long live = (*d_entries + kChunk - 1) / kChunk;
+        if (live < (unsigned long long)n_chunks) n_chunks = (long long)live;
+        n_tiles = (n_chunks + chunks_per_tile - 1) / chunks_per_tile;
+    }
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     unsigned long long carry = 0;  // (the same value in every thread)
     int round = 0;

@@ -81,6 +81,14 @@ __device__ __forceinline__ void stage_table_tma(void* smem_dst, const void* gmem
 }
 
 // ---- one particle ----------------------------------------------------------------------
+// a_k(1/3) of the Hankel expansion of K_{1/3} (DLMF 10.40.2, 10.17.1): a_k = prod_{j=1..k} (4 nu^2 - (2j-1)^2)/(8 j);
+// evaluated by the compiler (the callers pass literals)
+__host__ __device__ constexpr double hankel13(int k) {
+    double a = 1.0;
+    for (int j = 1; j <= k; ++j) a *= (4.0 / 9.0 - (2.0 * j - 1.0) * (2.0 * j - 1.0)) / (8.0 * j);
+    return a;
+}
+
 // Returns the decrement dN/dt * dt in the particle arithmetic type A (float or double).
 template <typename R, int SPECIES>
 __device__ __forceinline__ auto decrement_one(R pxr, R pyr, R pzr, R exr, R eyr, R ezr, R bxr, R byr, R bzr,
@@ -130,6 +138,17 @@ __device__ __forceinline__ auto decrement_one(R pxr, R pyr, R pzr, R exr, R eyr,
                 const double h2 = cbrt(y);
                 const double k = sm - sp * h2;  // K h sqrt3/pi
                 k2 = (1.5707963267948966 / 0.8660254037844386) * (1.5707963267948966 / 0.8660254037844386) * k * k / h2;
+            } else if (c2 < 2.8444e-3) {      // x > 25: the window just below a T table that starts at chi ~ 1e-2
+                // Hankel expansion (DLMF 10.40.2): K^2 = (pi/2x) e^{-2x} (sum_k a_k x^-k)^2, sixteen terms in
+                // Horner form with constant coefficients (the first term left out is < 1e-16 at x = 25); 1/x =
+                // (3/4) chi comes from one rsqrt: no division, no logarithm
+                const double rs = rsqrt_fast(c2);
+                const double x = (4.0 / 3.0) * rs, r = 0.75 * (c2 * rs);
+                double sum = hankel13(16);
+#pragma unroll
+                for (int k = 15; k >= 1; --k) sum = fma(sum, r, hankel13(k));
+                sum = fma(sum, r, 1.0);
+                k2 = 1.5707963267948966 * r * sum * sum * exp_fast(-2.0 * x);
             } else {
                 const double x = 4.0 / (3.0 * sqrt(c2));
                 k2 = exp(2.0 * (ln_bessel_k13_scaled(x) - x));

@@ -461,13 +461,15 @@ int chunk_scratch(picsarqed_ctx* c, long long n, ChunkScratch* out) {
     const size_t cnt_sz = ((size_t)nchunks * sizeof(unsigned short) + 255) & ~(size_t)255;
     // tiles hold at least 8 chunks: n_chunks/8 + 1 tile offsets are always enough
     const size_t off_sz = ((size_t)(nchunks / 8 + 2) * sizeof(unsigned long long) + 255) & ~(size_t)255;
-    if (rec_sz + cnt_sz + off_sz > c->rec_bytes) {  // grow (rare; synchronises)
-        PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (rec_sz + cnt_sz + off_sz > c->rec_bytes) {  // grow (synchronises): half as much again when a population
+        PXQ_CUDA(c, cudaStreamSynchronize(c->stream));  // creeps up step after step (closed loop), exact otherwise
+        const size_t need = rec_sz + cnt_sz + off_sz;
+        const size_t want = c->rec_bytes > 0 && need < c->rec_bytes + c->rec_bytes / 2 ? c->rec_bytes + c->rec_bytes / 2 : need;
         if (c->rec) cudaFree(c->rec);
         c->rec = nullptr;
         c->rec_bytes = 0;
-        PXQ_CUDA(c, cudaMalloc(&c->rec, rec_sz + cnt_sz + off_sz));
-        c->rec_bytes = rec_sz + cnt_sz + off_sz;
+        PXQ_CUDA(c, cudaMalloc(&c->rec, want));
+        c->rec_bytes = want;
     }
     out->rec = static_cast<unsigned char*>(c->rec);
     out->cnt = reinterpret_cast<unsigned short*>(out->rec + rec_sz);
@@ -506,7 +508,8 @@ int launch_event_pass(picsarqed_ctx* c, long long n, const ChunkScratch& cs, voi
     static const int kChunksOf[8] = {24, 32, 24, 16, 12, 24, 24, 32};  // must match the switch below
     const int chunks = kChunksOf[c->event_config];
     const long long n_tiles = (cs.n_chunks + chunks - 1) / chunks;
-    tile_scan_kernel<<<1, kScanThreads, 0, c->stream>>>(cs.cnt, cs.n_chunks, chunks, n_tiles, cs.off, c->link_slot_base, d_n_out);
+    tile_scan_kernel<<<1, kScanThreads, 0, c->stream>>>(cs.cnt, cs.n_chunks, chunks, n_tiles, cs.off, c->link_slot_base, d_n_out,
+                                                        nullptr);
 #define PXQ_LAUNCH_EVENTS(T, CH, MB)                                                                         \
     do {                                                                                                     \
         auto kern = event_kernel<R, TR, KIND, T, CH, MB>;                                                    \
@@ -599,7 +602,7 @@ int launch_append(picsarqed_ctx* c, long long m_max, const void* const* s_p, con
                                                        min_energy, cs.n_chunks, cs.cnt);
     const long long n_tiles = (cs.n_chunks + kAppendChunksPerTile - 1) / kAppendChunksPerTile;
     tile_scan_kernel<<<1, kScanThreads, 0, c->stream>>>(cs.cnt, cs.n_chunks, kAppendChunksPerTile, n_tiles, cs.off, nullptr,
-                                                        d_kept);
+                                                        d_kept, d_count);
     AppendArgs<R, TR> a;
     for (int k = 0; k < 3; ++k) {
         a.s_p[k] = (const R*)s_p[k];
@@ -1028,7 +1031,7 @@ extern "C" int picsarqed_energy_spectrum(picsarqed_ctx* c, int species, int dtyp
     if (int rc = check_arrays(c, a, 3)) return rc;
     PXQ_CUDA(c, cudaSetDevice(c->device));
     const double ln_min = std::log(e_min), scale = nbins / (std::log(e_max) - std::log(e_min));
-    const int grid = (int)std::max<long long>(1, std::min<long long>((n + 255) / 256, (long long)c->num_sms * 4));
+    const int grid = (int)std::max<long long>(1, std::min<long long>((n + 1023) / 1024, (long long)c->num_sms * 8));
     const size_t smem = (size_t)nbins * sizeof(unsigned int);
 #define PXQ_SPECTRUM(R, S)                                                                                     \
     spectrum_kernel<R, S><<<grid, 256, smem, c->stream>>>((const R*)px, (const R*)py, (const R*)pz, n, ln_min, \
