@@ -44,6 +44,10 @@ def parse():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-sample", type=int, default=1 << 23, help="particles in the oracle timing sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cascade", action="store_true",
+                    help="secondary workload (SURVEY.md 8(f)-1): closed loop of Ridgers case (iii) instead of the "
+                         "headline step; prints its own JSON line")
+    ap.add_argument("--cascade-dtype", default="f64", choices=["f64", "f32"])
     return ap.parse_args()
 
 
@@ -321,10 +325,52 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_cascade(args):
+    """closed loop in a uniform field (Ridgers case (iii): gamma_0 = 1000, B_0 = 9e-3 E_s/c, 0.1 fs in
+    `steps` steps, photons below 2 m_e c^2 dropped at creation): push + QED step of the three species + feedback per
+    step, populations growing from `particles`/2 electrons to ~4.4x as many particles.  Not the headline metric."""
+    import torch
+
+    import paper_2110_00256_b200 as q
+    torch.cuda.set_device(0)
+    ctx = q.Context(0)
+    ctx.build_tables(q.TableParams())          # the paper's benchmark tables (PAPER.md:301), 256 / 256x256
+    dt_ = torch.float64 if args.cascade_dtype == "f64" else torch.float32
+    n0 = args.particles // 2
+    steps = max(args.steps, 1)
+
+    def run():
+        pops = {k: q.Species(6 * n0, dt_, dt_, ib)
+                for k, ib in (("electrons", 0), ("positrons", 1 << 40), ("photons", 1 << 41))}
+        pops["electrons"].p[0][:n0] = float(np.sqrt(1000.0 ** 2 - 1))
+        pops["electrons"].n = n0
+        ctx.init_optical_depth(q.LEPTON, pops["electrons"].tau[:n0], SEED, 0)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        work = 0
+        for s in range(steps):
+            work += sum(p.n for p in pops.values())
+            ctx.cascade_step(pops, (0.0, 0.0, 0.0), (0.0, 0.0, 9e-3), 1e-16 / steps, SEED, s, photon_min_energy=2.0)
+        torch.cuda.synchronize()
+        return work, time.perf_counter() - t0, {k: p.n for k, p in pops.items()}
+
+    for _ in range(max(1, min(args.warmup, 2))):
+        run()                                  # scratch buffers reach their final size
+    work, sec, final = run()
+    print(json.dumps({"metric": "closed loop (Ridgers case iii) particle-steps/s", "value": work / sec,
+                      "unit": "particle-steps/s", "n_gpus": 1, "steps": steps, "warmup": args.warmup,
+                      "ms_per_step": 1e3 * sec / steps, "higher_is_better": True, "dtype": args.cascade_dtype,
+                      "data": "synthetic",
+                      "config": {"workload": "closed loop, uniform B = 9e-3 E_s/c, gamma_0 = 1000, 0.1 fs, photon "
+                                             "threshold 2 m_e c^2", "initial_electrons": n0, "final": final}}), flush=True)
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         run_reference(args)
+    elif args.cascade:
+        run_cascade(args)
     else:
         run_ours(args)
 
