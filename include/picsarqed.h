@@ -284,6 +284,22 @@ int picsarqed_cascade_step(picsarqed_ctx* ctx, int dtype, int tau_dtype,
                            unsigned long long seed, unsigned long long step, double photon_min_energy,
                            int push, unsigned long long* h_events);
 
+/* ---- the table functions per value (Figs.2-5) ---------------------
+ * What the hot path evaluates, exposed for single values so that table accuracy can be studied
+ * (error against table size) and so that a caller can sample
+ * outside a particle loop.  chi, r, out: device arrays of n reals of type `dtype`.
+ *
+ * table_function: kind 0: out[i] = G(chi[i]) by eq.27 (first/last value outside the table);
+ * kind 1: out[i] = T(chi[i]) by eq.23 inside the table, the Erber form outside.
+ * The kernel runs the evolve pass's own routine on a synthetic particle of that chi. */
+int picsarqed_table_function(picsarqed_ctx* ctx, int kind, int dtype, long long n, const void* chi, void* out);
+
+/* sample_xi: kind 0: xi = chi_gamma/chi of the emitted photon by eqs.28-30 from r[i] in (0,1);
+ * kind 1: xi = chi_-/chi_gamma of the electron of the pair by eqs.24-26, with the reflection
+ * r -> 1 - r, xi -> 1 - xi for r > 1/2.  The routines are those of the event pass. */
+int picsarqed_sample_xi(picsarqed_ctx* ctx, int kind, int dtype, long long n, const void* chi, const void* r,
+                        void* xi_out);
+
 #ifdef __cplusplus
 }
 #endif

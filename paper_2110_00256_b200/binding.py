@@ -74,6 +74,8 @@ _SIGNATURES = {
     "picsarqed_boris_push_uniform": (_i, [_vp, _i, _i64, _vp, _vp, _vp, _i, C.POINTER(_d), C.POINTER(_d), _d]),
     "picsarqed_append_secondaries": (_i, [_vp, _i, _i, _i64] + [_vp] * 5 + [_d] + [_vp] * 4 + [_i64, _i64, _vp]),
     "picsarqed_energy_spectrum": (_i, [_vp, _i, _i, _i64, _vp, _vp, _vp, _d, _d, _i, _vp]),
+    "picsarqed_table_function": (_i, [_vp, _i, _i, _i64, _vp, _vp]),
+    "picsarqed_sample_xi": (_i, [_vp, _i, _i, _i64, _vp, _vp, _vp]),
     "picsarqed_cascade_step": (_i, [_vp, _i, _i, C.POINTER(_CSpecies), C.POINTER(_CSpecies), C.POINTER(_CSpecies),
                                     C.POINTER(_d), C.POINTER(_d), _d, _u64, _u64, _d, _i, C.POINTER(_u64)]),
 }
@@ -265,6 +267,16 @@ class Context:
             tau.data_ptr(), float(dt), seed, step, id_base, capacity, C.cast(sec_ptrs, _vp),
             parent.data_ptr() if parent is not None else None, C.byref(n_out)))
         return int(n_out.value)
+
+    # ---- table functions per value -----------------------------------------
+    def table_function(self, kind, chi, out):
+        """out = G(chi) (kind LEPTON) or T(chi) (kind PHOTON) as the evolve pass evaluates them"""
+        self._check(lib().picsarqed_table_function(self._h, kind, _code(chi.dtype), chi.numel(), _dev(chi),
+                                                   _dev(out, chi.dtype)))
+
+    def sample_xi(self, kind, chi, r, xi):
+        self._check(lib().picsarqed_sample_xi(self._h, kind, _code(chi.dtype), chi.numel(), _dev(chi),
+                                              _dev(r, chi.dtype), _dev(xi, chi.dtype)))
 
     # ---- closed loop in a uniform field (SURVEY.md 8(f)-1, 8(f)-2) ------------------------------
     def boris_push_uniform(self, p, charge_sign, e, b, dt):

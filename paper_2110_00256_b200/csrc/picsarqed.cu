@@ -14,6 +14,7 @@
 #include "events.cuh"
 #include "tables.cuh"
 #include "cascade.cuh"
+#include "lookup.cuh"
 
 using namespace pxq;
 
@@ -1167,5 +1168,52 @@ extern "C" int picsarqed_cascade_step(picsarqed_ctx* c, int dtype, int tau_dtype
         sp[k]->n = std::min(new_n[k], sp[k]->capacity);
     }
     if (overflow) return fail(c, PICSARQED_ERR_INVALID, "cascade_step: a species exceeded its capacity");
+    return PICSARQED_OK;
+}
+
+// =====================================================================================
+//  table functions per value (lookup.cuh)
+// =====================================================================================
+extern "C" int picsarqed_table_function(picsarqed_ctx* c, int kind, int dtype, long long n, const void* chi, void* out) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (n < 0 || (kind != 0 && kind != 1)) return fail(c, PICSARQED_ERR_INVALID, "bad n or kind");
+    if (dtype != PICSARQED_F64 && dtype != PICSARQED_F32) return fail(c, PICSARQED_ERR_DTYPE, "bad dtype");
+    if (!c->have_tables) return fail(c, PICSARQED_ERR_NO_TABLES, "no tables: call build_tables or import_tables");
+    if (n == 0) return PICSARQED_OK;
+    const void* a[2] = {chi, out};
+    if (int rc = check_arrays(c, a, 2)) return rc;
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    const int grid = stream_grid(c, n, 256);
+#define PXQ_TF(R, K) table_function_kernel<R, K><<<grid, 256, 0, c->stream>>>((const R*)chi, (R*)out, n, view_1d<R>(c, K))
+    if (dtype == PICSARQED_F64) {
+        if (kind == 0) PXQ_TF(double, 0); else PXQ_TF(double, 1);
+    } else {
+        if (kind == 0) PXQ_TF(float, 0); else PXQ_TF(float, 1);
+    }
+#undef PXQ_TF
+    PXQ_CUDA(c, cudaGetLastError());
+    return PICSARQED_OK;
+}
+
+extern "C" int picsarqed_sample_xi(picsarqed_ctx* c, int kind, int dtype, long long n, const void* chi, const void* r,
+                                   void* xi_out) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (n < 0 || (kind != 0 && kind != 1)) return fail(c, PICSARQED_ERR_INVALID, "bad n or kind");
+    if (dtype != PICSARQED_F64 && dtype != PICSARQED_F32) return fail(c, PICSARQED_ERR_DTYPE, "bad dtype");
+    if (!c->have_tables) return fail(c, PICSARQED_ERR_NO_TABLES, "no tables: call build_tables or import_tables");
+    if (n == 0) return PICSARQED_OK;
+    const void* a[3] = {chi, r, xi_out};
+    if (int rc = check_arrays(c, a, 3)) return rc;
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    const int grid = stream_grid(c, n, 256);
+#define PXQ_SX(R, K) \
+    sample_xi_kernel<R, K><<<grid, 256, 0, c->stream>>>((const R*)chi, (const R*)r, (R*)xi_out, n, view_2d<R>(c, K))
+    if (dtype == PICSARQED_F64) {
+        if (kind == 0) PXQ_SX(double, 0); else PXQ_SX(double, 1);
+    } else {
+        if (kind == 0) PXQ_SX(float, 0); else PXQ_SX(float, 1);
+    }
+#undef PXQ_SX
+    PXQ_CUDA(c, cudaGetLastError());
     return PICSARQED_OK;
 }
