@@ -305,11 +305,11 @@ def run_ours(args):
                      "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
                      "traffic": EVOLVE_DRAM_TRAFFIC_BYTES, "algorithmic_bytes_per_launch": evolve_bytes,
                      "ms_per_launch": ms_evolve, "share_of_step": ms_evolve * args.steps / ms_total,
-                     # the whole step against the same peak: 88 B per particle + ~150 B per event (48 B record written and
-                     # read back once = 96, 40 B photon + 8 B parent index, four 8-byte parent stores = 32: DESIGN.md 6)
-                     "whole_step": {"algorithmic_bytes": evolve_bytes + 150 * fired_last,
-                                    "achieved": (evolve_bytes + 150 * fired_last) / (ms_total / args.steps * 1e-3) / 1e9,
-                                    "frac": (evolve_bytes + 150 * fired_last) / (ms_total / args.steps * 1e-3) / 1e9
+                     # the whole step against the same peak: 88 B per particle + 168 B per event (48 B record written and
+                     # read back once = 96, 32 B photon + 8 B parent index, four 8-byte parent stores = 32: DESIGN.md 6)
+                     "whole_step": {"algorithmic_bytes": evolve_bytes + 168 * fired_last,
+                                    "achieved": (evolve_bytes + 168 * fired_last) / (ms_total / args.steps * 1e-3) / 1e9,
+                                    "frac": (evolve_bytes + 168 * fired_last) / (ms_total / args.steps * 1e-3) / 1e9
                                             / peaks["hbm_gbs"]}},
         "kernels_ms": {"qed_step": {"evolve_pass": ms_evolve, "event_pass": ms_events},
                        "two_call_path": {"evolve_optical_depth": ms_evolve2, "generate_photons": ms_events2}},
