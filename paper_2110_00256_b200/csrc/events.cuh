@@ -144,7 +144,8 @@ __device__ __forceinline__ void event_commit(const EventArgs<R, TR>& a, long lon
 // one warp per chunk: tau < 0 (R1) -> ballot/popc.  No records are staged on this path.
 template <typename TR>
 __global__ void __launch_bounds__(256) count_chunks_kernel(const TR* __restrict__ tau, long long n, long long first_chunk,
-                                                           long long n_chunks, unsigned short* __restrict__ cnt) {
+                                                           long long n_chunks, unsigned short* __restrict__ cnt,
+                                                           unsigned int* __restrict__ tile_sum, int chunks_per_tile) {
     const int lane = threadIdx.x & 31;
     const long long warps = (long long)gridDim.x * (blockDim.x / 32);
     for (long long ch = first_chunk + (long long)blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5); ch < n_chunks; ch += warps) {
@@ -155,7 +156,10 @@ __global__ void __launch_bounds__(256) count_chunks_kernel(const TR* __restrict_
             const bool f = i < n && tau[i] < (TR)0;
             k += __popc(__ballot_sync(0xffffffffu, f));
         }
-        if (lane == 0) cnt[ch] = (unsigned short)(k | kStageNoRecords);
+        if (lane == 0) {
+            cnt[ch] = (unsigned short)(k | kStageNoRecords);
+            if (k > 0) atomicAdd(tile_sum + ch / chunks_per_tile, k);   // (see EvolveArgs::tile_sum)
+        }
     }
 }
 
@@ -165,7 +169,10 @@ __global__ void __launch_bounds__(256) count_chunks_kernel(const TR* __restrict_
 // carrying the running total; tile_offset[t] = number of events before tile t, *d_total = *d_base (0 when
 // d_base is NULL) + their number.  d_base chains the slabs of step_host: the events of a slab follow those of
 // the slabs before it in the secondary buffers.  d_entries (not NULL: the append of cascade.cuh) = device count of
-// the entries that exist: only the chunks that hold them are read.
+// the entries that exist: only the chunks that hold them are read.  tile_sum (not NULL: the QED step) holds the tile
+// sums already, accumulated by the kernels that counted the chunks; they are read instead of the 16-bit counts
+// (one word per tile: the scan of 16 Mi particles reads 22 KB instead of 262 KB through its single CTA) and
+// reset to zero for the next call.
 constexpr int kScanThreads = 1024;
 constexpr int kScanItems = 4;
 
@@ -174,7 +181,8 @@ __global__ void __launch_bounds__(kScanThreads) tile_scan_kernel(const unsigned 
                                                                  unsigned long long* __restrict__ tile_offset,
                                                                  const unsigned long long* d_base,
                                                                  unsigned long long* d_total,
-                                                                 const unsigned long long* d_entries) {
+                                                                 const unsigned long long* d_entries,
+                                                                 unsigned int* __restrict__ tile_sum) {
     __shared__ unsigned long long warp_sum[2][kScanThreads / 32];
     if (d_entries) {
         const unsigned long long live = (*d_entries + kChunk - 1) / kChunk;
@@ -187,6 +195,19 @@ __global__ void __launch_bounds__(kScanThreads) tile_scan_kernel(const unsigned 
     for (long long base = 0; base < n_tiles; base += kScanThreads * kScanItems, ++round) {
         const long long t0 = base + (long long)tid * kScanItems;
         unsigned int v[kScanItems];
+        if (tile_sum != nullptr) {
+            if (t0 + kScanItems <= n_tiles) {   // t0 is a multiple of 4: 16-byte aligned
+                const uint4 q = *reinterpret_cast<const uint4*>(tile_sum + t0);
+                v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
+                *reinterpret_cast<uint4*>(tile_sum + t0) = make_uint4(0u, 0u, 0u, 0u);
+            } else {
+#pragma unroll
+                for (int k = 0; k < kScanItems; ++k) {
+                    v[k] = t0 + k < n_tiles ? tile_sum[t0 + k] : 0u;
+                    if (t0 + k < n_tiles) tile_sum[t0 + k] = 0u;
+                }
+            }
+        } else
 #pragma unroll
         for (int k = 0; k < kScanItems; ++k) {
             const long long c0 = (t0 + k) * chunks_per_tile;

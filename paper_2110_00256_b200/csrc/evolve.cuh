@@ -31,6 +31,10 @@ struct EvolveArgs {
     unsigned char* stage_rec;   // [n_chunks][kStageCap] records (see StageRecord), in index order
     unsigned short* stage_cnt;  // [n_chunks]: fired particles of the chunk | flags (see kStage* below)
     unsigned table_bytes;       // dynamic shared memory: [table, padded to 128 B][per-warp record buffers]
+    // EMIT: every chunk count is also added to the sum of its event tile (one RED per warp and tile), so that the
+    // offsets scan reads one word per tile instead of every chunk count
+    unsigned int* tile_sum;
+    int chunks_per_tile;
 };
 
 constexpr int kChunk = 128;                 // particles one warp handles per tile: the unit of record staging
@@ -242,8 +246,10 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                     total += all;
                 }
                 const long long chunk = (base + (long long)warp * WCH) / kChunk;
-                if (lane == 0)
+                if (lane == 0) {
                     a.stage_cnt[chunk] = (unsigned short)(total <= (unsigned)kStageCap ? total : (total | kStageNoRecords));
+                    if (total > 0) atomicAdd(a.tile_sum + chunk / a.chunks_per_tile, total);
+                }
                 if (total > 0 && total <= (unsigned)kStageCap) {  // (overflow: the event kernel re-scans the chunk)
                     // records are assembled in this warp's shared-memory buffer (scattered writes are cheap there)
                     // and leave as one coalesced stream of 128-bit stores

@@ -49,6 +49,7 @@ struct picsarqed_ctx {
     // per-chunk scratch of the event path: staged records, counts, output offsets (see events.cuh)
     void* rec = nullptr;
     size_t rec_bytes = 0;
+    size_t rec_sum_bytes = 0;  // its first bytes: the tile sums
     // host-path staging
     void* stage = nullptr;
     size_t stage_bytes = 0;
@@ -401,11 +402,11 @@ int launch_chi(picsarqed_ctx* c, long long n, const void* const* a, void* out) {
     return PICSARQED_OK;
 }
 
-struct StageView { unsigned char* rec; unsigned short* cnt; };
+struct StageView { unsigned char* rec; unsigned short* cnt; unsigned int* tile_sum; int chunks_per_tile; };
 
 template <typename R, typename TR, int SPECIES, int U, bool EMIT>
 int launch_evolve_u(picsarqed_ctx* c, long long n, const void* const* a, double dt, void* tau,
-                    unsigned long long* d_n_events, StageView sv = StageView{nullptr, nullptr}) {
+                    unsigned long long* d_n_events, StageView sv = StageView{nullptr, nullptr, nullptr, 1}) {
     constexpr int V = 16 / sizeof(R);
     constexpr int TILE = kEvolveThreads * V * U;
     EvolveArgs<R, TR> args;
@@ -423,6 +424,8 @@ int launch_evolve_u(picsarqed_ctx* c, long long n, const void* const* a, double 
     args.d_n_events = d_n_events;
     args.stage_rec = sv.rec;
     args.stage_cnt = sv.cnt;
+    args.tile_sum = sv.tile_sum;
+    args.chunks_per_tile = sv.chunks_per_tile;
     size_t smem = ((size_t)args.tab.n * sizeof(R) + 127) & ~(size_t)127;
     args.table_in_smem = smem <= 96 * 1024;  // larger tables are read through L1/L2
     if (!args.table_in_smem) smem = 0;
@@ -452,34 +455,51 @@ int launch_evolve(picsarqed_ctx* c, long long n, const void* const* a, double dt
     return launch_evolve_u<R, TR, SPECIES, 2, false>(c, n, a, dt, tau, d_n_events);
 }
 
-// per-chunk scratch: [records][counts][offsets]
-struct ChunkScratch { unsigned char* rec; unsigned short* cnt; unsigned long long* off; long long n_chunks; };
+// per-chunk scratch: [tile sums][records][counts][offsets]
+struct ChunkScratch { unsigned char* rec; unsigned short* cnt; unsigned long long* off; unsigned int* sum; long long n_chunks; };
 
 template <typename R>
 int chunk_scratch(picsarqed_ctx* c, long long n, ChunkScratch* out) {
     const long long nchunks = (n + kChunk - 1) / kChunk;
     const size_t rec_sz = ((size_t)nchunks * kStageCap * StageRecord<R>::kBytes + 255) & ~(size_t)255;
     const size_t cnt_sz = ((size_t)nchunks * sizeof(unsigned short) + 255) & ~(size_t)255;
-    // tiles hold at least 8 chunks: n_chunks/8 + 1 tile offsets are always enough
+    // tiles hold at least 8 chunks: n_chunks/8 + 1 tile offsets and tile sums are always enough
     const size_t off_sz = ((size_t)(nchunks / 8 + 2) * sizeof(unsigned long long) + 255) & ~(size_t)255;
-    if (rec_sz + cnt_sz + off_sz > c->rec_bytes) {  // grow (synchronises): half as much again when a population
-        PXQ_CUDA(c, cudaStreamSynchronize(c->stream));  // creeps up step after step (closed loop), exact otherwise
-        const size_t need = rec_sz + cnt_sz + off_sz;
-        const size_t want = c->rec_bytes > 0 && need < c->rec_bytes + c->rec_bytes / 2 ? c->rec_bytes + c->rec_bytes / 2 : need;
+    const size_t sum_sz = ((size_t)(nchunks / 8 + 2) * sizeof(unsigned int) + 255) & ~(size_t)255;
+    // the tile sums live at the FRONT of the buffer (their place must not move with n: they are kept at zero
+    // between calls), then records, counts, offsets
+    const size_t body = rec_sz + cnt_sz + off_sz;
+    if (sum_sz > c->rec_sum_bytes || c->rec_sum_bytes + body > c->rec_bytes) {
+        // grow (synchronises): half as much again when a population creeps up step after step (closed loop),
+        // exact the first time
+        PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+        const bool headroom = c->rec_bytes > 0;
+        const size_t sum_want = headroom ? (sum_sz + sum_sz / 2 + 255) & ~(size_t)255 : sum_sz;
+        const size_t want = sum_want + (headroom ? body + body / 2 : body);
         if (c->rec) cudaFree(c->rec);
         c->rec = nullptr;
         c->rec_bytes = 0;
+        c->rec_sum_bytes = 0;
         PXQ_CUDA(c, cudaMalloc(&c->rec, want));
+        PXQ_CUDA(c, cudaMemsetAsync(c->rec, 0, sum_want, c->stream));   // tile sums start (and are kept) at zero
         c->rec_bytes = want;
+        c->rec_sum_bytes = sum_want;
     }
-    out->rec = static_cast<unsigned char*>(c->rec);
+    out->sum = static_cast<unsigned int*>(c->rec);
+    out->rec = static_cast<unsigned char*>(c->rec) + c->rec_sum_bytes;
     out->cnt = reinterpret_cast<unsigned short*>(out->rec + rec_sz);
     out->off = reinterpret_cast<unsigned long long*>(out->rec + rec_sz + cnt_sz);
     out->n_chunks = nchunks;
     return PICSARQED_OK;
 }
 
-// levels 2 and 3 of the compaction: chunk counts -> offsets -> events
+// chunks per tile of the configured event_kernel shape
+int event_chunks_per_tile(const picsarqed_ctx* c) {
+    static const int kChunksOf[8] = {24, 32, 24, 16, 12, 24, 24, 32};  // must match the switch in launch_event_pass
+    return kChunksOf[c->event_config];
+}
+
+// levels 2 and 3 of the compaction: chunk counts (and their tile sums) -> offsets -> events
 template <typename R, typename TR, int KIND>
 int launch_event_pass(picsarqed_ctx* c, long long n, const ChunkScratch& cs, void* const* p, const void* const* eb,
                       void* tau, unsigned long long seed, unsigned long long step, unsigned long long id_base,
@@ -506,11 +526,10 @@ int launch_event_pass(picsarqed_ctx* c, long long n, const ChunkScratch& cs, voi
     ev.tile_offset = cs.off;
     ev.slot_base = c->link_slot_base;
     ev.parent_base = c->link_parent_base;
-    static const int kChunksOf[8] = {24, 32, 24, 16, 12, 24, 24, 32};  // must match the switch below
-    const int chunks = kChunksOf[c->event_config];
+    const int chunks = event_chunks_per_tile(c);
     const long long n_tiles = (cs.n_chunks + chunks - 1) / chunks;
     tile_scan_kernel<<<1, kScanThreads, 0, c->stream>>>(cs.cnt, cs.n_chunks, chunks, n_tiles, cs.off, c->link_slot_base, d_n_out,
-                                                        nullptr);
+                                                        nullptr, cs.sum);
 #define PXQ_LAUNCH_EVENTS(T, CH, MB)                                                                         \
     do {                                                                                                     \
         auto kern = event_kernel<R, TR, KIND, T, CH, MB>;                                                    \
@@ -543,7 +562,8 @@ int launch_events(picsarqed_ctx* c, long long n, void* const* p, const void* con
     ChunkScratch cs;
     if (int rc = chunk_scratch<R>(c, n, &cs)) return rc;
     const int grid = (int)std::max<long long>(1, std::min<long long>((cs.n_chunks + 7) / 8, (long long)c->num_sms * 8));
-    count_chunks_kernel<TR><<<grid, 256, 0, c->stream>>>((const TR*)tau, n, 0, cs.n_chunks, cs.cnt);
+    count_chunks_kernel<TR><<<grid, 256, 0, c->stream>>>((const TR*)tau, n, 0, cs.n_chunks, cs.cnt, cs.sum,
+                                                         event_chunks_per_tile(c));
     return launch_event_pass<R, TR, KIND>(c, n, cs, p, eb, tau, seed, step, id_base, capacity, out_p, out_tau, parent,
                                           d_n_out);
 }
@@ -558,6 +578,8 @@ int launch_step(picsarqed_ctx* c, long long n, void* const* p, const void* const
     StageView sv;
     sv.rec = cs.rec;
     sv.cnt = cs.cnt;
+    sv.tile_sum = cs.sum;
+    sv.chunks_per_tile = event_chunks_per_tile(c);
     const void* a9[9] = {p[0], p[1], p[2], eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]};
     constexpr int U = kChunk / (32 * (16 / (int)sizeof(R)));  // fp64: 2, fp32: 1
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
@@ -568,7 +590,8 @@ int launch_step(picsarqed_ctx* c, long long n, void* const* p, const void* const
     if (int rc = launch_evolve_u<R, TR, SPECIES, U, true>(c, n, a9, dt, tau, nullptr, sv)) return rc;
     constexpr long long kTile = (long long)kEvolveThreads * (16 / (int)sizeof(R)) * U;
     if (n % kTile)  // the ragged last tile stages no records: count its chunks from the updated tau
-        count_chunks_kernel<TR><<<1, 256, 0, c->stream>>>((const TR*)tau, n, (n / kTile) * kTile / kChunk, cs.n_chunks, cs.cnt);
+        count_chunks_kernel<TR><<<1, 256, 0, c->stream>>>((const TR*)tau, n, (n / kTile) * kTile / kChunk, cs.n_chunks, cs.cnt,
+                                                          cs.sum, sv.chunks_per_tile);
     if (c->time_kernels) PXQ_CUDA(c, cudaEventRecord(ev[1], c->stream));
     if (int rc = launch_event_pass<R, TR, SPECIES>(c, n, cs, p, eb, tau, seed, step, id_base, capacity, out_p, out_tau,
                                                    parent, d_n_out))
@@ -603,7 +626,7 @@ int launch_append(picsarqed_ctx* c, long long m_max, const void* const* s_p, con
                                                        min_energy, cs.n_chunks, cs.cnt);
     const long long n_tiles = (cs.n_chunks + kAppendChunksPerTile - 1) / kAppendChunksPerTile;
     tile_scan_kernel<<<1, kScanThreads, 0, c->stream>>>(cs.cnt, cs.n_chunks, kAppendChunksPerTile, n_tiles, cs.off, nullptr,
-                                                        d_kept, d_count);
+                                                        d_kept, d_count, nullptr);
     AppendArgs<R, TR> a;
     for (int k = 0; k < 3; ++k) {
         a.s_p[k] = (const R*)s_p[k];
