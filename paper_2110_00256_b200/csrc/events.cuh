@@ -275,15 +275,20 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
         return (tile < n_tiles && lane < CHUNKS && ch < n_chunks) ? a.stage_cnt[ch] : (unsigned short)0;
     };
     const unsigned long long slot_base = a.slot_base ? *a.slot_base : 0ull;
-    long long tile = blockIdx.x;
-    unsigned short flags_next = load_flags(tile);
-    unsigned long long excl_next = tile < n_tiles ? a.tile_offset[tile] : 0ull;
-    for (; tile < n_tiles; tile += gridDim.x) {
+    // (the tiles are walked from the last one down: the particles the evolve pass streamed last are the ones whose
+    // sectors may still be in L2 when their parents are rewritten)
+#define PXQ_TILE_OF(it) (n_tiles - 1 - (it))
+    long long it = blockIdx.x;
+    unsigned short flags_next = it < n_tiles ? load_flags(PXQ_TILE_OF(it)) : (unsigned short)0;
+    unsigned long long excl_next = it < n_tiles ? a.tile_offset[PXQ_TILE_OF(it)] : 0ull;
+    for (; it < n_tiles; it += gridDim.x) {
+    const long long tile = PXQ_TILE_OF(it);
     const long long first_chunk = tile * CHUNKS;
     const unsigned short flags = flags_next;
     const unsigned long long excl = excl_next;                            // output slot of the tile's first event
-    flags_next = load_flags(tile + gridDim.x);
-    excl_next = tile + gridDim.x < n_tiles ? a.tile_offset[tile + gridDim.x] : 0ull;
+    const long long it_next = it + gridDim.x;
+    flags_next = it_next < n_tiles ? load_flags(PXQ_TILE_OF(it_next)) : (unsigned short)0;
+    excl_next = it_next < n_tiles ? a.tile_offset[PXQ_TILE_OF(it_next)] : 0ull;
     const unsigned int cnt = flags & kStageCountMask;
     unsigned int incl = cnt;                                             // offsets of the chunks inside the tile
 #pragma unroll
@@ -351,6 +356,7 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
         event_commit<R, TR, KIND>(a, i, slot, out);
     }
     }  // tiles
+#undef PXQ_TILE_OF
 }
 
 }  // namespace pxq
