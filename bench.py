@@ -28,9 +28,9 @@ UNIT = "particles/s"
 SEED = 2
 BYTES_PER_PARTICLE_EVOLVE = 88  # 9 reads + tau read + tau write, fp64
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the evolve pass (16 Mi particles), ncu --set full:
-# profiles/r1c_step_full.md (1.343656 GB read = the 80 B/particle of inputs; 109 MB written: part of the 134 MB of
+# profiles/r1d_step_full.md (1.343606 GB read = the 80 B/particle of inputs; 109 MB written: part of the 134 MB of
 # new tau is still dirty in L2 when the kernel ends, plus the staged records)
-EVOLVE_DRAM_TRAFFIC_BYTES = 1343656000 + 109172224
+EVOLVE_DRAM_TRAFFIC_BYTES = 1343606000 + 108954112
 
 
 def parse():
