@@ -84,6 +84,30 @@ int picsarqed_version(void);
  * "host_slabs" 0..64 = number of slabs step_host pipelines (0 = automatic: slabs of at least
  * 2^20 particles, at most 32; 1 = copy in, step, copy out, one after the other). */
 int picsarqed_set_option(picsarqed_ctx* ctx, const char* name, long long value);
+/* ---- unit systems --------------------------------------------------------
+ * The library's own units: momenta in m_e c, E in E_s = m_e^2 c^3/(q_e hbar), B in E_s/c, times in
+ * seconds.  set_units declares the unit system of the CALLER's arrays for chi,
+ * evolve_optical_depth, generate_photons, generate_pairs, qed_step, step_host and schwinger_rate:
+ * momenta and fields are scaled in registers where they are loaded, momenta back where they are
+ * stored (no extra pass over memory); dt is taken in the system's time unit.  Tables are
+ * adimensional and serve every system.  The closed-loop calls take the library's units only.
+ *   LIBRARY      the default
+ *   SI           kg m/s, V/m, T, s
+ *   NORM_OMEGA   c = q_e = m_e = 1 with a reference angular frequency `reference` [1/s]: p in m_e c,
+ *                E in m_e c omega/q_e, B in m_e omega/q_e, t in 1/omega
+ *   NORM_LAMBDA  the same with a reference length `reference` [m] (omega = c/lambda)
+ *   HL_MEV       Heaviside-Lorentz natural units (hbar = c = 1) with 1 MeV: p in MeV, E and B in MeV^2,
+ *                t in 1/MeV (the paper's internal system)
+ * get_unit_scales writes the four multipliers (p, E, B, t) that take the caller's values to the
+ * library's units. */
+#define PICSARQED_UNITS_LIBRARY 0
+#define PICSARQED_UNITS_SI 1
+#define PICSARQED_UNITS_NORM_OMEGA 2
+#define PICSARQED_UNITS_NORM_LAMBDA 3
+#define PICSARQED_UNITS_HL_MEV 4
+int picsarqed_set_units(picsarqed_ctx* ctx, int system, double reference);
+int picsarqed_get_unit_scales(picsarqed_ctx* ctx, double* scales /* host, 4 doubles */);
+
 /* With "time_kernels" = 1 every qed_step brackets its evolve pass and its event pass (offsets scan +
  * event kernel) with CUDA events on the context's stream.  get_timing synchronises, writes the
  * accumulated milliseconds host_ms[0] (evolve pass) and host_ms[1] (event pass) and the number of

@@ -14,6 +14,7 @@ from .build import build
 
 F32, F64 = 0, 1
 LEPTON, PHOTON = 0, 1
+UNITS_LIBRARY, UNITS_SI, UNITS_NORM_OMEGA, UNITS_NORM_LAMBDA, UNITS_HL_MEV = 0, 1, 2, 3, 4
 TAB_LNG, TAB_QS_LNP, TAB_LNT, TAB_BW_P = 0, 1, 2, 3
 
 _vp, _u64, _i64, _i, _d = C.c_void_p, C.c_uint64, C.c_longlong, C.c_int, C.c_double
@@ -57,6 +58,8 @@ _SIGNATURES = {
     "picsarqed_destroy": (_i, [_vp]),
     "picsarqed_last_error": (C.c_char_p, [_vp]),
     "picsarqed_set_option": (_i, [_vp, C.c_char_p, _i64]),
+    "picsarqed_set_units": (_i, [_vp, _i, _d]),
+    "picsarqed_get_unit_scales": (_i, [_vp, C.POINTER(_d)]),
     "picsarqed_get_timing": (_i, [_vp, C.POINTER(_d), C.POINTER(_i64)]),
     "picsarqed_build_tables": (_i, [_vp, C.POINTER(_CParams), _d]),
     "picsarqed_export_tables": (_i, [_vp, _i, _vp, C.c_size_t]),
@@ -267,6 +270,16 @@ class Context:
             tau.data_ptr(), float(dt), seed, step, id_base, capacity, C.cast(sec_ptrs, _vp),
             parent.data_ptr() if parent is not None else None, C.byref(n_out)))
         return int(n_out.value)
+
+    # ---- unit systems ---------------------------------------------------------
+    def set_units(self, system, reference=0.0):
+        self._check(lib().picsarqed_set_units(self._h, system, float(reference)))
+
+    def unit_scales(self):
+        """multipliers (p, E, B, t) from the caller's unit system to the library's"""
+        v = (_d * 4)()
+        self._check(lib().picsarqed_get_unit_scales(self._h, v))
+        return tuple(v)
 
     # ---- table functions per value (SURVEY.md 8(f)-4) -----------------------------------------
     def table_function(self, kind, chi, out):

@@ -44,6 +44,8 @@ struct EventArgs {
     // follow the *slot_base events of the slabs before it (device word, NULL = 0), parents are numbered globally
     const unsigned long long* slot_base;
     long long parent_base;
+    UnitScales units;   // the caller's unit system: momenta and fields are scaled where they are loaded, momenta back
+                        // where they are stored; the event arithmetic itself is in the library's units
 };
 
 template <typename R, typename TR>
@@ -73,15 +75,16 @@ __device__ __forceinline__ EventOut<R, TR> qs_event_compute(const EventArgs<R, T
     const double k2 = km1 * (1.0 - xi);         // emitter kinetic energy after the emission
     const double pn2 = sqrt(k2 * (k2 + 2.0));   // sqrt(gamma'^2 - 1)
     EventOut<R, TR> o;
-    o.sec[0] = (R)(gph * nx);                   // emitted along p
-    o.sec[1] = (R)(gph * ny);
-    o.sec[2] = (R)(gph * nz);
+    const double ip = a.units.inv_p;
+    o.sec[0] = (R)(gph * nx * ip);              // emitted along p
+    o.sec[1] = (R)(gph * ny * ip);
+    o.sec[2] = (R)(gph * nz * ip);
     o.sec[3] = o.sec[4] = o.sec[5] = (R)0;
     o.sec_tau[0] = draw_tau<TR>(wc.w[0], wc.w[1]);
     o.sec_tau[1] = (TR)0;
-    o.parent_p[0] = (R)(pn2 * nx);
-    o.parent_p[1] = (R)(pn2 * ny);
-    o.parent_p[2] = (R)(pn2 * nz);
+    o.parent_p[0] = (R)(pn2 * nx * ip);
+    o.parent_p[1] = (R)(pn2 * ny * ip);
+    o.parent_p[2] = (R)(pn2 * nz * ip);
     o.parent_tau = draw_tau<TR>(w.w[2], w.w[3]);
     return o;
 }
@@ -106,12 +109,13 @@ __device__ __forceinline__ EventOut<R, TR> bw_event_compute(const EventArgs<R, T
     const double inv_g = g > 0.0 ? 1.0 / g : 0.0;
     const double nx = px * inv_g, ny = py * inv_g, nz = pz * inv_g;
     EventOut<R, TR> o;
-    o.sec[0] = (R)(pe * nx);
-    o.sec[1] = (R)(pe * ny);
-    o.sec[2] = (R)(pe * nz);
-    o.sec[3] = (R)(pp * nx);
-    o.sec[4] = (R)(pp * ny);
-    o.sec[5] = (R)(pp * nz);
+    const double ip = a.units.inv_p;
+    o.sec[0] = (R)(pe * nx * ip);
+    o.sec[1] = (R)(pe * ny * ip);
+    o.sec[2] = (R)(pe * nz * ip);
+    o.sec[3] = (R)(pp * nx * ip);
+    o.sec[4] = (R)(pp * ny * ip);
+    o.sec[5] = (R)(pp * nz * ip);
     o.sec_tau[0] = draw_tau<TR>(wc.w[0], wc.w[1]);
     o.sec_tau[1] = draw_tau<TR>(wc.w[2], wc.w[3]);
     o.parent_p[0] = o.parent_p[1] = o.parent_p[2] = (R)0;   // photon removed: p = 0, tau = +inf
@@ -343,13 +347,16 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
             union { uint4 raw[StageRecord<R>::kVecs]; StageRecord<R> rec; } u;
 #pragma unroll
             for (int k = 0; k < StageRecord<R>::kVecs; ++k) u.raw[k] = __ldg(src + k);
-            px = u.rec.p[0]; py = u.rec.p[1]; pz = u.rec.p[2];
+            const double sp = a.units.p;
+            px = u.rec.p[0] * sp; py = u.rec.p[1] * sp; pz = u.rec.p[2] * sp;   // (records hold the caller's units)
             c2 = u.rec.c2;
             i = cbase + u.rec.idx;
         } else {
             i = cbase + list[j][r];
-            px = a.p[0][i]; py = a.p[1][i]; pz = a.p[2][i];
-            c2 = event_c2<KIND>(px, py, pz, a.e[0][i], a.e[1][i], a.e[2][i], a.b[0][i], a.b[1][i], a.b[2][i]);
+            const double sp = a.units.p, se = a.units.e, sb = a.units.b;
+            px = a.p[0][i] * sp; py = a.p[1][i] * sp; pz = a.p[2][i] * sp;
+            c2 = event_c2<KIND>(px, py, pz, a.e[0][i] * se, a.e[1][i] * se, a.e[2][i] * se, a.b[0][i] * sb, a.b[1][i] * sb,
+                                a.b[2][i] * sb);
         }
         const EventOut<R, TR> out = KIND == 0 ? qs_event_compute<R, TR>(a, i, px, py, pz, c2)
                                               : bw_event_compute<R, TR>(a, i, px, py, pz, c2);

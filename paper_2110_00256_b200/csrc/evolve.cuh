@@ -35,6 +35,7 @@ struct EvolveArgs {
     // offsets scan reads one word per tile instead of every chunk count
     unsigned int* tile_sum;
     int chunks_per_tile;
+    UnitScales units;           // the caller's unit system (picsarqed_set_units)
 };
 
 constexpr int kChunk = 128;                 // particles one warp handles per tile: the unit of record staging
@@ -96,13 +97,17 @@ __host__ __device__ constexpr double hankel13(int k) {
 }
 
 // Returns the decrement dN/dt * dt in the particle arithmetic type A (float or double).
-template <typename R, int SPECIES>
+// SCALED: the arrays are in another unit system (picsarqed_set_units): nine multiplications in registers.
+template <typename R, int SPECIES, bool SCALED = false>
 __device__ __forceinline__ auto decrement_one(R pxr, R pyr, R pzr, R exr, R eyr, R ezr, R bxr, R byr, R bzr,
                                               const R* tab, const Table1D<R>& T, double rate_dt,
-                                              double* c2_out = nullptr) -> R {
+                                              const UnitScales& us, double* c2_out = nullptr) -> R {
     typedef R A;
     double inv_g, g2;
-    const double c2 = chi_squared_of<SPECIES>(pxr, pyr, pzr, exr, eyr, ezr, bxr, byr, bzr, &inv_g, &g2);
+    const double c2 =
+        SCALED ? chi_squared_of<SPECIES>(pxr * us.p, pyr * us.p, pzr * us.p, exr * us.e, eyr * us.e, ezr * us.e,
+                                         bxr * us.b, byr * us.b, bzr * us.b, &inv_g, &g2)
+               : chi_squared_of<SPECIES>(pxr, pyr, pzr, exr, eyr, ezr, bxr, byr, bzr, &inv_g, &g2);
     if (c2_out) *c2_out = c2;
     A lc;
     if constexpr (sizeof(R) == 8) lc = 0.5 * log_pos(c2); else lc = 0.5f * logf((float)c2);
@@ -174,7 +179,7 @@ __device__ __forceinline__ auto decrement_one(R pxr, R pyr, R pzr, R exr, R eyr,
 // EMIT: also append a record (momentum, chi^2, index in chunk) of every particle that fired to the staging
 // segment of its 128-particle chunk, in index order (warp ballot/popc; no CTA barrier), for event_kernel.
 // Requires U*32*V == kChunk.
-template <typename R, typename TR, int SPECIES, int U, bool EMIT>
+template <typename R, typename TR, int SPECIES, int U, bool EMIT, bool SCALED>
 __global__ void __launch_bounds__(kEvolveThreads, U > 2 ? 1 : ((sizeof(R) == 4 && U == 1 && SPECIES == 0) ? 3 : 2))
 evolve_kernel(const EvolveArgs<R, TR> a) {
     constexpr int V = 16 / sizeof(R);
@@ -221,9 +226,9 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
             for (int u = 0; u < U; ++u) {
 #pragma unroll
                 for (int v = 0; v < V; ++v) {
-                    const R d = decrement_one<R, SPECIES>(q[0][u].v[v], q[1][u].v[v], q[2][u].v[v], q[3][u].v[v],
+                    const R d = decrement_one<R, SPECIES, SCALED>(q[0][u].v[v], q[1][u].v[v], q[2][u].v[v], q[3][u].v[v],
                                                           q[4][u].v[v], q[5][u].v[v], q[6][u].v[v], q[7][u].v[v],
-                                                          q[8][u].v[v], tab, a.tab, a.rate_dt,
+                                                          q[8][u].v[v], tab, a.tab, a.rate_dt, a.units,
                                                           EMIT ? &c2s[EMIT ? u * V + v : 0] : nullptr);
                     const TR tn = t[u].v[v] - (TR)d;
                     t[u].v[v] = tn;
@@ -287,9 +292,9 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
             }
         } else {  // ragged last tile: scalar, guarded (qed_step counts its chunks afterwards: count_chunks_kernel)
             for (long long i = base + threadIdx.x; i < a.n; i += kEvolveThreads) {
-                const R d = decrement_one<R, SPECIES>(a.p[0][i], a.p[1][i], a.p[2][i], a.e[0][i], a.e[1][i],
+                const R d = decrement_one<R, SPECIES, SCALED>(a.p[0][i], a.p[1][i], a.p[2][i], a.e[0][i], a.e[1][i],
                                                       a.e[2][i], a.b[0][i], a.b[1][i], a.b[2][i], tab, a.tab,
-                                                      a.rate_dt);
+                                                      a.rate_dt, a.units);
                 const TR tn = a.tau[i] - (TR)d;
                 a.tau[i] = tn;
                 fired += tn < (TR)0 ? 1u : 0u;
@@ -324,15 +329,17 @@ __global__ void __launch_bounds__(256) chi_kernel(const R* __restrict__ px, cons
                                                   const R* __restrict__ pz, const R* __restrict__ ex,
                                                   const R* __restrict__ ey, const R* __restrict__ ez,
                                                   const R* __restrict__ bx, const R* __restrict__ by,
-                                                  const R* __restrict__ bz, R* __restrict__ out, long long n) {
+                                                  const R* __restrict__ bz, R* __restrict__ out, long long n,
+                                                  const UnitScales us) {
     constexpr int V = 16 / sizeof(R);
     const long long nvec = n / V;
     const long long stride = (long long)gridDim.x * blockDim.x;
-    auto one = [](R pxr, R pyr, R pzr, R exr, R eyr, R ezr, R bxr, R byr, R bzr) -> R {
-        const double x = pxr, y = pyr, z = pzr;
+    auto one = [&us](R pxr, R pyr, R pzr, R exr, R eyr, R ezr, R bxr, R byr, R bzr) -> R {
+        const double x = pxr * us.p, y = pyr * us.p, z = pzr * us.p;
         const double p2 = fma(x, x, fma(y, y, z * z));
         const double g = sqrt(SPECIES == 0 ? 1.0 + p2 : p2);
-        return (R)sqrt(chi_squared<SPECIES>(x, y, z, exr, eyr, ezr, bxr, byr, bzr, g, p2));
+        return (R)sqrt(chi_squared<SPECIES>(x, y, z, exr * us.e, eyr * us.e, ezr * us.e, bxr * us.b, byr * us.b,
+                                            bzr * us.b, g, p2));
     };
     const unsigned long long pol = l2_policy_evict_first();
     for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < nvec; j += stride) {
@@ -391,11 +398,12 @@ template <typename R>
 __global__ void __launch_bounds__(256) schwinger_kernel(const R* __restrict__ ex, const R* __restrict__ ey,
                                                         const R* __restrict__ ez, const R* __restrict__ bx,
                                                         const R* __restrict__ by, const R* __restrict__ bz,
-                                                        double* __restrict__ out, long long n) {
+                                                        double* __restrict__ out, long long n, const UnitScales us) {
     constexpr int V = 16 / sizeof(R);
     const long long nvec = n / V;
     const long long stride = (long long)gridDim.x * blockDim.x;
     const unsigned long long pol = l2_policy_evict_first();
+    const double se = us.e, sb = us.b;
     for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < nvec; j += stride) {
         const long long i = j * V;
         const Vec<R, V> a0 = ld_stream<R, V>(ex + i, pol), a1 = ld_stream<R, V>(ey + i, pol), a2 = ld_stream<R, V>(ez + i, pol),
@@ -403,13 +411,14 @@ __global__ void __launch_bounds__(256) schwinger_kernel(const R* __restrict__ ex
 #pragma unroll
         for (int v = 0; v < V; v += 2) {
             double2 o;
-            o.x = schwinger_rate_one(a0.v[v], a1.v[v], a2.v[v], a3.v[v], a4.v[v], a5.v[v]);
-            o.y = schwinger_rate_one(a0.v[v + 1], a1.v[v + 1], a2.v[v + 1], a3.v[v + 1], a4.v[v + 1], a5.v[v + 1]);
+            o.x = schwinger_rate_one(a0.v[v] * se, a1.v[v] * se, a2.v[v] * se, a3.v[v] * sb, a4.v[v] * sb, a5.v[v] * sb);
+            o.y = schwinger_rate_one(a0.v[v + 1] * se, a1.v[v + 1] * se, a2.v[v + 1] * se, a3.v[v + 1] * sb, a4.v[v + 1] * sb,
+                                     a5.v[v + 1] * sb);
             *reinterpret_cast<double2*>(out + i + v) = o;
         }
     }
     for (long long i = nvec * V + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
-        out[i] = schwinger_rate_one(ex[i], ey[i], ez[i], bx[i], by[i], bz[i]);
+        out[i] = schwinger_rate_one(ex[i] * se, ey[i] * se, ez[i] * se, bx[i] * sb, by[i] * sb, bz[i] * sb);
 }
 
 // ---- tau = -ln U, purpose 0, step 0 -------------------------------

@@ -23,7 +23,7 @@ __global__ void __launch_bounds__(256) table_function_kernel(const R* __restrict
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
         const double c = chi[i];
-        const R d = decrement_one<R, KIND>((R)g, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)(c / g), T.L, T, 1.0);
+        const R d = decrement_one<R, KIND>((R)g, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)0, (R)(c / g), T.L, T, 1.0, UnitScales());
         const double gamma = KIND == 0 ? sqrt(1.0 + g * g) : g;
         out[i] = KIND == 0 ? (R)((double)d * gamma) : (R)((double)d * gamma / c);
     }

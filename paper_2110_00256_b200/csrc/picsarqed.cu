@@ -43,6 +43,10 @@ struct picsarqed_ctx {
     // tuning knobs (picsarqed_set_option)
     int evolve_unroll = 0;       // 0 = default per dtype
     int evolve_ctas_per_sm = 0;  // 0 = occupancy
+    // unit system of the caller's arrays (picsarqed_set_units): multipliers to p/(m_e c), E/E_s, cB/E_s, seconds
+    UnitScales units;
+    double t_scale = 1.0;
+    int unit_system = 0;
     int event_config = 0;        // shape of event_kernel: see launch_event_pass
     int time_kernels = 0;        // qed_step brackets its evolve pass and its event pass with CUDA events
     std::vector<cudaEvent_t> timing_events;  // triples (start, after evolve, after events), not yet read
@@ -326,6 +330,58 @@ int picsarqed_set_option(picsarqed_ctx* c, const char* name, long long value) {
     return PICSARQED_OK;
 }
 
+// PAPER.md:275.  CODATA 2018: c, h, e exact; m_e, alpha recommended values (qed_device.cuh).
+int picsarqed_set_units(picsarqed_ctx* c, int system, double reference) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    constexpr double kCharge = 1.602176634e-19;                       // C
+    constexpr double kHbar = kPlanck / (2.0 * kPi);                   // J s
+    constexpr double kMc = kElectronMass * kLightSpeed;               // m_e c, kg m/s
+    constexpr double kEs = kElectronMass * kElectronMass * kLightSpeed * kLightSpeed * kLightSpeed / (kCharge * kHbar);  // V/m
+    constexpr double kMeV = 1e6 * kCharge;                            // J
+    constexpr double kMassMeV = kElectronMass * kLightSpeed * kLightSpeed / kMeV;  // m_e c^2 in MeV
+    double sp = 1.0, se = 1.0, sb = 1.0, st = 1.0;
+    switch (system) {
+        case PICSARQED_UNITS_LIBRARY: break;
+        case PICSARQED_UNITS_SI:            // kg m/s, V/m, T, s
+            sp = 1.0 / kMc;
+            se = 1.0 / kEs;
+            sb = kLightSpeed / kEs;
+            break;
+        case PICSARQED_UNITS_NORM_OMEGA:    // c = e = m_e = 1 and a reference angular frequency omega [1/s]:
+            if (!(reference > 0.0)) return fail(c, PICSARQED_ERR_INVALID, "set_units: reference frequency must be > 0");
+            se = sb = kElectronMass * kLightSpeed * reference / kCharge / kEs;  // E unit m c omega/e, B unit m omega/e
+            st = 1.0 / reference;
+            break;
+        case PICSARQED_UNITS_NORM_LAMBDA:   // the same with a reference length lambda [m]: omega = c/lambda
+            if (!(reference > 0.0)) return fail(c, PICSARQED_ERR_INVALID, "set_units: reference length must be > 0");
+            se = sb = kElectronMass * kLightSpeed * kLightSpeed / (kCharge * reference) / kEs;
+            st = reference / kLightSpeed;
+            break;
+        case PICSARQED_UNITS_HL_MEV:        // Heaviside-Lorentz natural units (hbar = c = 1), 1 MeV: p in MeV, E and
+            sp = 1.0 / kMassMeV;            // B in MeV^2, t in 1/MeV; e_HL = sqrt(4 pi alpha), E_s = m^2/e_HL
+            se = sb = std::sqrt(4.0 * kPi * kFineStructure) / (kMassMeV * kMassMeV);
+            st = kHbar / kMeV;
+            break;
+        default: return fail(c, PICSARQED_ERR_INVALID, "set_units: unknown unit system");
+    }
+    c->units.p = sp;
+    c->units.e = se;
+    c->units.b = sb;
+    c->units.inv_p = 1.0 / sp;
+    c->t_scale = st;
+    c->unit_system = system;
+    return PICSARQED_OK;
+}
+
+int picsarqed_get_unit_scales(picsarqed_ctx* c, double* scales) {
+    if (!c || !scales) return PICSARQED_ERR_INVALID;
+    scales[0] = c->units.p;
+    scales[1] = c->units.e;
+    scales[2] = c->units.b;
+    scales[3] = c->t_scale;
+    return PICSARQED_OK;
+}
+
 int picsarqed_get_timing(picsarqed_ctx* c, double* host_ms, long long* host_calls) {
     if (!c || !host_ms || !host_calls) return PICSARQED_ERR_INVALID;
     PXQ_CUDA(c, cudaSetDevice(c->device));
@@ -397,7 +453,7 @@ int launch_chi(picsarqed_ctx* c, long long n, const void* const* a, void* out) {
     constexpr int V = 16 / sizeof(R);
     chi_kernel<R, SPECIES><<<stream_grid(c, (n + V - 1) / V, 256), 256, 0, c->stream>>>(
         (const R*)a[0], (const R*)a[1], (const R*)a[2], (const R*)a[3], (const R*)a[4], (const R*)a[5],
-        (const R*)a[6], (const R*)a[7], (const R*)a[8], (R*)out, n);
+        (const R*)a[6], (const R*)a[7], (const R*)a[8], (R*)out, n, c->units);
     PXQ_CUDA(c, cudaGetLastError());
     return PICSARQED_OK;
 }
@@ -418,7 +474,8 @@ int launch_evolve_u(picsarqed_ctx* c, long long n, const void* const* a, double 
     args.tau = (TR*)tau;
     args.n = n;
     args.tab = view_1d<R>(c, SPECIES);
-    args.rate_dt = (SPECIES == 0 ? 2.0 / 3.0 : 1.0) * kAlphaOverTauC * dt;
+    args.rate_dt = (SPECIES == 0 ? 2.0 / 3.0 : 1.0) * kAlphaOverTauC * (dt * c->t_scale);  // dt in the caller's time unit
+    args.units = c->units;
     args.partials = c->partials;
     args.ticket = c->ticket;
     args.d_n_events = d_n_events;
@@ -431,7 +488,9 @@ int launch_evolve_u(picsarqed_ctx* c, long long n, const void* const* a, double 
     if (!args.table_in_smem) smem = 0;
     args.table_bytes = (unsigned)smem;
     if (EMIT) smem += (size_t)(kEvolveThreads / 32) * kStageCap * StageRecord<R>::kBytes;
-    auto kern = evolve_kernel<R, TR, SPECIES, U, EMIT>;
+    // (the scaled variant only when the caller's arrays are in another unit system: the default path pays nothing)
+    auto kern = c->unit_system != PICSARQED_UNITS_LIBRARY ? evolve_kernel<R, TR, SPECIES, U, EMIT, true>
+                                                          : evolve_kernel<R, TR, SPECIES, U, EMIT, false>;
     if (smem > 48 * 1024) PXQ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
     PXQ_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kEvolveThreads, smem));
@@ -526,6 +585,7 @@ int launch_event_pass(picsarqed_ctx* c, long long n, const ChunkScratch& cs, voi
     ev.tile_offset = cs.off;
     ev.slot_base = c->link_slot_base;
     ev.parent_base = c->link_parent_base;
+    ev.units = c->units;
     const int chunks = event_chunks_per_tile(c);
     const long long n_tiles = (cs.n_chunks + chunks - 1) / chunks;
     tile_scan_kernel<<<1, kScanThreads, 0, c->stream>>>(cs.cnt, cs.n_chunks, chunks, n_tiles, cs.off, c->link_slot_base, d_n_out,
@@ -687,11 +747,11 @@ int picsarqed_schwinger_rate(picsarqed_ctx* c, int dtype, long long n, const voi
     if (dtype == PICSARQED_F64)
         schwinger_kernel<double><<<stream_grid(c, (n + 1) / 2, 256), 256, 0, c->stream>>>(
             (const double*)ex, (const double*)ey, (const double*)ez, (const double*)bx, (const double*)by,
-            (const double*)bz, rate_out, n);
+            (const double*)bz, rate_out, n, c->units);
     else if (dtype == PICSARQED_F32)
         schwinger_kernel<float><<<stream_grid(c, (n + 3) / 4, 256), 256, 0, c->stream>>>(
             (const float*)ex, (const float*)ey, (const float*)ez, (const float*)bx, (const float*)by, (const float*)bz,
-            rate_out, n);
+            rate_out, n, c->units);
     else
         return fail(c, PICSARQED_ERR_DTYPE, "bad dtype");
     PXQ_CUDA(c, cudaGetLastError());
@@ -997,6 +1057,8 @@ extern "C" int picsarqed_build_tables(picsarqed_ctx* c, const picsarqed_table_pa
 extern "C" int picsarqed_boris_push_uniform(picsarqed_ctx* c, int dtype, long long n, void* px, void* py, void* pz,
                                             int charge_sign, const double* e, const double* b, double dt) {
     if (!c) return PICSARQED_ERR_INVALID;
+    if (c->unit_system != PICSARQED_UNITS_LIBRARY)
+        return fail(c, PICSARQED_ERR_INVALID, "the closed-loop calls take the library's own units");
     if (n < 0 || (charge_sign != 1 && charge_sign != -1) || !e || !b)
         return fail(c, PICSARQED_ERR_INVALID, "bad n, charge_sign, e or b");
     if (dtype != PICSARQED_F64 && dtype != PICSARQED_F32) return fail(c, PICSARQED_ERR_DTYPE, "bad dtype");
@@ -1046,6 +1108,8 @@ extern "C" int picsarqed_energy_spectrum(picsarqed_ctx* c, int species, int dtyp
                                          const void* py, const void* pz, double e_min, double e_max, int nbins,
                                          unsigned long long* hist) {
     if (!c) return PICSARQED_ERR_INVALID;
+    if (c->unit_system != PICSARQED_UNITS_LIBRARY)
+        return fail(c, PICSARQED_ERR_INVALID, "the closed-loop calls take the library's own units");
     if (n < 0 || (species != 0 && species != 1) || !(e_min > 0.0) || !(e_max > e_min) || nbins < 1 ||
         nbins > kSpectrumMaxBins || !hist)
         return fail(c, PICSARQED_ERR_INVALID, "bad n, species, energy range, nbins or hist");
@@ -1075,6 +1139,8 @@ extern "C" int picsarqed_cascade_step(picsarqed_ctx* c, int dtype, int tau_dtype
                                       const double* b, double dt, unsigned long long seed, unsigned long long step,
                                       double photon_min_energy, int push, unsigned long long* h_events) {
     if (!c) return PICSARQED_ERR_INVALID;
+    if (c->unit_system != PICSARQED_UNITS_LIBRARY)
+        return fail(c, PICSARQED_ERR_INVALID, "the closed-loop calls take the library's own units");
     if (!el || !po || !ph || !e || !b || !(photon_min_energy >= 0.0))
         return fail(c, PICSARQED_ERR_INVALID, "null species, e or b, or bad photon_min_energy");
     if ((dtype != 0 && dtype != 1) || (tau_dtype != 0 && tau_dtype != 1) || (dtype == 1 && tau_dtype == 0))

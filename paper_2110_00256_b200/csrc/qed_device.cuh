@@ -22,6 +22,14 @@ constexpr double kPlanck = 6.62607015e-34;          // J s
 constexpr double kAlphaOverTauC =
     kFineStructure * kElectronMass * kLightSpeed * kLightSpeed / (kPlanck / (2.0 * kPi));  // 5.6652563985e18
 
+// ---- unit system of the caller's arrays ---------------------------------
+// Multipliers that take the caller's momenta, electric and magnetic fields to the library's units (p/(m_e c), E/E_s,
+// cB/E_s), applied in registers where the arrays are loaded; inv_p takes momenta back where they are stored.
+// All 1 for the library's own units: x * 1.0 is exact, results are bit-identical to unscaled code.
+struct UnitScales {
+    double p = 1.0, e = 1.0, b = 1.0, inv_p = 1.0;
+};
+
 // ---- table views: plain structs passed by value to the kernels ----
 template <typename R>
 struct Table1D {      // ln G or ln T on a log-spaced chi grid
