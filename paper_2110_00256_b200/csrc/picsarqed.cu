@@ -554,7 +554,7 @@ int chunk_scratch(picsarqed_ctx* c, long long n, ChunkScratch* out) {
 
 // chunks per tile of the configured event_kernel shape
 int event_chunks_per_tile(const picsarqed_ctx* c) {
-    static const int kChunksOf[8] = {24, 32, 24, 16, 12, 24, 24, 32};  // must match the switch in launch_event_pass
+    static const int kChunksOf[8] = {32, 32, 24, 16, 12, 24, 24, 24};  // must match the switch in launch_event_pass
     return kChunksOf[c->event_config];
 }
 
@@ -606,8 +606,8 @@ int launch_event_pass(picsarqed_ctx* c, long long n, const ChunkScratch& cs, voi
         case 4: PXQ_LAUNCH_EVENTS(128, 12, 8); break;
         case 5: PXQ_LAUNCH_EVENTS(256, 24, 5); break;
         case 6: PXQ_LAUNCH_EVENTS(256, 24, 6); break;
-        case 7: PXQ_LAUNCH_EVENTS(384, 32, 2); break;
-        default: PXQ_LAUNCH_EVENTS(256, 24, 3); break;
+        case 7: PXQ_LAUNCH_EVENTS(256, 24, 3); break;
+        default: PXQ_LAUNCH_EVENTS(384, 32, 2); break;  // measured best on B200 (config 2: 1-4 us ahead of (256, 24, 3))
     }
 #undef PXQ_LAUNCH_EVENTS
     PXQ_CUDA(c, cudaGetLastError());
