@@ -48,6 +48,9 @@ def parse():
                     help="secondary workload (SURVEY.md 8(f)-1): closed loop of Ridgers case (iii) instead of the "
                          "headline step; prints its own JSON line")
     ap.add_argument("--cascade-dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--tables", action="store_true",
+                    help="secondary workload (BASELINE config 4): build the 4096-point 1D tables and the 4096x2048 2D "
+                         "tables on the GPU; prints its own JSON line")
     return ap.parse_args()
 
 
@@ -371,10 +374,37 @@ def run_cascade(args):
                                              "threshold 2 m_e c^2", "initial_electrons": n0, "final": final}}), flush=True)
 
 
+def run_tables(args):
+    """BASELINE config 4: picsarqed_build_tables on 4096 log-spaced chi points over [1e-4, 1e3], 2048 xi columns,
+    both processes (the 2D tables carry all 4096 rows: DESIGN.md 4).  Time per build, median of `steps`."""
+    import torch
+
+    import paper_2110_00256_b200 as q
+    from paper_2110_00256_b200 import workloads as w
+    torch.cuda.set_device(0)
+    ctx = q.Context(0)
+    tp = q.TableParams(**w.table_params(4))
+    times = []
+    for _ in range(max(1, args.warmup) + max(1, min(args.steps, 10))):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ctx.build_tables(tp)                      # synchronises
+        times.append(time.perf_counter() - t0)
+    ms = 1e3 * float(np.median(times[max(1, args.warmup):]))
+    cells = 2 * tp.qs_n_chi * tp.qs_n_xi
+    print(json.dumps({"metric": "table build time (BASELINE config 4)", "value": ms, "unit": "ms", "n_gpus": 1,
+                      "steps": len(times) - max(1, args.warmup), "warmup": max(1, args.warmup), "ms_per_step": ms,
+                      "higher_is_better": False, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": "4096-point lnG, lnT on [1e-4, 1e3]; two 4096 x 2048 CDF tables",
+                                 "cells": cells, "cells_per_s": cells / (ms * 1e-3)}}), flush=True)
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         run_reference(args)
+    elif args.tables:
+        run_tables(args)
     elif args.cascade:
         run_cascade(args)
     else:
