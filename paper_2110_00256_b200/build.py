@@ -9,7 +9,6 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _LIB = os.path.join(_HERE, "libpicsarqed.so")
 _SOURCES = ["picsarqed.cu"]
-_HEADERS = ["qed_device.cuh", "evolve.cuh", "events.cuh", "tables.cuh"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
@@ -23,7 +22,8 @@ def _stale() -> bool:
     if not os.path.exists(_LIB):
         return True
     t = os.path.getmtime(_LIB)
-    deps = [os.path.join(_CSRC, f) for f in _SOURCES + _HEADERS]
+    # every file under csrc/ is a dependency (picsarqed.cu includes all the .cuh headers)
+    deps = [os.path.join(_CSRC, f) for f in os.listdir(_CSRC) if f.endswith((".cu", ".cuh", ".h"))]
     deps.append(os.path.join(os.path.dirname(_HERE), "include", "picsarqed.h"))
     return any(os.path.getmtime(d) > t for d in deps)
 

@@ -336,6 +336,101 @@ def test_inverse_cdf_closed_form_tables(orc):
         assert orc.bw_sample_xi(t, 3.0, r) == pytest.approx(r, abs=1e-15)
 
 
+def _row_dependent_tables(orc):
+    """closed-form CDF tables whose rows DEPEND on chi: QS ln P[n][m] = a_n ln xi_m and BW P[n][m] = (2 xi_m)^2 (c_n +
+    (1/2 - c_n) (2 xi_m)), with a_n and c_n linear in ln chi_n.  Interpolating the rows linearly in ln chi (PAPER.md:214
+    eq.24, :257 eq.28) then gives exactly a(chi) ln xi and the same polynomial with c(chi), at any chi between rows."""
+    p = orc.TableParams(qs_chi_min=1e-2, qs_chi_max=1e2, qs_n_chi=5, qs_xi_min=1e-6, qs_n_xi=13,
+                        bw_chi_min=1e-1, bw_chi_max=1e3, bw_n_chi=5, bw_n_xi=9)
+    lq = np.linspace(math.log(p.qs_chi_min), math.log(p.qs_chi_max), p.qs_n_chi)
+    lb = np.linspace(math.log(p.bw_chi_min), math.log(p.bw_chi_max), p.bw_n_chi)
+    a_of = lambda lc: 0.25 + 0.05 * (lc - lq[0])           # 0.25 .. 0.71 over the table
+    c_of = lambda lc: 0.05 + 0.04 * (lc - lb[0])           # 0.05 .. 0.42
+    lxi = math.log(p.qs_xi_min) * (1 - np.arange(p.qs_n_xi) / (p.qs_n_xi - 1))
+    qs = np.outer(a_of(lq), lxi)
+    u = 2 * (0.5 * np.arange(p.bw_n_xi) / (p.bw_n_xi - 1))
+    bw = np.array([u * u * (c + (0.5 - c) * u) for c in c_of(lb)])
+    return orc.Tables(p, np.zeros(p.qs_n_chi), qs, np.zeros(p.bw_n_chi), bw), a_of, c_of
+
+
+def test_row_interpolation_weight_is_linear_in_ln_chi(orc):
+    """the weight of eq.24 / eq.28 between rows n and n+1 is (ln chi - ln chi_n)/(ln chi_{n+1} - ln chi_n)
+    (PAPER.md:214, :257): a weight linear in chi itself gives another row and fails these closed forms"""
+    t, a_of, c_of = _row_dependent_tables(orc)
+    # QS: interpolated row = a(chi) ln xi  =>  eq.30 (log-log, exact for a power law) gives xi = r^{1/a(chi)}
+    for chi in (0.013, 0.3, 1.0, 2.7, 31.0, 88.0):           # strictly between rows (rows at 1e-2, 1e-1, 1, 10, 100)
+        a = a_of(math.log(chi))
+        for r in (0.05, 0.4, 0.93):
+            if r > 1e-6 ** a:                                 # above the first column
+                assert orc.qs_sample_xi(t, chi, r) == pytest.approx(r ** (1 / a), rel=1e-12)
+    # the mid-point in ln chi between two rows, against the mid-point in chi (which must NOT be what is used)
+    lo, hi = 1.0, 10.0
+    chi_geo, a_geo = math.sqrt(lo * hi), 0.5 * (a_of(math.log(lo)) + a_of(math.log(hi)))
+    assert orc.qs_sample_xi(t, chi_geo, 0.4) == pytest.approx(0.4 ** (1 / a_geo), rel=1e-12)
+    assert orc.qs_sample_xi(t, 0.5 * (lo + hi), 0.4) != pytest.approx(0.4 ** (1 / a_geo), rel=1e-3)
+    # BW: interpolated row = u^2 (c + (1/2 - c) u), u = 2 xi, c = c(chi) linear in ln chi; eq.26 interpolates linearly
+    # between columns, so compare at the table's own columns where that is exact: r' = P(xi_m) -> xi_m
+    for chi in (0.17, 3.3, 40.0, 700.0):
+        c = c_of(math.log(chi))
+        for m in (2, 5, 7):
+            xi_m = 0.5 * m / 8
+            u = 2 * xi_m
+            assert orc.bw_sample_xi(t, chi, u * u * (c + (0.5 - c) * u)) == pytest.approx(xi_m, abs=1e-13)
+        # and inside a cell: the linear inverse of the two bracketing columns of THAT interpolated row
+        u0, u1 = 2 * 0.5 * 4 / 8, 2 * 0.5 * 5 / 8
+        P0, P1 = u0 * u0 * (c + (0.5 - c) * u0), u1 * u1 * (c + (0.5 - c) * u1)
+        rp = 0.3 * P0 + 0.7 * P1
+        assert orc.bw_sample_xi(t, chi, rp) == pytest.approx(0.5 * (4 + 0.7) / 8, abs=1e-13)
+
+
+def test_row_interpolation_between_rows_of_a_built_table(orc):
+    """at chi strictly between two closely spaced rows of an oracle-built table, the sampled xi has the exact CDF
+    value r (eq.11 / eq.18 by quadrature at THAT chi) up to the interpolation error of the table"""
+    p = orc.TableParams(qs_chi_min=0.8, qs_chi_max=1.25, qs_n_chi=3, qs_xi_min=1e-12, qs_n_xi=193,
+                        bw_chi_min=0.8, bw_chi_max=1.25, bw_n_chi=3, bw_n_xi=129)
+    t = orc.build_tables(p)
+    for chi in (0.9, 1.1):                                     # rows at 0.8, 1.0, 1.25
+        for r in (0.1, 0.5, 0.9):
+            assert orc.qs_cdf(chi, orc.qs_sample_xi(t, chi, r)) == pytest.approx(r, rel=2e-3)
+        for r in (0.1, 0.3, 0.5):
+            assert orc.bw_cdf(chi, orc.bw_sample_xi(t, chi, r)) == pytest.approx(r, rel=2e-3)
+
+
+def _stream_uniform(orc, seed, pid, step, purpose, species, pair):
+    """the documented stream, typed out here: key = (seed_lo, seed_hi),
+    counter = (id_lo, id_hi, step_lo, purpose | species << 8 | step_hi16 << 16); words (2 pair, 2 pair + 1) -> the top
+    52 bits + 1/2, times 2^-52.  Only the block function comes from the oracle (pinned by the published vectors)."""
+    ctr = (pid & 0xFFFFFFFF, pid >> 32, step & 0xFFFFFFFF, purpose | (species << 8) | (((step >> 32) & 0xFFFF) << 16))
+    w = orc.philox4x32_10(ctr, (seed & 0xFFFFFFFF, seed >> 32))
+    k = ((w[2 * pair] << 32) | w[2 * pair + 1]) >> 12
+    return (k + 0.5) * 2.0 ** -52
+
+
+def test_children_and_parent_streams(orc, small_tables):
+    """purpose 1 words (2,3): the parent's new optical depth; purpose 2 words (0,1): photon / electron, words (2,3):
+    positron -- so the two members of a pair are born with DIFFERENT optical depths"""
+    rng = np.random.default_rng(11)
+    n, seed, step, base = 400, 77, (3 << 32) | 5, 1 << 40
+    ids = base + np.arange(n, dtype=np.uint64)
+    tau = np.where(rng.random(n) < 0.5, -rng.random(n), rng.random(n) + 0.1)
+    p, e, b, _ = _population(rng, n, LEPTON)
+    o = orc.generate_photons(small_tables, F64, F64, p, e, b, tau, seed, step, ids=ids)
+    for slot, i in enumerate(o["parent"]):
+        pid = base + int(i)
+        assert o["tau"][i] == pytest.approx(-math.log(_stream_uniform(orc, seed, pid, step, 1, LEPTON, 1)), rel=1e-15)
+        assert o["ph_tau"][slot] == pytest.approx(-math.log(_stream_uniform(orc, seed, pid, step, 2, LEPTON, 0)), rel=1e-15)
+    p, e, b, _ = _population(rng, n, PHOTON)
+    o = orc.generate_pairs(small_tables, F64, F64, p, e, b, tau, seed, step, ids=ids)
+    assert o["n_fired"] > 100
+    for slot, i in enumerate(o["parent"]):
+        pid = base + int(i)
+        assert o["el_tau"][slot] == pytest.approx(-math.log(_stream_uniform(orc, seed, pid, step, 2, PHOTON, 0)), rel=1e-15)
+        assert o["po_tau"][slot] == pytest.approx(-math.log(_stream_uniform(orc, seed, pid, step, 2, PHOTON, 1)), rel=1e-15)
+    assert np.all(o["el_tau"] != o["po_tau"])
+    # and the oracle's own orc_uniform helper follows the same layout (it is what the GPU tests call)
+    assert orc.uniform(seed, base + 9, step, 2, PHOTON, 1, F64) == _stream_uniform(orc, seed, base + 9, step, 2, PHOTON, 1)
+
+
 # ----------------------------------------------------------------------------- Schwinger rate (SURVEY.md 8(f)-3)
 def test_schwinger_rate_closed_forms(orc):
     """PAPER.md:171-183 eqs.19-22: prefactor from CODATA, pure-E textbook limit, E parallel B, null fields"""
