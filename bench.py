@@ -44,6 +44,8 @@ def parse():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-sample", type=int, default=1 << 23, help="particles in the oracle timing sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
+                    help="picsarqed_set_option before the run (tuning experiments), e.g. --opt fused_step=0")
     ap.add_argument("--cascade", action="store_true",
                     help="secondary workload (SURVEY.md 8(f)-1): closed loop of Ridgers case (iii) instead of the "
                          "headline step; prints its own JSON line")
@@ -186,6 +188,9 @@ def run_ours(args):
     cap = n // 8
 
     ctx = q.Context(local)
+    for kv in args.opt:
+        name, value = kv.split("=")
+        ctx.set_option(name, int(value))
     tp_kwargs = w.table_params(2)
     t0 = time.perf_counter()
     ctx.build_tables(q.TableParams(**tp_kwargs))

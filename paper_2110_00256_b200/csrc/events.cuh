@@ -37,7 +37,9 @@ struct EventArgs {
     TR* out_tau[2];   // QS: photon tau.            BW: electron, positron tau
     long long* parent;
     // per 128-particle chunk (context scratch, see evolve.cuh):
-    const unsigned char* stage_rec;           // staged records (unused for chunks flagged kStageNoRecords)
+    const unsigned char* stage_rec;           // staged records (unused for chunks flagged kStageNoRecords), or, for
+                                              // chunks flagged kStageDone, staged StepResult records (fused step)
+    long long stage_stride;                   // bytes from one chunk's segment to the next
     const unsigned short* stage_cnt;          // count | flags
     const unsigned long long* tile_offset;    // [n_tiles] number of events before the tile
     // a call that handles the slab [parent_base, parent_base + n) of a longer array (step_host): its events
@@ -60,20 +62,21 @@ struct EventOut {
 template <typename R, typename TR>
 __device__ __forceinline__ EventOut<R, TR> qs_event_compute(const EventArgs<R, TR>& a, long long i, double px, double py,
                                                             double pz, double c2) {
+    // (lean fp64 routines of qed_device.cuh: every argument here is a positive normal number or handled apart)
     const double p2 = fma(px, px, fma(py, py, pz * pz));
-    const double g = sqrt(1.0 + p2);
+    const double g = (1.0 + p2) * rsqrt_fast(1.0 + p2);
     const unsigned long long id = a.id_base + (unsigned long long)i;
     const Words4 w = qed_words(a.seed, id, a.step, 1, 0);
     const Words4 wc = qed_words(a.seed, id, a.step, 2, 0);
     const double r = (double)uniform_open<R>(w.w[0], w.w[1]);
-    const double xi = qs_sample_xi(a.cdf, 0.5 * log(c2), r);
-    const double pn = sqrt(p2);
-    const double inv_pn = pn > 0.0 ? 1.0 / pn : 0.0;
+    const double xi = qs_sample_xi(a.cdf, 0.5 * log_pos(c2), r);
+    const double inv_pn = p2 > 1e-300 ? rsqrt_fast(p2) : 0.0;
     const double nx = px * inv_pn, ny = py * inv_pn, nz = pz * inv_pn;
-    const double km1 = p2 / (g + 1.0);          // gamma - 1 without cancellation
+    const double km1 = p2 * rcp_fast(g + 1.0);  // gamma - 1 without cancellation
     const double gph = km1 * xi;                // gamma_gamma = (gamma-1) xi
     const double k2 = km1 * (1.0 - xi);         // emitter kinetic energy after the emission
-    const double pn2 = sqrt(k2 * (k2 + 2.0));   // sqrt(gamma'^2 - 1)
+    const double q2 = k2 * (k2 + 2.0);
+    const double pn2 = q2 > 1e-300 ? q2 * rsqrt_fast(q2) : 0.0;   // sqrt(gamma'^2 - 1)
     EventOut<R, TR> o;
     const double ip = a.units.inv_p;
     o.sec[0] = (R)(gph * nx * ip);              // emitted along p
@@ -94,19 +97,20 @@ template <typename R, typename TR>
 __device__ __forceinline__ EventOut<R, TR> bw_event_compute(const EventArgs<R, TR>& a, long long i, double px, double py,
                                                             double pz, double c2) {
     const double p2 = fma(px, px, fma(py, py, pz * pz));
-    const double g = sqrt(p2);                  // gamma_gamma = |p|
+    const double inv_g = p2 > 1e-300 ? rsqrt_fast(p2) : 0.0;
+    const double g = p2 * inv_g;                // gamma_gamma = |p|
     const unsigned long long id = a.id_base + (unsigned long long)i;
     const Words4 w = qed_words(a.seed, id, a.step, 1, 1);
     const Words4 wc = qed_words(a.seed, id, a.step, 2, 1);
     const double r = (double)uniform_open<R>(w.w[0], w.w[1]);
     const bool electron_side = r <= 0.5;        // PAPER.md:212 "If r <= 0.5"
     const double rp = electron_side ? r : 1.0 - r;
-    const double xi = bw_sample_xi(a.cdf, 0.5 * log(c2), rp);
+    const double xi = bw_sample_xi(a.cdf, 0.5 * log_pos(c2), rp);
     const double xe = electron_side ? xi : 1.0 - xi;   // chi_-/chi_gamma
     const double xp = electron_side ? 1.0 - xi : xi;   // chi_+/chi_gamma (eq.6)
     const double ke = (g - 2.0) * xe, kp = (g - 2.0) * xp;  // K = (gamma_gamma-2) chi_pm/chi_gamma
-    const double pe = sqrt(ke * (ke + 2.0)), pp = sqrt(kp * (kp + 2.0));
-    const double inv_g = g > 0.0 ? 1.0 / g : 0.0;
+    const double qe = ke * (ke + 2.0), qp = kp * (kp + 2.0);
+    const double pe = qe > 1e-300 ? qe * rsqrt_fast(qe) : 0.0, pp = qp > 1e-300 ? qp * rsqrt_fast(qp) : 0.0;
     const double nx = px * inv_g, ny = py * inv_g, nz = pz * inv_g;
     EventOut<R, TR> o;
     const double ip = a.units.inv_p;
@@ -305,6 +309,7 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
     if (total == 0) continue;
     const unsigned int rescan_mask =
         __ballot_sync(0xffffffffu, cnt > 0 && (cnt > (unsigned)kStageCap || (flags & kStageNoRecords) != 0));
+    const unsigned int done_mask = __ballot_sync(0xffffffffu, cnt > 0 && (flags & kStageDone) != 0);
     if (rescan_mask) {  // chunks without records: find their fired particles again (tau < 0), in index order
         __syncthreads();  // (every warp is done with the list of the previous tile that needed one)
         for (int j = warp; j < CHUNKS; j += WARPS) {
@@ -335,15 +340,37 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
         }
         const unsigned int off_j = __shfl_sync(0xffffffffu, off_lane, j);
         const long long slot = (long long)(slot_base + excl + e);
-        if (e >= total || slot >= a.capacity) continue;  // capacity rule (R16): later parents untouched
+        if (e >= total) continue;
         const unsigned int r = e - off_j;
         const long long cbase = (first_chunk + j) * kChunk;
+        if ((done_mask >> j) & 1u) {
+            // the fused step generated this event already and rewrote its parent: move the secondaries to their slot
+            typedef StepResult<R, TR, KIND> Res;
+            const uint4* src = reinterpret_cast<const uint4*>(a.stage_rec + (first_chunk + j) * a.stage_stride + r * sizeof(Res));
+            union { uint4 raw[sizeof(Res) / 16]; Res res; } u;
+#pragma unroll
+            for (int k = 0; k < (int)(sizeof(Res) / 16); ++k) u.raw[k] = __ldcs(src + k);
+            const long long i = cbase + u.res.idx;
+            if (slot < a.capacity) {
+#pragma unroll
+                for (int c = 0; c < (KIND == 0 ? 3 : 6); ++c) a.out_p[c][slot] = u.res.sec[c];
+                a.out_tau[0][slot] = u.res.sec_tau[0];
+                if (KIND == 1) a.out_tau[1][slot] = u.res.sec_tau[KIND == 1 ? 1 : 0];
+                if (a.parent) a.parent[slot] = a.parent_base + i;
+            } else {   // capacity rule (R16): parents beyond the capacity are left as the evolve pass left them
+#pragma unroll
+                for (int c = 0; c < 3; ++c) a.p[c][i] = u.res.old_p[c];
+                a.tau[i] = u.res.tau_ev;
+            }
+            continue;
+        }
+        if (slot >= a.capacity) continue;  // capacity rule (R16): later parents untouched
         const bool staged = !((rescan_mask >> j) & 1u);
         double px, py, pz, c2;
         long long i;
         if (staged) {
             const uint4* src = reinterpret_cast<const uint4*>(
-                a.stage_rec + ((first_chunk + j) * (long long)kStageCap + r) * StageRecord<R>::kBytes);
+                a.stage_rec + (first_chunk + j) * a.stage_stride + r * StageRecord<R>::kBytes);
             union { uint4 raw[StageRecord<R>::kVecs]; StageRecord<R> rec; } u;
 #pragma unroll
             for (int k = 0; k < StageRecord<R>::kVecs; ++k) u.raw[k] = __ldg(src + k);

@@ -28,7 +28,8 @@ struct EvolveArgs {
     unsigned long long* d_n_events;
     int table_in_smem;
     // record emission (EMIT kernels only): every 128-particle chunk owns a segment of kStageCap records
-    unsigned char* stage_rec;   // [n_chunks][kStageCap] records (see StageRecord), in index order
+    unsigned char* stage_rec;   // [n_chunks] segments of kStageCap records (see StageRecord), in index order
+    long long stage_stride;     // bytes from one chunk's segment to the next
     unsigned short* stage_cnt;  // [n_chunks]: fired particles of the chunk | flags (see kStage* below)
     unsigned table_bytes;       // dynamic shared memory: [table, padded to 128 B][per-warp record buffers]
     // EMIT: every chunk count is also added to the sum of its event tile (one RED per warp and tile), so that the
@@ -42,8 +43,11 @@ constexpr int kChunk = 128;                 // particles one warp handles per ti
 constexpr int kStageCap = 24;               // records per chunk segment (mean at 5 % firing: 6.4)
 // stage_cnt[chunk]: bits 0..14 = number of particles of the chunk that fired; bit 15 = the chunk has no staged
 // records (segment overflow, or counted by count_chunks_kernel: generate_* calls and the ragged last tile)
-constexpr unsigned short kStageCountMask = 0x7FFFu;
+// bit 14 = the events of the chunk have been generated already (fused step, step.cuh): its segment holds StepResult
+// records -- the secondaries, waiting for their slots
+constexpr unsigned short kStageCountMask = 0x3FFFu;
 constexpr unsigned short kStageNoRecords = 0x8000u;
+constexpr unsigned short kStageDone = 0x4000u;
 
 // one staged record: what event generation needs of a particle that fired -- its momentum, chi^2 (computed by the
 // evolve pass anyway) and its index inside the chunk.  Sizes are multiples of 16 bytes so that records move as
@@ -61,6 +65,20 @@ template <> struct alignas(16) StageRecord<float> {
     static constexpr int kBytes = 32, kVecs = 2;
 };
 static_assert(sizeof(StageRecord<double>) == 48 && sizeof(StageRecord<float>) == 32, "record layout");
+
+// one staged result of the fused step (step.cuh): the secondaries of an event whose parent has been rewritten already,
+// plus what undoes that rewrite if the event falls beyond the capacity of the output (R16): the parent's old
+// momentum, its evolved optical depth and its index in the chunk.  KIND 0: one photon; KIND 1: electron and positron.
+template <typename R, typename TR, int KIND> struct alignas(16) StepResult {
+    TR sec_tau[KIND == 0 ? 1 : 2];
+    TR tau_ev;
+    R sec[KIND == 0 ? 3 : 6];
+    R old_p[3];
+    unsigned idx;
+};
+static_assert(sizeof(StepResult<double, double, 0>) == 80 && sizeof(StepResult<float, double, 0>) == 48 &&
+              sizeof(StepResult<float, float, 0>) == 48 && sizeof(StepResult<double, double, 1>) == 112 &&
+              sizeof(StepResult<float, double, 1>) == 64 && sizeof(StepResult<float, float, 1>) == 64, "result layout");
 
 // ---- TMA bulk copy of a 1D table into shared memory ------------------------------------
 __device__ __forceinline__ void stage_table_tma(void* smem_dst, const void* gmem_src, unsigned bytes,
@@ -96,19 +114,11 @@ __host__ __device__ constexpr double hankel13(int k) {
     return a;
 }
 
-// Returns the decrement dN/dt * dt in the particle arithmetic type A (float or double).
-// SCALED: the arrays are in another unit system (picsarqed_set_units): nine multiplications in registers.
-template <typename R, int SPECIES, bool SCALED = false>
-__device__ __forceinline__ auto decrement_one(R pxr, R pyr, R pzr, R exr, R eyr, R ezr, R bxr, R byr, R bzr,
-                                              const R* tab, const Table1D<R>& T, double rate_dt,
-                                              const UnitScales& us, double* c2_out = nullptr) -> R {
+// The decrement dN/dt * dt from chi^2 (all cases, one particle), in the particle arithmetic type A = R.
+template <typename R, int SPECIES>
+__device__ __forceinline__ R rate_from_c2(double c2, double inv_g, double g2, const R* tab, const Table1D<R>& T,
+                                          double rate_dt) {
     typedef R A;
-    double inv_g, g2;
-    const double c2 =
-        SCALED ? chi_squared_of<SPECIES>(pxr * us.p, pyr * us.p, pzr * us.p, exr * us.e, eyr * us.e, ezr * us.e,
-                                         bxr * us.b, byr * us.b, bzr * us.b, &inv_g, &g2)
-               : chi_squared_of<SPECIES>(pxr, pyr, pzr, exr, eyr, ezr, bxr, byr, bzr, &inv_g, &g2);
-    if (c2_out) *c2_out = c2;
     A lc;
     if constexpr (sizeof(R) == 8) lc = 0.5 * log_pos(c2); else lc = 0.5f * logf((float)c2);
     const A ln_min = (A)T.ln_min, ln_max = (A)T.ln_max, inv_delta = (A)T.inv_delta;
@@ -173,6 +183,74 @@ __device__ __forceinline__ auto decrement_one(R pxr, R pyr, R pzr, R exr, R eyr,
     }
 }
 
+// Returns the decrement dN/dt * dt in the particle arithmetic type (float or double).
+// SCALED: the arrays are in another unit system (picsarqed_set_units): nine multiplications in registers.
+template <typename R, int SPECIES, bool SCALED = false>
+__device__ __forceinline__ auto decrement_one(R pxr, R pyr, R pzr, R exr, R eyr, R ezr, R bxr, R byr, R bzr,
+                                              const R* tab, const Table1D<R>& T, double rate_dt,
+                                              const UnitScales& us, double* c2_out = nullptr) -> R {
+    double inv_g, g2;
+    const double c2 =
+        SCALED ? chi_squared_of<SPECIES>(pxr * us.p, pyr * us.p, pzr * us.p, exr * us.e, eyr * us.e, ezr * us.e,
+                                         bxr * us.b, byr * us.b, bzr * us.b, &inv_g, &g2)
+               : chi_squared_of<SPECIES>(pxr, pyr, pzr, exr, eyr, ezr, bxr, byr, bzr, &inv_g, &g2);
+    if (c2_out) *c2_out = c2;
+    return rate_from_c2<R, SPECIES>(c2, inv_g, g2, tab, T, rate_dt);
+}
+
+// The same for the V particles a thread holds in one 128-bit vector per array: identical arithmetic, but the common path
+// (leptons; photons inside the T table) is written stage by stage over the V particles, so that it is one straight line
+// the compiler can interleave, with the logarithm and the exponential in their V-at-once forms (qed_device.cuh).
+// in[c][v]: component c (px, py, pz, ex, ey, ez, bx, by, bz) of particle v.
+template <typename R, int SPECIES, bool SCALED, int V>
+__device__ __forceinline__ void decrement_vec(const R (&in)[9][V], const R* tab, const Table1D<R>& T, double rate_dt,
+                                              const UnitScales& us, R (&d)[V], double (&c2)[V]) {
+    double inv_g[V], g2[V];
+#pragma unroll
+    for (int v = 0; v < V; ++v)
+        c2[v] = SCALED ? chi_squared_of<SPECIES>(in[0][v] * us.p, in[1][v] * us.p, in[2][v] * us.p, in[3][v] * us.e,
+                                                 in[4][v] * us.e, in[5][v] * us.e, in[6][v] * us.b, in[7][v] * us.b,
+                                                 in[8][v] * us.b, &inv_g[v], &g2[v])
+                       : chi_squared_of<SPECIES>(in[0][v], in[1][v], in[2][v], in[3][v], in[4][v], in[5][v], in[6][v],
+                                                 in[7][v], in[8][v], &inv_g[v], &g2[v]);
+    if constexpr (SPECIES == 1) {
+        // photons that cannot decay or lie outside the T table (Erber form): the general routine, one by one
+        bool plain = true;
+        const double lo2 = T.chi_min * T.chi_min, hi2 = T.chi_max * T.chi_max;
+#pragma unroll
+        for (int v = 0; v < V; ++v) plain = plain && g2[v] > 4.0 && c2[v] >= lo2 && c2[v] <= hi2;
+        if (!plain) {
+#pragma unroll
+            for (int v = 0; v < V; ++v) d[v] = rate_from_c2<R, SPECIES>(c2[v], inv_g[v], g2[v], tab, T, rate_dt);
+            return;
+        }
+    }
+    if constexpr (sizeof(R) == 8) {
+        double lc[V], L[V], ex[V];
+        log_pos_v<V>(c2, lc);
+        const double ln_min = T.ln_min, ln_max = T.ln_max, inv_delta = T.inv_delta;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            lc[v] = 0.5 * lc[v];
+            lc[v] = lc[v] < ln_min ? ln_min : (lc[v] > ln_max ? ln_max : lc[v]);
+            L[v] = lookup_ln<R, double>(tab, T.n, lc[v], ln_min, inv_delta);
+            if (SPECIES == 1) L[v] = L[v] + lc[v];                                  // eq.8: chi T
+        }
+        exp_fast_v<V>(L, ex);
+#pragma unroll
+        for (int v = 0; v < V; ++v) d[v] = rate_dt * ex[v] * inv_g[v];
+    } else {
+        const float ln_min = (float)T.ln_min, ln_max = (float)T.ln_max, inv_delta = (float)T.inv_delta;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            float lc = 0.5f * logf((float)c2[v]);
+            lc = lc < ln_min ? ln_min : (lc > ln_max ? ln_max : lc);
+            const float L = lookup_ln<R, float>(tab, T.n, lc, ln_min, inv_delta);
+            d[v] = (float)rate_dt * expf(SPECIES == 1 ? L + lc : L) * (float)inv_g[v];
+        }
+    }
+}
+
 // ---- fused evolve kernel ------------------------------------------------------------
 // V = particles per 128-bit load of R; U = independent vectors per thread per tile.  A warp owns U*32*V
 // contiguous particles of the tile (every load instruction still covers 512 contiguous bytes).
@@ -221,19 +299,26 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                 t[u] = ld_stream_rw<TR, V>(a.tau + i, pol_stream);
             }
             unsigned int fired_bits = 0;
-            double c2s[EMIT ? U * V : 1];
+            double c2s[U * V];
+            {
+                // all U*V particles of the thread at once (decrement_vec interleaves their dependent chains)
+                R in[9][U * V], d[U * V];
 #pragma unroll
-            for (int u = 0; u < U; ++u) {
+                for (int c = 0; c < 9; ++c)
 #pragma unroll
-                for (int v = 0; v < V; ++v) {
-                    const R d = decrement_one<R, SPECIES, SCALED>(q[0][u].v[v], q[1][u].v[v], q[2][u].v[v], q[3][u].v[v],
-                                                          q[4][u].v[v], q[5][u].v[v], q[6][u].v[v], q[7][u].v[v],
-                                                          q[8][u].v[v], tab, a.tab, a.rate_dt, a.units,
-                                                          EMIT ? &c2s[EMIT ? u * V + v : 0] : nullptr);
-                    const TR tn = t[u].v[v] - (TR)d;
-                    t[u].v[v] = tn;
-                    fired += tn < (TR)0 ? 1u : 0u;
-                    if (EMIT && tn < (TR)0) fired_bits |= 1u << (u * V + v);
+                    for (int u = 0; u < U; ++u)
+#pragma unroll
+                        for (int v = 0; v < V; ++v) in[c][u * V + v] = q[c][u].v[v];
+                decrement_vec<R, SPECIES, SCALED, U * V>(in, tab, a.tab, a.rate_dt, a.units, d, c2s);
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+#pragma unroll
+                    for (int v = 0; v < V; ++v) {
+                        const TR tn = t[u].v[v] - (TR)d[u * V + v];
+                        t[u].v[v] = tn;
+                        fired += tn < (TR)0 ? 1u : 0u;
+                        if (EMIT && tn < (TR)0) fired_bits |= 1u << (u * V + v);
+                    }
                 }
             }
             if constexpr (EMIT) {
@@ -279,7 +364,7 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                     }
                     __syncwarp();
                     const uint4* src = reinterpret_cast<const uint4*>(wbuf);
-                    uint4* dst = reinterpret_cast<uint4*>(a.stage_rec + chunk * (long long)(kStageCap * StageRecord<R>::kBytes));
+                    uint4* dst = reinterpret_cast<uint4*>(a.stage_rec + chunk * a.stage_stride);
                     const unsigned int nvec = total * StageRecord<R>::kVecs;
                     for (unsigned int k = lane; k < nvec; k += 32) st_policy(dst + k, src[k], pol_keep);
                     __syncwarp();
@@ -288,7 +373,7 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const long long i = base + (long long)warp * WCH + (u * 32 + lane) * V;
-                *reinterpret_cast<Vec<TR, V>*>(a.tau + i) = t[u];
+                st_vec<TR, V>(a.tau + i, t[u]);
             }
         } else {  // ragged last tile: scalar, guarded (qed_step counts its chunks afterwards: count_chunks_kernel)
             for (long long i = base + threadIdx.x; i < a.n; i += kEvolveThreads) {

@@ -15,6 +15,7 @@
 #include "tables.cuh"
 #include "cascade.cuh"
 #include "lookup.cuh"
+#include "step.cuh"
 
 using namespace pxq;
 
@@ -48,6 +49,9 @@ struct picsarqed_ctx {
     double t_scale = 1.0;
     int unit_system = 0;
     int event_config = 0;        // shape of event_kernel: see launch_event_pass
+    int fused_step = 0;          // qed_step: 1 = the warp-specialised fused kernel (step.cuh), 0 = evolve pass + event pass
+    int step_spill = 1;          // fused kernel: 1 = a streaming warp whose queue is full hands the chunk to the record path
+    int step_config = 0;         // fused kernel: see launch_fused_step
     int time_kernels = 0;        // qed_step brackets its evolve pass and its event pass with CUDA events
     std::vector<cudaEvent_t> timing_events;  // triples (start, after evolve, after events), not yet read
     // per-chunk scratch of the event path: staged records, counts, output offsets (see events.cuh)
@@ -321,8 +325,14 @@ int picsarqed_set_option(picsarqed_ctx* c, const char* name, long long value) {
         c->evolve_ctas_per_sm = (int)value;
     else if (!std::strcmp(name, "time_kernels") && (value == 0 || value == 1))
         c->time_kernels = (int)value;
-    else if (!std::strcmp(name, "event_config") && value >= 0 && value <= 7)
+    else if (!std::strcmp(name, "event_config") && value >= 0 && value <= 1)
         c->event_config = (int)value;
+    else if (!std::strcmp(name, "fused_step") && (value == 0 || value == 1))
+        c->fused_step = (int)value;
+    else if (!std::strcmp(name, "step_config") && (value == 0 || value == 1))
+        c->step_config = (int)value;
+    else if (!std::strcmp(name, "step_spill") && (value == 0 || value == 1))
+        c->step_spill = (int)value;
     else if (!std::strcmp(name, "host_slabs") && value >= 0 && value <= kMaxSlabs)
         c->host_slabs = (int)value;
     else
@@ -458,11 +468,11 @@ int launch_chi(picsarqed_ctx* c, long long n, const void* const* a, void* out) {
     return PICSARQED_OK;
 }
 
-struct StageView { unsigned char* rec; unsigned short* cnt; unsigned int* tile_sum; int chunks_per_tile; };
+struct StageView { unsigned char* rec; unsigned short* cnt; unsigned int* tile_sum; int chunks_per_tile; long long stride; };
 
 template <typename R, typename TR, int SPECIES, int U, bool EMIT>
 int launch_evolve_u(picsarqed_ctx* c, long long n, const void* const* a, double dt, void* tau,
-                    unsigned long long* d_n_events, StageView sv = StageView{nullptr, nullptr, nullptr, 1}) {
+                    unsigned long long* d_n_events, StageView sv = StageView{nullptr, nullptr, nullptr, 1, 0}) {
     constexpr int V = 16 / sizeof(R);
     constexpr int TILE = kEvolveThreads * V * U;
     EvolveArgs<R, TR> args;
@@ -480,6 +490,7 @@ int launch_evolve_u(picsarqed_ctx* c, long long n, const void* const* a, double 
     args.ticket = c->ticket;
     args.d_n_events = d_n_events;
     args.stage_rec = sv.rec;
+    args.stage_stride = sv.stride;
     args.stage_cnt = sv.cnt;
     args.tile_sum = sv.tile_sum;
     args.chunks_per_tile = sv.chunks_per_tile;
@@ -515,12 +526,12 @@ int launch_evolve(picsarqed_ctx* c, long long n, const void* const* a, double dt
 }
 
 // per-chunk scratch: [tile sums][records][counts][offsets]
-struct ChunkScratch { unsigned char* rec; unsigned short* cnt; unsigned long long* off; unsigned int* sum; long long n_chunks; };
+struct ChunkScratch { unsigned char* rec; unsigned short* cnt; unsigned long long* off; unsigned int* sum; long long n_chunks; long long stride; };
 
-template <typename R>
-int chunk_scratch(picsarqed_ctx* c, long long n, ChunkScratch* out) {
+// seg_bytes: bytes of one entry of a chunk's segment (a staged record, or a staged result of the fused step; 0 = none)
+int chunk_scratch(picsarqed_ctx* c, long long n, size_t seg_bytes, ChunkScratch* out) {
     const long long nchunks = (n + kChunk - 1) / kChunk;
-    const size_t rec_sz = ((size_t)nchunks * kStageCap * StageRecord<R>::kBytes + 255) & ~(size_t)255;
+    const size_t rec_sz = ((size_t)nchunks * kStageCap * seg_bytes + 255) & ~(size_t)255;
     const size_t cnt_sz = ((size_t)nchunks * sizeof(unsigned short) + 255) & ~(size_t)255;
     // tiles hold at least 8 chunks: n_chunks/8 + 1 tile offsets and tile sums are always enough
     const size_t off_sz = ((size_t)(nchunks / 8 + 2) * sizeof(unsigned long long) + 255) & ~(size_t)255;
@@ -549,13 +560,14 @@ int chunk_scratch(picsarqed_ctx* c, long long n, ChunkScratch* out) {
     out->cnt = reinterpret_cast<unsigned short*>(out->rec + rec_sz);
     out->off = reinterpret_cast<unsigned long long*>(out->rec + rec_sz + cnt_sz);
     out->n_chunks = nchunks;
+    out->stride = (long long)(kStageCap * seg_bytes);
     return PICSARQED_OK;
 }
 
 // chunks per tile of the configured event_kernel shape
 int event_chunks_per_tile(const picsarqed_ctx* c) {
-    static const int kChunksOf[8] = {32, 32, 24, 16, 12, 24, 24, 24};  // must match the switch in launch_event_pass
-    return kChunksOf[c->event_config];
+    (void)c;
+    return 32;  // both shapes of launch_event_pass
 }
 
 // levels 2 and 3 of the compaction: chunk counts (and their tile sums) -> offsets -> events
@@ -581,6 +593,7 @@ int launch_event_pass(picsarqed_ctx* c, long long n, const ChunkScratch& cs, voi
     for (int k = 0; k < 2; ++k) ev.out_tau[k] = (TR*)out_tau[k];
     ev.parent = parent;
     ev.stage_rec = cs.rec;
+    ev.stage_stride = cs.stride;
     ev.stage_cnt = cs.cnt;
     ev.tile_offset = cs.off;
     ev.slot_base = c->link_slot_base;
@@ -601,12 +614,6 @@ int launch_event_pass(picsarqed_ctx* c, long long n, const ChunkScratch& cs, voi
     } while (0)
     switch (c->event_config) {
         case 1: PXQ_LAUNCH_EVENTS(256, 32, 3); break;
-        case 2: PXQ_LAUNCH_EVENTS(256, 24, 4); break;
-        case 3: PXQ_LAUNCH_EVENTS(256, 16, 4); break;
-        case 4: PXQ_LAUNCH_EVENTS(128, 12, 8); break;
-        case 5: PXQ_LAUNCH_EVENTS(256, 24, 5); break;
-        case 6: PXQ_LAUNCH_EVENTS(256, 24, 6); break;
-        case 7: PXQ_LAUNCH_EVENTS(256, 24, 3); break;
         default: PXQ_LAUNCH_EVENTS(384, 32, 2); break;  // measured best on B200 (config 2: 1-4 us ahead of (256, 24, 3))
     }
 #undef PXQ_LAUNCH_EVENTS
@@ -620,7 +627,7 @@ int launch_events(picsarqed_ctx* c, long long n, void* const* p, const void* con
                   unsigned long long seed, unsigned long long step, unsigned long long id_base, long long capacity,
                   void* const* out_p, void* const* out_tau, long long* parent, unsigned long long* d_n_out) {
     ChunkScratch cs;
-    if (int rc = chunk_scratch<R>(c, n, &cs)) return rc;
+    if (int rc = chunk_scratch(c, n, 0, &cs)) return rc;
     const int grid = (int)std::max<long long>(1, std::min<long long>((cs.n_chunks + 7) / 8, (long long)c->num_sms * 8));
     count_chunks_kernel<TR><<<grid, 256, 0, c->stream>>>((const TR*)tau, n, 0, cs.n_chunks, cs.cnt, cs.sum,
                                                          event_chunks_per_tile(c));
@@ -628,15 +635,128 @@ int launch_events(picsarqed_ctx* c, long long n, void* const* p, const void* con
                                           d_n_out);
 }
 
+// qed_step, fused (step.cuh): streaming warps evolve, event warps of the same CTA generate the events and rewrite the
+// parents while their sectors are in L2; then the offsets scan and the placement of the staged secondaries
+template <typename R, typename TR, int SPECIES, int C, int REG_S, int REG_E>
+int launch_fused_step_c(picsarqed_ctx* c, long long n, void* const* p, const void* const* eb, void* tau, double dt,
+                        unsigned long long seed, unsigned long long step, unsigned long long id_base, long long capacity,
+                        void* const* out_p, void* const* out_tau, long long* parent, unsigned long long* d_n_out) {
+    constexpr int SW = 16, NS = 2;
+    typedef StepLayout<R, TR, SW, C, NS> L;
+    constexpr int THREADS = L::THREADS;
+    constexpr long long kTile = (long long)SW * kChunk;
+    typedef StepResult<R, TR, SPECIES> Res;
+    ChunkScratch cs;
+    if (int rc = chunk_scratch(c, n, std::max<size_t>(sizeof(Res), StageRecord<R>::kBytes), &cs)) return rc;
+    StepArgs<R, TR, SPECIES> sa;
+    EvolveArgs<R, TR>& args = sa.ev;
+    for (int k = 0; k < 3; ++k) {
+        args.p[k] = (const R*)p[k];
+        args.e[k] = (const R*)eb[k];
+        args.b[k] = (const R*)eb[3 + k];
+        sa.ge.p[k] = (R*)p[k];
+        sa.ge.e[k] = (const R*)eb[k];
+        sa.ge.b[k] = (const R*)eb[3 + k];
+    }
+    args.tau = (TR*)tau;
+    args.n = n;
+    args.tab = view_1d<R>(c, SPECIES);
+    args.rate_dt = (SPECIES == 0 ? 2.0 / 3.0 : 1.0) * kAlphaOverTauC * (dt * c->t_scale);
+    args.units = c->units;
+    args.partials = nullptr;
+    args.ticket = nullptr;
+    args.d_n_events = nullptr;
+    args.stage_rec = nullptr;
+    args.stage_stride = cs.stride;
+    args.stage_cnt = cs.cnt;
+    args.tile_sum = cs.sum;
+    args.chunks_per_tile = event_chunks_per_tile(c);
+    // shared memory: [1D table][sub-chunk stages][record queues]; a table that does not fit beside them is read through L1
+    constexpr size_t kSmemMax = 227 * 1024 - 2048;   // (2 KB: the kernel's static shared memory)
+    size_t smem = ((size_t)args.tab.n * sizeof(R) + 127) & ~(size_t)127;
+    args.table_in_smem = smem + L::stages_bytes + L::queue_bytes <= kSmemMax;
+    if (!args.table_in_smem) smem = 0;
+    args.table_bytes = (unsigned)smem;
+    smem += L::stages_bytes + L::queue_bytes;
+    sa.ge.tau = (TR*)tau;
+    sa.ge.n = n;
+    sa.ge.cdf = view_2d<R>(c, SPECIES);
+    sa.ge.seed = seed;
+    sa.ge.step = step;
+    sa.ge.id_base = id_base;
+    sa.ge.capacity = capacity;
+    for (int k = 0; k < 6; ++k) sa.ge.out_p[k] = nullptr;
+    for (int k = 0; k < 2; ++k) sa.ge.out_tau[k] = nullptr;
+    sa.ge.parent = nullptr;
+    sa.ge.stage_rec = nullptr;
+    sa.ge.stage_stride = cs.stride;
+    sa.ge.stage_cnt = nullptr;
+    sa.ge.tile_offset = nullptr;
+    sa.ge.slot_base = nullptr;
+    sa.ge.parent_base = 0;
+    sa.ge.units = c->units;
+    sa.stage_res = cs.rec;
+    sa.spill = c->step_spill;
+    const bool scaled = c->unit_system != PICSARQED_UNITS_LIBRARY;
+    // registers (REG_S, REG_E != 0): the launch gives every thread floor(64 Ki / THREADS) rounded down to a multiple of 8
+    // (72 for 896 threads); the streaming warps hand some back and the event warps take them
+    void (*kern)(StepArgs<R, TR, SPECIES>) =
+        scaled ? step_kernel<R, TR, SPECIES, true, SW, C, NS, REG_S, REG_E> : step_kernel<R, TR, SPECIES, false, SW, C, NS, REG_S, REG_E>;
+    if (REG_S != 0) {
+        cudaFuncAttributes fa;
+        PXQ_CUDA(c, cudaFuncGetAttributes(&fa, kern));
+        if ((long long)fa.numRegs * THREADS < (long long)SW * 32 * REG_S + (long long)(THREADS - SW * 32) * REG_E)
+            return fail(c, PICSARQED_ERR_CUDA, "internal: the fused step kernel was built with too few registers for setmaxnreg");
+    }
+    PXQ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const long long ntiles = n / kTile;
+    const int grid = (int)std::max<long long>(1, std::min<long long>(ntiles, (long long)c->num_sms));
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    if (c->time_kernels) {
+        for (int k = 0; k < 3; ++k) PXQ_CUDA(c, cudaEventCreate(&ev[k]));
+        PXQ_CUDA(c, cudaEventRecord(ev[0], c->stream));
+    }
+    kern<<<grid, THREADS, smem, c->stream>>>(sa);
+    PXQ_CUDA(c, cudaGetLastError());
+    if (n % kTile)  // the ragged last tile stages nothing: count its chunks from the updated tau
+        count_chunks_kernel<TR><<<1, 256, 0, c->stream>>>((const TR*)tau, n, (n / kTile) * kTile / kChunk, cs.n_chunks, cs.cnt,
+                                                          cs.sum, args.chunks_per_tile);
+    if (c->time_kernels) PXQ_CUDA(c, cudaEventRecord(ev[1], c->stream));
+    if (int rc = launch_event_pass<R, TR, SPECIES>(c, n, cs, p, eb, tau, seed, step, id_base, capacity, out_p, out_tau,
+                                                   parent, d_n_out))
+        return rc;
+    if (c->time_kernels) {
+        PXQ_CUDA(c, cudaEventRecord(ev[2], c->stream));
+        for (int k = 0; k < 3; ++k) c->timing_events.push_back(ev[k]);
+    }
+    return PICSARQED_OK;
+}
+
+template <typename R, typename TR, int SPECIES>
+int launch_fused_step(picsarqed_ctx* c, long long n, void* const* p, const void* const* eb, void* tau, double dt,
+                      unsigned long long seed, unsigned long long step, unsigned long long id_base, long long capacity,
+                      void* const* out_p, void* const* out_tau, long long* parent, unsigned long long* d_n_out) {
+    // "step_config": 0 = 16 streaming warps in 64 registers + 12 event warps in 80; 1 = 16 + 8 event warps, all in 80
+    if (c->step_config == 1)
+        return launch_fused_step_c<R, TR, SPECIES, 2, 0, 0>(c, n, p, eb, tau, dt, seed, step, id_base, capacity, out_p, out_tau,
+                                                           parent, d_n_out);
+    return launch_fused_step_c<R, TR, SPECIES, 3, 64, 80>(c, n, p, eb, tau, dt, seed, step, id_base, capacity, out_p, out_tau,
+                                                          parent, d_n_out);
+}
+
 // qed_step: the evolve pass stages the records of the particles that fire, then the common event pass
 template <typename R, typename TR, int SPECIES>
 int launch_step(picsarqed_ctx* c, long long n, void* const* p, const void* const* eb, void* tau, double dt,
                 unsigned long long seed, unsigned long long step, unsigned long long id_base, long long capacity,
                 void* const* out_p, void* const* out_tau, long long* parent, unsigned long long* d_n_out) {
+    if (c->fused_step)
+        return launch_fused_step<R, TR, SPECIES>(c, n, p, eb, tau, dt, seed, step, id_base, capacity, out_p, out_tau, parent,
+                                                 d_n_out);
     ChunkScratch cs;
-    if (int rc = chunk_scratch<R>(c, n, &cs)) return rc;
+    if (int rc = chunk_scratch(c, n, StageRecord<R>::kBytes, &cs)) return rc;
     StageView sv;
     sv.rec = cs.rec;
+    sv.stride = cs.stride;
     sv.cnt = cs.cnt;
     sv.tile_sum = cs.sum;
     sv.chunks_per_tile = event_chunks_per_tile(c);
@@ -680,7 +800,7 @@ int launch_append(picsarqed_ctx* c, long long m_max, const void* const* s_p, con
                   const unsigned long long* d_dst_n, long long dst_capacity, unsigned long long* d_kept,
                   unsigned long long* d_new_n) {
     ChunkScratch cs;
-    if (int rc = chunk_scratch<R>(c, m_max, &cs)) return rc;
+    if (int rc = chunk_scratch(c, m_max, 0, &cs)) return rc;
     const int grid = (int)std::max<long long>(1, std::min<long long>((cs.n_chunks + 7) / 8, (long long)c->num_sms * 8));
     keep_count_kernel<R><<<grid, 256, 0, c->stream>>>((const R*)s_p[0], (const R*)s_p[1], (const R*)s_p[2], d_count, m_max,
                                                        min_energy, cs.n_chunks, cs.cnt);

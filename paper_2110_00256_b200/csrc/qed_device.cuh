@@ -92,20 +92,20 @@ template <> __device__ __forceinline__ double uniform_open<double>(uint32_t a, u
 template <> __device__ __forceinline__ float uniform_open<float>(uint32_t a, uint32_t) {
     return ((float)(a >> 9) + 0.5f) * 0x1p-23f;                  // k < 2^23: exact
 }
-// tau = -ln U (PAPER.md:195)
-template <typename T> __device__ __forceinline__ T draw_tau(uint32_t a, uint32_t b);
-template <> __device__ __forceinline__ double draw_tau<double>(uint32_t a, uint32_t b) {
-    return -log(uniform_open<double>(a, b));
-}
-template <> __device__ __forceinline__ float draw_tau<float>(uint32_t a, uint32_t b) {
-    return -logf(uniform_open<float>(a, b));
-}
-
 // ---- lean fp64 elementary functions for the streaming kernel ------------------------------------
 // The CUDA library log/exp cost ~85 / ~50 instructions per call (special cases, constant moves); in the evolve
 // kernel they were 45 % of all instructions (profiles/r1b_step_full.md).  These versions assume what holds
 // there -- log of a positive normal number (anything else takes the library path), exp of a finite argument --
 // and keep the error at the 1e-16 level: a few ulp, far inside the 1e-9 tolerance on the optical depth.
+// They are written for V arguments at once (log_pos_v, exp_fast_v; the scalar names are V = 1): the common path is one
+// straight line for all V, so that the compiler interleaves the V dependent chains, and the special cases are selects
+// or one rarely taken branch at the end.  The polynomial coefficients live in constant memory: an FMA takes them as a
+// constant-bank operand, where an immediate costs two moves per use.
+__constant__ double kLogCoef[9] = {1.0 / 19.0, 1.0 / 17.0, 1.0 / 15.0, 1.0 / 13.0, 1.0 / 11.0, 1.0 / 9.0, 1.0 / 7.0, 1.0 / 5.0, 1.0 / 3.0};
+__constant__ double kExpCoef[12] = {1.0 / 6227020800.0, 1.0 / 479001600.0, 1.0 / 39916800.0, 1.0 / 3628800.0, 1.0 / 362880.0,
+                                    1.0 / 40320.0, 1.0 / 5040.0, 1.0 / 720.0, 1.0 / 120.0, 1.0 / 24.0, 1.0 / 6.0, 0.5};
+__constant__ double kLn2[3] = {6.93147180369123816490e-01, 1.90821492927058770002e-10, 1.4426950408889634074};  // hi, lo, log2(e)
+
 __device__ __forceinline__ double rcp_fast(double x) {        // 1/x for normal x, ~1 ulp
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));     // ~20 bits
@@ -119,57 +119,94 @@ __device__ __forceinline__ double rsqrt_fast(double x) {      // 1/sqrt(x) for n
     y = fma(fma(-hx * y, y, 0.5), y, y);
     return fma(fma(-hx * y, y, 0.5), y, y);
 }
-__device__ __forceinline__ double log_pos(double x) {
-    int hi = __double2hiint(x);
-    const int lo = __double2loint(x);
-    if ((unsigned)(hi - 0x00100000) >= 0x7fe00000u) return log(x);  // zero, denormal, inf, nan, negative
-    int e = (hi >> 20) - 1023;
-    hi = (hi & 0x000fffff) | 0x3ff00000;                     // mantissa in [1, 2)
-    if (hi >= 0x3ff6a09e) { hi -= 0x00100000; e += 1; }      // -> [sqrt(1/2), sqrt(2))
-    const double m = __hiloint2double(hi, lo);
-    const double num = m - 1.0, den = m + 1.0;
-    const double r = rcp_fast(den);
-    double s = num * r;
-    s = fma(fma(-s, den, num), r, s);                        // s = (m-1)/(m+1), |s| <= 0.1716
-    const double s2 = s * s;
+// ln x for positive normal x; anything else (zero, denormal, inf, nan, negative) takes the library routine
+template <int V>
+__device__ __forceinline__ void log_pos_v(const double (&x)[V], double (&y)[V]) {
+    double s[V], s2[V], p[V], ed[V];
+    bool special = false;
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+        int hi = __double2hiint(x[v]);
+        const int lo = __double2loint(x[v]);
+        special = special || (unsigned)(hi - 0x00100000) >= 0x7fe00000u;
+        int e = (hi >> 20) - 1023;
+        hi = (hi & 0x000fffff) | 0x3ff00000;                 // mantissa in [1, 2)
+        const bool up = hi >= 0x3ff6a09e;                    // -> [sqrt(1/2), sqrt(2))
+        hi = up ? hi - 0x00100000 : hi;
+        e = up ? e + 1 : e;
+        ed[v] = (double)e;
+        const double m = __hiloint2double(hi, lo);
+        const double num = m - 1.0, den = m + 1.0;
+        const double r = rcp_fast(den);
+        const double s0 = num * r;
+        s[v] = fma(fma(-s0, den, num), r, s0);               // s = (m-1)/(m+1), |s| <= 0.1716
+        s2[v] = s[v] * s[v];
+        p[v] = kLogCoef[0];
+    }
     // ln m = 2 atanh(s) = 2 s (1 + s^2/3 + s^4/5 + ... + s^18/19); the first dropped term is < 3e-17
-    double p = 1.0 / 19.0;
-    p = fma(p, s2, 1.0 / 17.0);
-    p = fma(p, s2, 1.0 / 15.0);
-    p = fma(p, s2, 1.0 / 13.0);
-    p = fma(p, s2, 1.0 / 11.0);
-    p = fma(p, s2, 1.0 / 9.0);
-    p = fma(p, s2, 1.0 / 7.0);
-    p = fma(p, s2, 1.0 / 5.0);
-    p = fma(p, s2, 1.0 / 3.0);
-    const double two_s = s + s;
-    const double lnm = fma(two_s * s2, p, two_s);
-    const double ed = (double)e;
-    return fma(ed, 6.93147180369123816490e-01, fma(ed, 1.90821492927058770002e-10, lnm));  // e ln2 (hi + lo)
+#pragma unroll
+    for (int k = 1; k < 9; ++k)
+#pragma unroll
+        for (int v = 0; v < V; ++v) p[v] = fma(p[v], s2[v], kLogCoef[k]);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+        const double two_s = s[v] + s[v];
+        const double lnm = fma(two_s * s2[v], p[v], two_s);
+        y[v] = fma(ed[v], kLn2[0], fma(ed[v], kLn2[1], lnm));   // e ln2 (hi + lo)
+    }
+    if (special) {
+#pragma unroll
+        for (int v = 0; v < V; ++v)
+            if ((unsigned)(__double2hiint(x[v]) - 0x00100000) >= 0x7fe00000u) y[v] = log(x[v]);
+    }
+}
+// e^x for any x (0 below -707, e^709 above 709, nan for nan)
+template <int V>
+__device__ __forceinline__ void exp_fast_v(const double (&x)[V], double (&y)[V]) {
+    double r[V], p[V];
+    int k[V];
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+        double xc = x[v] > 709.0 ? 709.0 : x[v];
+        xc = xc > -707.0 ? xc : -707.0;                      // (keeps k in range; the result is replaced below)
+        const double t = fma(xc, kLn2[2], 6755399441055744.0);   // k = rint(x log2 e) in the low word
+        k[v] = __double2loint(t);
+        const double kd = t - 6755399441055744.0;
+        r[v] = fma(kd, -kLn2[1], fma(kd, -kLn2[0], xc));     // |r| <= 0.3466
+        p[v] = kExpCoef[0];                                  // Taylor to r^13/13!: remainder < 2e-17
+    }
+#pragma unroll
+    for (int j = 1; j < 12; ++j)
+#pragma unroll
+        for (int v = 0; v < V; ++v) p[v] = fma(p[v], r[v], kExpCoef[j]);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+        p[v] = fma(p[v], r[v], 1.0);
+        p[v] = fma(p[v], r[v], 1.0);
+        const double e = __hiloint2double(__double2hiint(p[v]) + (k[v] << 20), __double2loint(p[v]));  // p 2^k, k in [-1021, 1023]
+        y[v] = x[v] > -707.0 ? e : (x[v] < 0.0 ? 0.0 : x[v]);   // underflow (or nan)
+    }
+}
+__device__ __forceinline__ double log_pos(double x) {
+    const double a[1] = {x};
+    double y[1];
+    log_pos_v<1>(a, y);
+    return y[0];
 }
 __device__ __forceinline__ double exp_fast(double x) {
-    if (!(x > -707.0)) return x < 0.0 ? 0.0 : x;             // underflow (or nan)
-    x = x > 709.0 ? 709.0 : x;
-    const double t = fma(x, 1.4426950408889634074, 6755399441055744.0);  // k = rint(x log2 e) in the low word
-    const int k = __double2loint(t);
-    const double kd = t - 6755399441055744.0;
-    double r = fma(kd, -6.93147180369123816490e-01, x);
-    r = fma(kd, -1.90821492927058770002e-10, r);             // |r| <= 0.3466
-    double p = 1.0 / 6227020800.0;                           // Taylor to r^13/13!: remainder < 2e-17
-    p = fma(p, r, 1.0 / 479001600.0);
-    p = fma(p, r, 1.0 / 39916800.0);
-    p = fma(p, r, 1.0 / 3628800.0);
-    p = fma(p, r, 1.0 / 362880.0);
-    p = fma(p, r, 1.0 / 40320.0);
-    p = fma(p, r, 1.0 / 5040.0);
-    p = fma(p, r, 1.0 / 720.0);
-    p = fma(p, r, 1.0 / 120.0);
-    p = fma(p, r, 1.0 / 24.0);
-    p = fma(p, r, 1.0 / 6.0);
-    p = fma(p, r, 0.5);
-    p = fma(p, r, 1.0);
-    p = fma(p, r, 1.0);
-    return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));  // p 2^k, k in [-1021, 1023]
+    const double a[1] = {x};
+    double y[1];
+    exp_fast_v<1>(a, y);
+    return y[0];
+}
+
+// tau = -ln U (PAPER.md:195)
+template <typename T> __device__ __forceinline__ T draw_tau(uint32_t a, uint32_t b);
+template <> __device__ __forceinline__ double draw_tau<double>(uint32_t a, uint32_t b) {
+    return -log_pos(uniform_open<double>(a, b));   // (u is a positive normal number: the lean logarithm applies)
+}
+template <> __device__ __forceinline__ float draw_tau<float>(uint32_t a, uint32_t b) {
+    return -logf(uniform_open<float>(a, b));
 }
 
 // ---- chi^2 --------------------------------------------------------------------------
@@ -362,14 +399,14 @@ __device__ __forceinline__ double qs_sample_xi(const Table2D<R>& T, double ln_ch
     const int M = T.n_xi;
     const R* __restrict__ r0 = T.P + (size_t)k * M;
     const double e0a = (double)__ldg(r0), e0b = (double)__ldg(r0 + M);
-    const double lr = log(r);
-    if (lr < fma(w, e0b - e0a, e0a)) return exp(T.ln_xi_min);  // below the first column (R6)
+    const double lr = log_pos(r);
+    if (lr < fma(w, e0b - e0a, e0a)) return exp_fast(T.ln_xi_min);  // below the first column (R6)
     double a, b;
     const int ms = search_row(T, k, w, lr, &a, &b);            // eq.29
     const double step = -T.ln_xi_min / (double)(M - 1);        // ln xi_{m+1} - ln xi_m
     const double lx0 = T.ln_xi_min + step * (double)ms;
-    if (!(b > a)) return exp(lx0);
-    return exp(fma((lr - a) / (b - a), step, lx0));            // eq.30
+    if (!(b > a)) return exp_fast(lx0);
+    return exp_fast(fma((lr - a) * rcp_fast(b - a), step, lx0));   // eq.30
 }
 
 // eqs.24-26 on r' = min(r, 1-r): xi = chi_-/chi_gamma in [0, 1/2]
@@ -383,7 +420,7 @@ __device__ __forceinline__ double bw_sample_xi(const Table2D<R>& T, double ln_ch
     const double step = 0.5 / (double)(M - 1);
     const double x0 = step * (double)ms;
     if (!(b > a)) return x0;
-    return fma((rp - a) / (b - a), step, x0);                  // eq.26
+    return fma((rp - a) * rcp_fast(b - a), step, x0);          // eq.26
 }
 
 // ---- 128-bit streaming loads / stores with L2 eviction policies -------------------------------
@@ -428,6 +465,31 @@ __device__ __forceinline__ Vec<T, V> ld_stream_rw(const T* p, unsigned long long
         o[4 * h] = a; o[4 * h + 1] = b; o[4 * h + 2] = c; o[4 * h + 3] = d;
     }
     return r;
+}
+// plain 128-bit loads that bypass L1 and carry no eviction hint (arrays the fused step rewrites a few microseconds
+// later: they should outlive the evict-first field lines in L2)
+template <typename T, int V>
+__device__ __forceinline__ Vec<T, V> ld_keep(const T* p) {
+    static_assert(sizeof(T) * V == 16 || sizeof(T) * V == 32, "128- or 256-bit vectors");
+    Vec<T, V> r;
+    uint32_t* o = reinterpret_cast<uint32_t*>(&r);
+#pragma unroll
+    for (int h = 0; h < (int)(sizeof(T) * V / 16); ++h) {
+        uint32_t a, b, c, d;
+        asm volatile("ld.global.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                     : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "l"(reinterpret_cast<const char*>(p) + 16 * h) : "memory");
+        o[4 * h] = a; o[4 * h + 1] = b; o[4 * h + 2] = c; o[4 * h + 3] = d;
+    }
+    return r;
+}
+// vector store in 128-bit pieces: the ABI promises 16-byte alignment only, and a Vec<double, 4> (fp32 particles with an
+// fp64 optical depth) stored whole would be one 256-bit store that faults on a 16-byte-aligned view
+template <typename T, int V>
+__device__ __forceinline__ void st_vec(T* p, const Vec<T, V>& v) {
+    static_assert(sizeof(T) * V == 16 || sizeof(T) * V == 32, "128- or 256-bit vectors");
+    const uint4* s = reinterpret_cast<const uint4*>(&v);
+#pragma unroll
+    for (int h = 0; h < (int)(sizeof(T) * V / 16); ++h) reinterpret_cast<uint4*>(p)[h] = s[h];
 }
 __device__ __forceinline__ void st_policy(uint4* p, const uint4& v, unsigned long long policy) {
     asm volatile("st.global.L2::cache_hint.v4.u32 [%0], {%1,%2,%3,%4}, %5;"
