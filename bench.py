@@ -44,6 +44,7 @@ def parse():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-sample", type=int, default=1 << 23, help="particles in the oracle timing sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--dt-scale", type=float, default=1.0, help="multiply the 5 %% time step (tuning experiments)")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
                     help="picsarqed_set_option before the run (tuning experiments), e.g. --opt fused_step=0")
     ap.add_argument("--cascade", action="store_true",
@@ -218,7 +219,7 @@ def run_ours(args):
     probe = torch.zeros(m, dtype=torch.float64, device=dev)
     ctx.evolve_optical_depth(q.LEPTON, [t[:m] for t in p], [t[:m] for t in fields[0][:3]],
                              [t[:m] for t in fields[0][3:]], 1.0, probe)
-    dt = w.choose_dt((-probe).cpu().numpy(), 0.05)
+    dt = w.choose_dt((-probe).cpu().numpy(), 0.05) * args.dt_scale
 
     def step(s):
         f = fields[s % n_sets]

@@ -69,7 +69,19 @@ __device__ __forceinline__ EventOut<R, TR> qs_event_compute(const EventArgs<R, T
     const Words4 w = qed_words(a.seed, id, a.step, 1, 0);
     const Words4 wc = qed_words(a.seed, id, a.step, 2, 0);
     const double r = (double)uniform_open<R>(w.w[0], w.w[1]);
-    const double xi = qs_sample_xi(a.cdf, 0.5 * log_pos(c2), r);
+    // the logarithms of the event at once (ln r, ln chi^2 and, for an fp64 optical depth, the two re-draws): four
+    // independent chains the V-at-once routine interleaves
+    double lg[4];
+    if constexpr (sizeof(TR) == 8) {
+        const double la[4] = {r, c2, uniform_open<double>(w.w[2], w.w[3]), uniform_open<double>(wc.w[0], wc.w[1])};
+        log_pos_v<4>(la, lg);
+    } else {
+        const double la[2] = {r, c2};
+        double l2[2];
+        log_pos_v<2>(la, l2);
+        lg[0] = l2[0]; lg[1] = l2[1]; lg[2] = lg[3] = 0.0;
+    }
+    const double xi = qs_sample_xi_ln(a.cdf, 0.5 * lg[1], lg[0]);
     const double inv_pn = p2 > 1e-300 ? rsqrt_fast(p2) : 0.0;
     const double nx = px * inv_pn, ny = py * inv_pn, nz = pz * inv_pn;
     const double km1 = p2 * rcp_fast(g + 1.0);  // gamma - 1 without cancellation
@@ -83,12 +95,12 @@ __device__ __forceinline__ EventOut<R, TR> qs_event_compute(const EventArgs<R, T
     o.sec[1] = (R)(gph * ny * ip);
     o.sec[2] = (R)(gph * nz * ip);
     o.sec[3] = o.sec[4] = o.sec[5] = (R)0;
-    o.sec_tau[0] = draw_tau<TR>(wc.w[0], wc.w[1]);
+    if constexpr (sizeof(TR) == 8) o.sec_tau[0] = -lg[3]; else o.sec_tau[0] = draw_tau<TR>(wc.w[0], wc.w[1]);
     o.sec_tau[1] = (TR)0;
     o.parent_p[0] = (R)(pn2 * nx * ip);
     o.parent_p[1] = (R)(pn2 * ny * ip);
     o.parent_p[2] = (R)(pn2 * nz * ip);
-    o.parent_tau = draw_tau<TR>(w.w[2], w.w[3]);
+    if constexpr (sizeof(TR) == 8) o.parent_tau = -lg[2]; else o.parent_tau = draw_tau<TR>(w.w[2], w.w[3]);
     return o;
 }
 
@@ -105,7 +117,14 @@ __device__ __forceinline__ EventOut<R, TR> bw_event_compute(const EventArgs<R, T
     const double r = (double)uniform_open<R>(w.w[0], w.w[1]);
     const bool electron_side = r <= 0.5;        // PAPER.md:212 "If r <= 0.5"
     const double rp = electron_side ? r : 1.0 - r;
-    const double xi = bw_sample_xi(a.cdf, 0.5 * log_pos(c2), rp);
+    double lg[3];
+    if constexpr (sizeof(TR) == 8) {
+        const double la[3] = {c2, uniform_open<double>(wc.w[0], wc.w[1]), uniform_open<double>(wc.w[2], wc.w[3])};
+        log_pos_v<3>(la, lg);
+    } else {
+        lg[0] = log_pos(c2); lg[1] = lg[2] = 0.0;
+    }
+    const double xi = bw_sample_xi(a.cdf, 0.5 * lg[0], rp);
     const double xe = electron_side ? xi : 1.0 - xi;   // chi_-/chi_gamma
     const double xp = electron_side ? 1.0 - xi : xi;   // chi_+/chi_gamma (eq.6)
     const double ke = (g - 2.0) * xe, kp = (g - 2.0) * xp;  // K = (gamma_gamma-2) chi_pm/chi_gamma
@@ -120,8 +139,8 @@ __device__ __forceinline__ EventOut<R, TR> bw_event_compute(const EventArgs<R, T
     o.sec[3] = (R)(pp * nx * ip);
     o.sec[4] = (R)(pp * ny * ip);
     o.sec[5] = (R)(pp * nz * ip);
-    o.sec_tau[0] = draw_tau<TR>(wc.w[0], wc.w[1]);
-    o.sec_tau[1] = draw_tau<TR>(wc.w[2], wc.w[3]);
+    if constexpr (sizeof(TR) == 8) { o.sec_tau[0] = -lg[1]; o.sec_tau[1] = -lg[2]; }
+    else { o.sec_tau[0] = draw_tau<TR>(wc.w[0], wc.w[1]); o.sec_tau[1] = draw_tau<TR>(wc.w[2], wc.w[3]); }
     o.parent_p[0] = o.parent_p[1] = o.parent_p[2] = (R)0;   // photon removed: p = 0, tau = +inf
     o.parent_tau = (TR)INFINITY;
     return o;

@@ -6,6 +6,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -50,7 +51,8 @@ struct picsarqed_ctx {
     int unit_system = 0;
     int event_config = 0;        // shape of event_kernel: see launch_event_pass
     int fused_step = 0;          // qed_step: 1 = the warp-specialised fused kernel (step.cuh), 0 = evolve pass + event pass
-    int step_spill = 1;          // fused kernel: 1 = a streaming warp whose queue is full hands the chunk to the record path
+    int step_spill = 0;          // fused kernel: 1 = a streaming warp whose queue is full hands the chunk to the record path
+    int step_batch_wait = 0;     // fused kernel: polls (2 us each) an event warp waits for four chunks before it takes fewer
     int step_config = 0;         // fused kernel: see launch_fused_step
     int time_kernels = 0;        // qed_step brackets its evolve pass and its event pass with CUDA events
     std::vector<cudaEvent_t> timing_events;  // triples (start, after evolve, after events), not yet read
@@ -284,6 +286,19 @@ int picsarqed_create(picsarqed_ctx** out, int cuda_device, void* cuda_stream) {
         return PICSARQED_ERR_CUDA;
     }
     *out = c;
+    // PICSARQED_OPTIONS="name=value,name=value": set_option calls applied to every new context (tuning experiments)
+    if (const char* env = std::getenv("PICSARQED_OPTIONS")) {
+        std::string all(env);
+        size_t pos = 0;
+        while (pos < all.size()) {
+            const size_t end = all.find(',', pos);
+            const std::string item = all.substr(pos, end == std::string::npos ? std::string::npos : end - pos);
+            const size_t eq = item.find('=');
+            if (eq != std::string::npos) picsarqed_set_option(c, item.substr(0, eq).c_str(), std::atoll(item.c_str() + eq + 1));
+            if (end == std::string::npos) break;
+            pos = end + 1;
+        }
+    }
     return PICSARQED_OK;
 }
 
@@ -329,10 +344,12 @@ int picsarqed_set_option(picsarqed_ctx* c, const char* name, long long value) {
         c->event_config = (int)value;
     else if (!std::strcmp(name, "fused_step") && (value == 0 || value == 1))
         c->fused_step = (int)value;
-    else if (!std::strcmp(name, "step_config") && (value == 0 || value == 1))
+    else if (!std::strcmp(name, "step_config") && value >= 0 && value <= 1)
         c->step_config = (int)value;
     else if (!std::strcmp(name, "step_spill") && (value == 0 || value == 1))
         c->step_spill = (int)value;
+    else if (!std::strcmp(name, "step_batch_wait") && value >= 0 && value <= 64)
+        c->step_batch_wait = (int)value;
     else if (!std::strcmp(name, "host_slabs") && value >= 0 && value <= kMaxSlabs)
         c->host_slabs = (int)value;
     else
@@ -637,12 +654,12 @@ int launch_events(picsarqed_ctx* c, long long n, void* const* p, const void* con
 
 // qed_step, fused (step.cuh): streaming warps evolve, event warps of the same CTA generate the events and rewrite the
 // parents while their sectors are in L2; then the offsets scan and the placement of the staged secondaries
-template <typename R, typename TR, int SPECIES, int C, int REG_S, int REG_E>
+template <typename R, typename TR, int SPECIES, int EW, int D, int REG_S, int REG_E>
 int launch_fused_step_c(picsarqed_ctx* c, long long n, void* const* p, const void* const* eb, void* tau, double dt,
                         unsigned long long seed, unsigned long long step, unsigned long long id_base, long long capacity,
                         void* const* out_p, void* const* out_tau, long long* parent, unsigned long long* d_n_out) {
     constexpr int SW = 16, NS = 2;
-    typedef StepLayout<R, TR, SW, C, NS> L;
+    typedef StepLayout<R, TR, SW, EW, D, NS> L;
     constexpr int THREADS = L::THREADS;
     constexpr long long kTile = (long long)SW * kChunk;
     typedef StepResult<R, TR, SPECIES> Res;
@@ -697,11 +714,12 @@ int launch_fused_step_c(picsarqed_ctx* c, long long n, void* const* p, const voi
     sa.ge.units = c->units;
     sa.stage_res = cs.rec;
     sa.spill = c->step_spill;
+    sa.batch_wait = c->step_batch_wait;
     const bool scaled = c->unit_system != PICSARQED_UNITS_LIBRARY;
     // registers (REG_S, REG_E != 0): the launch gives every thread floor(64 Ki / THREADS) rounded down to a multiple of 8
     // (72 for 896 threads); the streaming warps hand some back and the event warps take them
     void (*kern)(StepArgs<R, TR, SPECIES>) =
-        scaled ? step_kernel<R, TR, SPECIES, true, SW, C, NS, REG_S, REG_E> : step_kernel<R, TR, SPECIES, false, SW, C, NS, REG_S, REG_E>;
+        scaled ? step_kernel<R, TR, SPECIES, true, SW, EW, D, NS, REG_S, REG_E> : step_kernel<R, TR, SPECIES, false, SW, EW, D, NS, REG_S, REG_E>;
     if (REG_S != 0) {
         cudaFuncAttributes fa;
         PXQ_CUDA(c, cudaFuncGetAttributes(&fa, kern));
@@ -736,12 +754,13 @@ template <typename R, typename TR, int SPECIES>
 int launch_fused_step(picsarqed_ctx* c, long long n, void* const* p, const void* const* eb, void* tau, double dt,
                       unsigned long long seed, unsigned long long step, unsigned long long id_base, long long capacity,
                       void* const* out_p, void* const* out_tau, long long* parent, unsigned long long* d_n_out) {
-    // "step_config": 0 = 16 streaming warps in 64 registers + 12 event warps in 80; 1 = 16 + 8 event warps, all in 80
-    if (c->step_config == 1)
-        return launch_fused_step_c<R, TR, SPECIES, 2, 0, 0>(c, n, p, eb, tau, dt, seed, step, id_base, capacity, out_p, out_tau,
-                                                           parent, d_n_out);
-    return launch_fused_step_c<R, TR, SPECIES, 3, 64, 80>(c, n, p, eb, tau, dt, seed, step, id_base, capacity, out_p, out_tau,
-                                                          parent, d_n_out);
+    // "step_config": 0 = 16 streaming warps in 80 registers + 12 event warps in 56; 1 = 16 + 8 event warps, all in 80
+#define PXQ_FUSED(EW, D, RS, RE)                                                                                         \
+    return launch_fused_step_c<R, TR, SPECIES, EW, D, RS, RE>(c, n, p, eb, tau, dt, seed, step, id_base, capacity, out_p, \
+                                                              out_tau, parent, d_n_out)
+    if (c->step_config == 1) PXQ_FUSED(8, 3, 0, 0);
+    PXQ_FUSED(12, 3, 80, 56);
+#undef PXQ_FUSED
 }
 
 // qed_step: the evolve pass stages the records of the particles that fire, then the common event pass

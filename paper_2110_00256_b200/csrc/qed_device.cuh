@@ -320,27 +320,40 @@ __device__ __forceinline__ void row_bracket(const Table2D<R>& T, double ln_chi, 
 // rows bounds the interpolated row); it is verified against the table and dropped if a rounding of the bin
 // index made it wrong; (2) every level probes eight interior points at once (nine-way split), so the
 // bracket closes in one or two round trips instead of log2(M).
+// The guide entries of a key (four 16-bit loads that depend on the row and the key only: the callers issue them together
+// with whatever else they load first, one round trip instead of two).
+struct GuideBracket { int lo, hi; bool guided; };
 template <typename R>
-__device__ __forceinline__ int search_row(const Table2D<R>& T, int k, double w, double key, double* a_out, double* b_out) {
-    const int M = T.n_xi;
-    const R* __restrict__ r0 = T.P + (size_t)k * M;
-    const R* __restrict__ r1 = r0 + M;
-    auto ell = [&](int m) { const double a = (double)__ldg(r0 + m); return fma(w, (double)__ldg(r1 + m) - a, a); };
-    int lo = 0, hi = M - 1;
-    bool verified = true;
-    if (T.guide != nullptr) {
+__device__ __forceinline__ GuideBracket guide_bracket(const Table2D<R>& T, int k, double key) {
+    GuideBracket g;
+    g.lo = 0;
+    g.hi = T.n_xi - 1;
+    g.guided = T.guide != nullptr;
+    if (g.guided) {
         const int J = T.guide_bins;
         int j = (int)((key - T.guide_k0) * T.guide_inv_dk);
         j = max(0, min(j, J - 1));
         const unsigned short* g0 = T.guide + (size_t)k * (J + 1) + j;
         const unsigned short* g1 = g0 + (J + 1);
         const int a0 = __ldg(g0), a1 = __ldg(g0 + 1), b0 = __ldg(g1), b1 = __ldg(g1 + 1);
-        lo = j == 0 ? 0 : min(a0, b0);
-        hi = min(max(a1, b1) + 1, M - 1);
-        verified = false;
+        g.lo = j == 0 ? 0 : min(a0, b0);
+        g.hi = min(max(a1, b1) + 1, T.n_xi - 1);
     }
+    return g;
+}
+
+template <typename R>
+__device__ __forceinline__ int search_row(const Table2D<R>& T, int k, double w, double key, const GuideBracket& gb,
+                                          double* a_out, double* b_out) {
+    const int M = T.n_xi;
+    const R* __restrict__ r0 = T.P + (size_t)k * M;
+    const R* __restrict__ r1 = r0 + M;
+    auto ell = [&](int m) { const double a = (double)__ldg(r0 + m); return fma(w, (double)__ldg(r1 + m) - a, a); };
+    int lo = gb.lo, hi = gb.hi;
+    bool verified = !gb.guided;
+    bool have_vb = false;         // vb = ell(hi) is known (always, once a guide bracket has been verified)
     double va = 0.0, vb = 0.0;
-    if (verified) va = ell(0);  // (vb is never used before it is set: hi = M-1 needs no upper value)
+    if (verified) va = ell(0);    // (unguided: hi = M-1, whose value is fetched at the end if it is still the upper end)
     while (true) {
         const int span = hi - lo;
         const int step = (span + 8) / 9;
@@ -354,10 +367,12 @@ __device__ __forceinline__ int search_row(const Table2D<R>& T, int k, double w, 
             va = ell(lo);
             vb = ell(hi);
             verified = true;
+            have_vb = true;
             if (!(va <= key) || !(vb > key || hi == M - 1)) {  // guide bracket does not hold: full range
                 lo = 0;
                 hi = M - 1;
                 va = ell(0);
+                have_vb = false;
                 continue;
             }
         }
@@ -373,7 +388,7 @@ __device__ __forceinline__ int search_row(const Table2D<R>& T, int k, double w, 
             if (q + 1 == cnt) na = v[q];
             if (q == cnt && nhi_c < hi) nb = v[q];
         }
-        if (nhi_c < hi) hi = nhi_c;
+        if (nhi_c < hi) { hi = nhi_c; have_vb = true; }
         lo = nlo;
         va = na;
         vb = nb;
@@ -382,7 +397,7 @@ __device__ __forceinline__ int search_row(const Table2D<R>& T, int k, double w, 
         lo = M - 2;
         va = ell(lo);
         vb = ell(lo + 1);
-    } else if (hi == M - 1) {
+    } else if (!have_vb) {
         vb = ell(hi);             // the upper end was never probed
     }
     *a_out = va;
@@ -390,23 +405,27 @@ __device__ __forceinline__ int search_row(const Table2D<R>& T, int k, double w, 
     return lo;
 }
 
-// eqs.28-30: xi = chi_gamma/chi of the emitted photon for uniform r.
+// eqs.28-30: xi = chi_gamma/chi of the emitted photon for uniform r (lr = ln r).
 // Event arithmetic is fp64 whatever the table element type (events are rare).
 template <typename R>
-__device__ __forceinline__ double qs_sample_xi(const Table2D<R>& T, double ln_chi, double r) {
+__device__ __forceinline__ double qs_sample_xi_ln(const Table2D<R>& T, double ln_chi, double lr) {
     int k; double w;
     row_bracket(T, ln_chi, &k, &w);
     const int M = T.n_xi;
     const R* __restrict__ r0 = T.P + (size_t)k * M;
+    const GuideBracket gb = guide_bracket(T, k, lr);           // (issued together with the first column)
     const double e0a = (double)__ldg(r0), e0b = (double)__ldg(r0 + M);
-    const double lr = log_pos(r);
     if (lr < fma(w, e0b - e0a, e0a)) return exp_fast(T.ln_xi_min);  // below the first column (R6)
     double a, b;
-    const int ms = search_row(T, k, w, lr, &a, &b);            // eq.29
+    const int ms = search_row(T, k, w, lr, gb, &a, &b);        // eq.29
     const double step = -T.ln_xi_min / (double)(M - 1);        // ln xi_{m+1} - ln xi_m
     const double lx0 = T.ln_xi_min + step * (double)ms;
     if (!(b > a)) return exp_fast(lx0);
     return exp_fast(fma((lr - a) * rcp_fast(b - a), step, lx0));   // eq.30
+}
+template <typename R>
+__device__ __forceinline__ double qs_sample_xi(const Table2D<R>& T, double ln_chi, double r) {
+    return qs_sample_xi_ln(T, ln_chi, log_pos(r));
 }
 
 // eqs.24-26 on r' = min(r, 1-r): xi = chi_-/chi_gamma in [0, 1/2]
@@ -416,7 +435,8 @@ __device__ __forceinline__ double bw_sample_xi(const Table2D<R>& T, double ln_ch
     row_bracket(T, ln_chi, &k, &w);
     const int M = T.n_xi;
     double a, b;
-    const int ms = search_row(T, k, w, rp, &a, &b);            // eq.25 (P(0) = 0 <= r')
+    const GuideBracket gb = guide_bracket(T, k, rp);
+    const int ms = search_row(T, k, w, rp, gb, &a, &b);        // eq.25 (P(0) = 0 <= r')
     const double step = 0.5 / (double)(M - 1);
     const double x0 = step * (double)ms;
     if (!(b > a)) return x0;

@@ -59,6 +59,7 @@ struct StepArgs {
     EventArgs<R, TR> ge;        // cdf table, seed, step, id_base, units (its arrays alias ev's, writable)
     unsigned char* stage_res;   // [n_chunks] segments (ev.stage_stride apart) of kStageCap StepResult<R, TR, SPECIES> --
                                 // or StageRecord<R>, for the chunks a full queue sent to the record path of event_kernel
+    int batch_wait;             // polls an event warp waits for a full batch (see the event warps' loop)
     int spill;                  // 1: a streaming warp that finds its queue buffer taken does not wait: the chunk goes to
                                 // the record path of event_kernel (same routines, same results; its parents are then
                                 // rewritten by scattered read-modify-writes)
@@ -113,7 +114,7 @@ __device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gmem_src, u
 }
 
 // shared-memory layout of the kernel, after the table: [stages][record queues]
-template <typename R, typename TR, int SW, int C, int NS>
+template <typename R, typename TR, int SW, int EW, int D, int NS>
 struct StepLayout {
     static constexpr int V = 16 / sizeof(R);            // particles per lane and sub-chunk
     static constexpr int SUB = 32 * V;                  // particles per sub-chunk
@@ -122,17 +123,24 @@ struct StepLayout {
     static constexpr unsigned TB = SUB * sizeof(TR);
     static constexpr unsigned STAGE = 9 * AB + TB;
     static constexpr size_t stages_bytes = (size_t)SW * NS * STAGE;
-    static constexpr size_t queue_bytes = (size_t)SW * C * kStageCap * sizeof(StepRecord<R, TR>);
-    static constexpr int THREADS = (SW + (SW / kStepGroup) * C) * 32;
+    static constexpr size_t queue_bytes = (size_t)SW * D * kStageCap * sizeof(StepRecord<R, TR>);
+    static constexpr int THREADS = (SW + EW) * 32;
+    static constexpr int LAUNCH_REGS = ((65536 / THREADS) / 8) * 8;   // what __launch_bounds__(THREADS, 1) gives a thread
 };
 
+template <int N, int LAUNCH> __device__ __forceinline__ void reg_set() {   // N registers per thread from here on
+    if constexpr (N > LAUNCH) reg_alloc<N>();
+    else if constexpr (N > 0 && N < LAUNCH) reg_dealloc<N>();
+}
+
+// SW streaming warps (SW <= 32), EW event warps, D record buffers per streaming warp, NS sub-chunk stages per streaming warp.
 // REG_S / REG_E: registers per thread of the two roles after setmaxnreg (0 = keep the launch allocation).
-template <typename R, typename TR, int SPECIES, bool SCALED, int SW, int C, int NS, int REG_S, int REG_E>
-__global__ void __launch_bounds__((SW + (SW / kStepGroup) * C) * 32, 1) step_kernel(const StepArgs<R, TR, SPECIES> sa) {
-    typedef StepLayout<R, TR, SW, C, NS> L;
+template <typename R, typename TR, int SPECIES, bool SCALED, int SW, int EW, int D, int NS, int REG_S, int REG_E>
+__global__ void __launch_bounds__((SW + EW) * 32, 1) step_kernel(const StepArgs<R, TR, SPECIES> sa) {
+    typedef StepLayout<R, TR, SW, EW, D, NS> L;
     constexpr int V = L::V, SUB = L::SUB, HALVES = L::HALVES;
     constexpr int TILE = SW * kChunk;
-    static_assert(SW % kStepGroup == 0 && kStepGroup <= 32, "four streaming warps per group of event warps");
+    static_assert(SW <= 32 && SW % 4 == 0 && EW % 4 == 0, "lane q of an event warp watches queue q; setmaxnreg acts on groups of four warps");
     typedef StepRecord<R, TR> Rec;
     typedef StepResult<R, TR, SPECIES> Res;
     const EvolveArgs<R, TR>& a = sa.ev;
@@ -141,8 +149,10 @@ __global__ void __launch_bounds__((SW + (SW / kStepGroup) * C) * 32, 1) step_ker
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ unsigned long long mbar;
     __shared__ unsigned long long full_bar[SW][NS];
-    __shared__ unsigned q_full[SW][C], q_empty[SW][C], finished[SW];
-    __shared__ StepQueueHeader header[SW][C];
+    // queue of streaming warp q: entry n lives in buffer n % D.  produced[q] entries published (by q), claimed[q] entries
+    // taken (compare-and-swap by the event warps), released[q][b] times buffer b has been handed back
+    __shared__ unsigned produced[SW], claimed[SW], released[SW][D], finished[SW];
+    __shared__ StepQueueHeader header[SW][D];
 
     const R* tab = a.tab.L;
     if (a.table_in_smem) {
@@ -151,19 +161,19 @@ __global__ void __launch_bounds__((SW + (SW / kStepGroup) * C) * 32, 1) step_ker
         tab = reinterpret_cast<const R*>(smem_raw);
     }
     if (threadIdx.x < SW) {
-        finished[threadIdx.x] = 0u;
-        for (int b = 0; b < C; ++b) q_full[threadIdx.x][b] = q_empty[threadIdx.x][b] = 0u;
+        finished[threadIdx.x] = produced[threadIdx.x] = claimed[threadIdx.x] = 0u;
+        for (int b = 0; b < D; ++b) released[threadIdx.x][b] = 0u;
         for (int s = 0; s < NS; ++s) mbar_init(&full_bar[threadIdx.x][s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
     unsigned char* const stages = smem_raw + a.table_bytes;
-    Rec* const recs = reinterpret_cast<Rec*>(stages + L::stages_bytes);   // [SW][C][kStageCap]
+    Rec* const recs = reinterpret_cast<Rec*>(stages + L::stages_bytes);   // [SW][D][kStageCap]
     const long long ntiles_full = a.n / TILE;
 
     if (warp < SW) {
         // ================================ streaming warps =========================================
-        if constexpr (REG_S > 0) reg_dealloc<REG_S>();
+        reg_set<REG_S, L::LAUNCH_REGS>();
         const unsigned long long pol_stream = l2_policy_evict_first();
         // this warp's sequence of sub-chunks: j = 0, 1, ...; tile blockIdx.x + (j / HALVES) gridDim.x, half j % HALVES
         const long long my_tiles = ntiles_full > blockIdx.x ? (ntiles_full - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
@@ -240,12 +250,12 @@ __global__ void __launch_bounds__((SW + (SW / kStepGroup) * C) * 32, 1) step_ker
             // the evolved tau goes out BEFORE the chunk is published: the event warp's store of the new tau must land on top
             st_vec<TR, V>(a.tau + base + lane * V, t);
             if (all > 0 && queued && !spilled && !have_buf) {
-                // the first records of the chunk: take buffer n_pub % C of this warp's queue (free when its consumer is
-                // done with entry n_pub - C)
-                const unsigned b = n_pub % C, k = n_pub / C;
+                // the first records of the chunk: take buffer n_pub % D of this warp's queue (free when entry n_pub - D
+                // has been handed back)
+                const unsigned b = n_pub % D, k = n_pub / D;
                 auto room = [&]() {
                     unsigned e = 0;
-                    if (lane == 0) e = ld_flag(&q_empty[warp][b]);
+                    if (lane == 0) e = ld_flag(&released[warp][b]);
                     return __shfl_sync(0xffffffffu, e, 0) == k;
                 };
                 if (sa.spill) {
@@ -253,7 +263,7 @@ __global__ void __launch_bounds__((SW + (SW / kStepGroup) * C) * 32, 1) step_ker
                 } else {
                     while (!room()) __nanosleep(64);
                 }
-                wbuf = recs + ((size_t)warp * C + b) * kStageCap;
+                wbuf = recs + ((size_t)warp * D + b) * kStageCap;
                 have_buf = !spilled;
             }
             if (total > (unsigned)kStageCap) queued = false;   // too many for a segment: the re-scan path of event_kernel
@@ -289,14 +299,14 @@ __global__ void __launch_bounds__((SW + (SW / kStepGroup) * C) * 32, 1) step_ker
                                                                                     : (queued ? total : (total | kStageNoRecords))));
                     if (total > 0) atomicAdd(a.tile_sum + chunk / a.chunks_per_tile, total);
                     if (publish) {
-                        header[warp][n_pub % C].chunk = chunk;
-                        header[warp][n_pub % C].total = total;
+                        header[warp][n_pub % D].chunk = chunk;
+                        header[warp][n_pub % D].total = total;
                     }
                 }
                 if (publish) {
                     __syncwarp();
-                    if (lane == 0) st_flag(&q_full[warp][n_pub % C], n_pub / C + 1);   // release: records, header, tau stores
                     ++n_pub;
+                    if (lane == 0) st_flag(&produced[warp], n_pub);   // release: records, header, tau stores
                 }
             }
         }
@@ -313,60 +323,92 @@ __global__ void __launch_bounds__((SW + (SW / kStepGroup) * C) * 32, 1) step_ker
         if (lane == 0) st_flag(&finished[warp], 1u);
     } else {
         // ================================ event warps ============================================
-        if constexpr (REG_E > 0) reg_alloc<REG_E>();
+        reg_set<REG_E, L::LAUNCH_REGS>();
         const EventArgs<R, TR>& g = sa.ge;
         const int ew = warp - SW;
-        const int grp = ew / C, buf = ew % C;                           // this warp consumes buffer `buf` of its group's queues
-        const int my_q = grp * kStepGroup + (lane < kStepGroup ? lane : 0);   // the queue lane q < 4 watches
-        unsigned cons = 0;                                              // entries of (my_q, buf) consumed so far
         int idle_polls = 0;
+        unsigned rot = (unsigned)(ew * 4) % SW;   // where this warp starts looking (spreads the event warps over the queues)
         while (true) {
-            unsigned cnt = 0, fin = 1;
-            long long chunk_l = 0;
-            if (lane < kStepGroup) {
-                fin = ld_flag(&finished[my_q]);                         // (read before q_full: a finished queue is final)
-                const unsigned prod = ld_flag(&q_full[my_q][buf]);
-                if (prod != cons) {
-                    const StepQueueHeader h = header[my_q][buf];
-                    cnt = h.total;
-                    chunk_l = h.chunk;
-                    fin = 0;
-                }
+            // lane q < SW looks at queue q
+            unsigned avail = 0, fin = 1, my_claim = 0;
+            if (lane < SW) {
+                fin = ld_flag(&finished[lane]);                         // (read before `produced`: a finished queue is final)
+                my_claim = *reinterpret_cast<volatile unsigned*>(&claimed[lane]);
+                const unsigned prod = ld_flag(&produced[lane]);
+                avail = prod != my_claim ? 1u : 0u;
+                if (avail) fin = 0;
             }
-            __syncwarp();          // (the lanes that did not read the flags are ordered after the acquire as well)
-            unsigned incl = cnt;   // offsets of the (at most four) chunks of this batch
+            const unsigned avail_mask = __ballot_sync(0xffffffffu, avail != 0);
+            // A pass costs the same instructions whether 5 or 32 lanes hold an event, and the kernel is bound by instruction
+            // issue: wait for four chunks (about 31 events) unless the queues are running dry.
+            if (avail_mask == 0 || (__popc(avail_mask) < 4 && idle_polls < sa.batch_wait)) {
+                if (avail_mask == 0 && __all_sync(0xffffffffu, fin != 0)) break;
+                ++idle_polls;
+                __nanosleep(2000);   // (a poll costs issue slots the streaming warps need; a chunk arrives every few microseconds)
+                continue;
+            }
+            idle_polls = 0;
+            // take up to four queues, first come from `rot` on, and claim their next entry (another event warp may be
+            // quicker: up to three rounds over what is left)
+            constexpr unsigned kAll = (SW == 32) ? 0xffffffffu : ((1u << SW) - 1u);
+            unsigned left = ((avail_mask >> rot) | (avail_mask << (SW - rot))) & kAll;   // bit k: queue (rot + k) % SW
+            unsigned got_mask = 0;
+            bool got = false;
+            for (int round = 0; round < 3 && left != 0 && __popc(got_mask) < 4; ++round) {
+                unsigned pick = 0;
+                const int need = 4 - __popc(got_mask);
+                for (int k = 0; k < need && left != 0; ++k) {
+                    const unsigned low = left & (0u - left);
+                    pick |= low;
+                    left ^= low;
+                }
+                const unsigned pick_mask = ((pick << rot) | (pick >> (SW - rot))) & kAll;
+                bool ok = false;
+                if ((pick_mask >> lane) & 1u) ok = atomicCAS(&claimed[lane], my_claim, my_claim + 1u) == my_claim;
+                got = got || ok;
+                got_mask |= __ballot_sync(0xffffffffu, ok);
+            }
+            rot = (rot + 5) % SW;
+            if (got_mask == 0) continue;
+            unsigned cnt_src = 0;
+            long long chunk_src = 0;
+            if (got) {
+                const StepQueueHeader h = header[lane][my_claim % D];
+                cnt_src = h.total;
+                chunk_src = h.chunk;
+            }
+            // lanes 0..3 take over the (at most four) entries of the batch, in queue order
+            const int n_got = __popc(got_mask);
+            const int src = lane < n_got ? (int)__fns(got_mask, 0, lane + 1) : 0;
+            unsigned cnt = __shfl_sync(0xffffffffu, cnt_src, src);
+            const long long chunk_l = __shfl_sync(0xffffffffu, chunk_src, src);
+            const unsigned entry_l = __shfl_sync(0xffffffffu, my_claim, src);
+            if (lane >= n_got) cnt = 0;
+            const int q_l = src;
+            unsigned incl = cnt;   // offsets of the chunks of this batch
 #pragma unroll
-            for (int d = 1; d < kStepGroup; d <<= 1) {
+            for (int d = 1; d < 4; d <<= 1) {
                 const unsigned o = __shfl_up_sync(0xffffffffu, incl, d);
                 if (lane >= d) incl += o;
             }
             const unsigned off_l = incl - cnt;
-            const unsigned total = __shfl_sync(0xffffffffu, incl, kStepGroup - 1);
-            // A pass costs the same instructions whether 5 or 32 lanes hold an event, and the kernel is bound by instruction
-            // issue: wait until every queue that is still being fed has an entry for this warp (about 31 events), but not
-            // for ever -- a streaming warp whose chunks hold no event publishes nothing.
-            const bool all_in = __all_sync(0xffffffffu, cnt > 0 || fin != 0);
-            if (total == 0 || (!all_in && idle_polls < 16)) {
-                if (total == 0 && __all_sync(0xffffffffu, fin != 0)) break;
-                ++idle_polls;
-                __nanosleep(1000);   // (a poll costs issue slots the streaming warps need; a chunk arrives every few microseconds)
-                continue;
-            }
-            idle_polls = 0;
+            const unsigned total = __shfl_sync(0xffffffffu, incl, 3);
             for (unsigned e0 = 0; e0 < total; e0 += 32) {
                 const unsigned e = e0 + lane;
                 int j = 0;
 #pragma unroll
-                for (int k = 1; k < kStepGroup; ++k) {
+                for (int k = 1; k < 4; ++k) {
                     const unsigned ok = __shfl_sync(0xffffffffu, off_l, k);
                     const unsigned ck = __shfl_sync(0xffffffffu, cnt, k);
                     if (ck > 0 && ok <= e) j = k;
                 }
                 const unsigned off_j = __shfl_sync(0xffffffffu, off_l, j);
                 const long long chunk = __shfl_sync(0xffffffffu, chunk_l, j);
+                const unsigned entry = __shfl_sync(0xffffffffu, entry_l, j);
+                const int q = __shfl_sync(0xffffffffu, q_l, j);
                 if (e >= total) continue;
                 const unsigned r = e - off_j;
-                const Rec rec = recs[((size_t)(grp * kStepGroup + j) * C + buf) * kStageCap + r];
+                const Rec rec = recs[((size_t)q * D + entry % D) * kStageCap + r];
                 const long long i = chunk * kChunk + rec.idx;
                 const double sp = g.units.p;
                 const double px = rec.p[0] * sp, py = rec.p[1] * sp, pz = rec.p[2] * sp;
@@ -391,10 +433,7 @@ __global__ void __launch_bounds__((SW + (SW / kStepGroup) * C) * 32, 1) step_ker
                 for (int k = 0; k < (int)(sizeof(Res) / 16); ++k) dst[k] = o.raw[k];
             }
             __syncwarp();
-            if (lane < kStepGroup && cnt > 0) {
-                ++cons;
-                st_flag(&q_empty[my_q][buf], cons);   // release: the buffer may be overwritten
-            }
+            if (lane < n_got) st_flag(&released[q_l][entry_l % D], entry_l / D + 1u);   // release: the buffer may be overwritten
         }
     }
 }
