@@ -27,9 +27,11 @@ METRIC = "QED MC step particles/sec (fp64/fp32) at 1 B200; achieved HBM GB/s vs 
 UNIT = "particles/s"
 SEED = 2
 BYTES_PER_PARTICLE_EVOLVE = 88  # 9 reads + tau read + tau write, fp64
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the evolve pass (16 Mi particles), ncu --set full:
-# profiles/r1d_step_full.md (1.343606 GB read = the 80 B/particle of inputs; 109 MB written: part of the 134 MB of
-# new tau is still dirty in L2 when the kernel ends, plus the staged records)
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the evolve pass at 16 Mi particles, from the ncu --set full
+# capture named in EVOLVE_TRAFFIC_SOURCE (1.3436 GB read = the 80 B/particle of inputs; 109 MB written: part of the 134 MB
+# of new tau is still dirty in L2 when the kernel ends, plus the staged records).  A profile figure, not a measurement of
+# the timed run: the line says so in `traffic_source`, and carries it only at the profiled size.
+EVOLVE_TRAFFIC_SOURCE = "profiles/r2_step_full.md (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum, 16 Mi particles)"
 EVOLVE_DRAM_TRAFFIC_BYTES = 1343606000 + 108954112
 
 
@@ -44,6 +46,8 @@ def parse():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-sample", type=int, default=1 << 23, help="particles in the oracle timing sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="only the headline configuration 2 (skip configs 3, 5 and 4 in `other_configs`)")
     ap.add_argument("--dt-scale", type=float, default=1.0, help="multiply the 5 %% time step (tuning experiments)")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
                     help="picsarqed_set_option before the run (tuning experiments), e.g. --opt fused_step=0")
@@ -163,6 +167,248 @@ def run_reference(args):
                              "sample": "%d particles x %d steps (evolve + photon emission)" % (n, steps_run)},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+#  the other configurations of BASELINE.json (the fp32 half of the metric, the table build)
+# ------------------------------------------------------------------------------------------------
+def event_bytes(species, es, ts, with_parent_index):
+    """algorithmic bytes of one event: the parent's momentum and optical depth rewritten, the
+    secondaries (3 reals + optical depth each) written, 8 bytes of parent index when the caller asks for it"""
+    nsec = 1 if species == 0 else 2
+    return (3 * es + ts) + nsec * (3 * es + ts) + (8 if with_parent_index else 0)
+
+
+def timed_steps(torch, ctx, step_fn, reseed_fn, steps, warmup):
+    """per-step CUDA events on the context's stream; reseed_fn (restoring consumed photons) runs between steps, outside
+    the timed brackets.  Returns (mean ms per step, evolve-pass ms, event-pass ms)"""
+    for s in range(warmup):
+        reseed_fn()
+        step_fn(s)
+    torch.cuda.synchronize()
+    ctx.set_option("time_kernels", 1)
+    ctx.get_timing()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for k in range(steps):
+        reseed_fn()
+        ev[k][0].record()
+        step_fn(warmup + k)
+        ev[k][1].record()
+    torch.cuda.synchronize()
+    ms_a, ms_b, calls = ctx.get_timing()
+    ctx.set_option("time_kernels", 0)
+    ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
+    return ms, ms_a / max(steps, 1), ms_b / max(steps, 1)
+
+
+def leg_roofline(peaks, peak_kind, kernel, evolve_bytes, ms_evolve, step_bytes, ms_step):
+    ach = evolve_bytes / (ms_evolve * 1e-3) / 1e9
+    whole = step_bytes / (ms_step * 1e-3) / 1e9
+    return {"bound": "hbm", "kernel": kernel, "achieved": ach, "peak": peaks["hbm_gbs"],
+            "peak_kind": peak_kind + " (MEASURED_PEAKS.json hbm_gbs, copy)", "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
+            "traffic": None, "algorithmic_bytes_per_launch": evolve_bytes, "ms_per_launch": ms_evolve,
+            "whole_step": {"algorithmic_bytes": step_bytes, "achieved": whole, "frac": whole / peaks["hbm_gbs"]}}
+
+
+def run_config3(args, torch, q, w, ctx, dev, peaks, peak_kind):
+    """BASELINE config 3: 16 Mi photons, fp32, Breit-Wheeler only; every event makes a pair; the photons that decayed are
+    re-seeded between steps, so every step sees 16 Mi live photons"""
+    n, seed = args.particles, 3
+    cap = n // 8
+    p_h, gamma = w.config3(seed=seed, n=n)
+    n_sets = 4
+    p = [torch.from_numpy(a).to(dev) for a in p_h]
+    fields = []
+    for s_ in range(n_sets):
+        e_h, b_h = w.config3_fields(seed, s_, gamma)
+        fields.append([torch.from_numpy(a).to(dev) for a in (*e_h, *b_h)])
+    tau = torch.empty(n, dtype=torch.float32, device=dev)
+    ctx.init_optical_depth(q.PHOTON, tau, seed, 0)
+    p0, tau0 = [t.clone() for t in p], tau.clone()
+    m = min(n, 1 << 16)
+    probe = torch.zeros(m, dtype=torch.float32, device=dev)
+    ctx.evolve_optical_depth(q.PHOTON, [t[:m] for t in p], [t[:m] for t in fields[0][:3]], [t[:m] for t in fields[0][3:]], 1.0, probe)
+    dt = w.choose_dt((-probe).double().cpu().numpy(), 0.05)
+    el = [torch.empty(cap, dtype=torch.float32, device=dev) for _ in range(4)]
+    po = [torch.empty(cap, dtype=torch.float32, device=dev) for _ in range(4)]
+    parent = torch.empty(cap, dtype=torch.int64, device=dev)
+    n_out = torch.zeros(1, dtype=torch.int64, device=dev)
+
+    def reseed():     # dead photons (p = 0, tau = +inf) come back as they were; the survivors keep their optical depth
+        dead = torch.isinf(tau)
+        for a, a0 in zip(p, p0):
+            torch.where(dead, a0, a, out=a)
+        torch.where(dead, tau0, tau, out=tau)
+
+    def step(s_):
+        f = fields[s_ % n_sets]
+        ctx.qed_step(q.PHOTON, p, f[:3], f[3:], tau, dt, seed, s_, 0, cap, el[:3], el[3], po[:3], po[3], parent, n_out)
+
+    steps = max(20, args.steps) if args.steps >= 5 else args.steps
+    ms, ms_ev, ms_evt = timed_steps(torch, ctx, step, reseed, steps, args.warmup)
+    fired = ctx.read_count(n_out)
+    evolve_bytes = 44 * n
+    step_bytes = evolve_bytes + event_bytes(1, 4, 4, True) * fired
+    leg = {"workload": "config 3: Breit-Wheeler pair production only, fp32, %d photons, 1024-pt lnT + 1024x1024 pair CDF "
+                       "(fp32 copy), evolve + pair creation per step, decayed photons re-seeded between steps" % n,
+           "dtype": "f32", "value": n / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms, "steps": steps,
+           "fired_fraction_last_step": fired / n, "dt_s": dt,
+           "timing": "mean of per-step CUDA events; the re-seeding of decayed photons runs between the brackets",
+           "kernels_ms": {"evolve_pass": ms_ev, "event_pass": ms_evt},
+           "roofline": leg_roofline(peaks, peak_kind, "evolve_kernel<float,float,PHOTON,U=1,EMIT> (evolve pass of qed_step)",
+                                    evolve_bytes, ms_ev, step_bytes, ms)}
+    if not args.no_cpu_baseline:
+        import oracle
+        ns, steps_cpu = min(n, 1 << 21), 3
+        tabs = oracle_tables_from(w.table_params(3), [ctx.export_tables(k) for k in range(4)]).with_fp32_reads(True)
+        ph, ga = w.config3(seed=seed, n=ns)
+        tau_h = oracle.init_optical_depth(1, 0, ns, seed)
+        flds = [w.config3_fields(seed, s_, ga) for s_ in range(steps_cpu)]
+        t0 = time.perf_counter()
+        for s_ in range(steps_cpu):
+            e_, b_ = flds[s_]
+            t_ = oracle.evolve_optical_depth(tabs, 1, 0, ph, e_, b_, dt, tau_h)["tau"]
+            oracle.generate_pairs(tabs, 0, 0, ph, e_, b_, t_, seed, s_, capacity=ns // 8)
+        sec = time.perf_counter() - t0
+        leg["cpu_baseline"] = {"value": ns * steps_cpu / sec, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                               "sample": "first %d photons of the workload x %d steps (evolve + pair creation), %.1f s" % (ns, steps_cpu, sec)}
+    return leg
+
+
+def run_config5(args, torch, q, w, ctx, dev, peaks, peak_kind):
+    """BASELINE config 5: 256 Mi leptons + 64 Mi photons, fp32 with fp64 optical depth, plane wave + noise; both
+    processes per step.  The population is generated on the host in slabs of 16 Mi (seed 5 + 1000 slab: the same
+    distribution as one draw of the whole), in parallel threads."""
+    from concurrent.futures import ThreadPoolExecutor
+    scale = args.particles / float(1 << 24)             # --particles scales every configuration alike
+    n_lep, n_pho = int((1 << 28) * scale), int((1 << 26) * scale)
+    slab = min(1 << 24, n_pho)
+    seed = 5
+    pops = {}
+
+    def gen(job):
+        sp, k, m = job
+        return sp, k, w.config5(seed=seed + 1000 * k + 500 * sp, n=m, species=sp)
+
+    for sp, n_sp in ((q.LEPTON, n_lep), (q.PHOTON, n_pho)):
+        pops[sp] = [torch.empty(n_sp, dtype=torch.float32, device=dev) for _ in range(9)]
+    jobs = [(sp, k, min(slab, n_sp - k * slab)) for sp, n_sp in ((q.LEPTON, n_lep), (q.PHOTON, n_pho))
+            for k in range((n_sp + slab - 1) // slab)]
+    with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
+        for sp, k, (p_h, e_h, b_h) in ex.map(gen, jobs):
+            for a, h in zip(pops[sp], (*p_h, *e_h, *b_h)):
+                a[k * slab:k * slab + h.size].copy_(torch.from_numpy(h))
+    tau = {sp: torch.empty(pops[sp][0].numel(), dtype=torch.float64, device=dev) for sp in pops}
+    id_base = {q.LEPTON: 0, q.PHOTON: n_lep}
+    dts = []
+    for sp in pops:
+        ctx.init_optical_depth(sp, tau[sp], seed, id_base[sp])
+        m = min(pops[sp][0].numel(), 1 << 16)
+        probe = torch.zeros(m, dtype=torch.float64, device=dev)
+        ctx.evolve_optical_depth(sp, [t[:m] for t in pops[sp][:3]], [t[:m] for t in pops[sp][3:6]], [t[:m] for t in pops[sp][6:]], 1.0, probe)
+        dts.append((-probe).cpu().numpy())
+    dt = w.choose_dt(np.concatenate(dts), 0.05)        # one time step for both species (5 % rule over both)
+    cap = {sp: pops[sp][0].numel() // 4 for sp in pops}
+    sec = {sp: [[torch.empty(cap[sp], dtype=torch.float32, device=dev) for _ in range(3)] for _ in range(1 + sp)] for sp in pops}
+    sec_t = {sp: [torch.empty(cap[sp], dtype=torch.float64, device=dev) for _ in range(1 + sp)] for sp in pops}
+    n_out = {sp: torch.zeros(1, dtype=torch.int64, device=dev) for sp in pops}
+    ph = pops[q.PHOTON]
+    ph0, tau_ph0 = [t.clone() for t in ph[:3]], tau[q.PHOTON].clone()
+
+    def reseed():
+        dead = torch.isinf(tau[q.PHOTON])
+        for a, a0 in zip(ph[:3], ph0):
+            torch.where(dead, a0, a, out=a)
+        torch.where(dead, tau_ph0, tau[q.PHOTON], out=tau[q.PHOTON])
+
+    def step(s_):
+        for sp in (q.LEPTON, q.PHOTON):
+            a = pops[sp]
+            ctx.qed_step(sp, a[:3], a[3:6], a[6:], tau[sp], dt, seed, s_, id_base[sp], cap[sp], sec[sp][0], sec_t[sp][0],
+                         sec[sp][1] if sp == q.PHOTON else None, sec_t[sp][1] if sp == q.PHOTON else None, None, n_out[sp])
+
+    steps = 10 if args.steps >= 5 else args.steps
+    ms, ms_ev, ms_evt = timed_steps(torch, ctx, step, reseed, steps, min(args.warmup, 3))
+    fired = {sp: ctx.read_count(n_out[sp]) for sp in pops}
+    n = n_lep + n_pho
+    evolve_bytes = 52 * n
+    step_bytes = evolve_bytes + sum(event_bytes(sp, 4, 8, False) * fired[sp] for sp in pops)
+    leg = {"workload": "config 5: laser-plasma-like population, fp32 particles with fp64 optical depth, %d leptons + %d "
+                       "photons, plane wave a0 = 500 + noise, both processes, compaction and re-draw per step; decayed photons "
+                       "re-seeded between steps" % (n_lep, n_pho),
+           "dtype": "f32 (optical depth f64)", "value": n / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms, "steps": steps,
+           "fired_fraction_last_step": {"leptons": fired[q.LEPTON] / n_lep, "photons": fired[q.PHOTON] / n_pho}, "dt_s": dt,
+           "timing": "mean of per-step CUDA events; the re-seeding of decayed photons runs between the brackets",
+           "kernels_ms": {"evolve_passes": ms_ev, "event_passes": ms_evt},
+           "roofline": leg_roofline(peaks, peak_kind, "evolve_kernel<float,double,*,U=1,EMIT> (the two evolve passes of the step)",
+                                    evolve_bytes, ms_ev, step_bytes, ms)}
+    if not args.no_cpu_baseline:
+        import oracle
+        tabs = oracle_tables_from(w.table_params(5), [ctx.export_tables(k) for k in range(4)]).with_fp32_reads(True)
+        ns = {q.LEPTON: min(n_lep, 1 << 21), q.PHOTON: min(n_pho, 1 << 19)}
+        data = {sp: w.config5(seed=seed + 500 * sp, n=ns[sp], species=sp) for sp in ns}
+        taus = {sp: oracle.init_optical_depth(sp, 1, ns[sp], seed) for sp in ns}
+        steps_cpu = 3
+        t0 = time.perf_counter()
+        for s_ in range(steps_cpu):
+            for sp in ns:
+                p_, e_, b_ = data[sp]
+                t_ = oracle.evolve_optical_depth(tabs, sp, 1, p_, e_, b_, dt, taus[sp])["tau"]
+                (oracle.generate_photons if sp == q.LEPTON else oracle.generate_pairs)(tabs, 0, 1, p_, e_, b_, t_, seed, s_)
+        sec_cpu = time.perf_counter() - t0
+        leg["cpu_baseline"] = {"value": sum(ns.values()) * steps_cpu / sec_cpu, "unit": UNIT, "cores": oracle.num_threads(),
+                               "kind": "oracle", "sample": "%d leptons + %d photons of the same recipe x %d steps (both processes), "
+                                                           "%.1f s" % (ns[q.LEPTON], ns[q.PHOTON], steps_cpu, sec_cpu)}
+    return leg
+
+
+# FP64 instructions (warp level) of one build of the configuration-4 tables: smsp__inst_executed_pipe_fp64.sum of the two
+# table_rows_kernel launches per process, from the ncu capture named in TABLES_FP64_SOURCE
+TABLES_FP64_SOURCE = "profiles/r2_tables_full.md"
+TABLES_FP64_WARP_INST = None        # filled in from that capture; None = not measured for this build
+
+
+def run_config4(args, torch, q, w, peaks):
+    """BASELINE config 4: 4096-point lnG, lnT on [1e-4, 1e3] and 2048 x 2048 CDF tables from the Bessel quadratures.
+    The kernel is bound by the FP64 pipe: roofline = FP64 warp instructions / time against 148 SMs x 4 sub-partitions x
+    16 lanes x 1 instruction per 2 cycles... reported as the fraction of cycles the pipe could have issued"""
+    ctx = q.Context(0)
+    tp = q.TableParams(**w.table_params(4))
+    times = []
+    for _ in range(2 + 5):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ctx.build_tables(tp)
+        times.append(time.perf_counter() - t0)
+    ms = 1e3 * float(np.median(times[2:]))
+    cells = tp.rows_2d()[0] * tp.qs_n_xi + tp.rows_2d()[1] * tp.bw_n_xi
+    leg = {"workload": "config 4: table generation, fp64: 4096-point lnG and lnT on [1e-4, 1e3], two 2048 x 2048 CDF tables",
+           "dtype": "f64", "metric": "table build time", "value": ms, "unit": "ms", "higher_is_better": False,
+           "builds_timed": 5, "cells": cells, "cells_per_s": cells / (ms * 1e-3)}
+    sm_mhz = peaks.get("sm_max_mhz", 1965.0)
+    if TABLES_FP64_WARP_INST:
+        # an SM issues one FP64 warp instruction every 2 cycles per sub-partition (16 lanes each, 64 FMA per SM per cycle)
+        peak = 148 * 4 * 0.5 * sm_mhz * 1e6
+        ach = TABLES_FP64_WARP_INST / (ms * 1e-3)
+        leg["roofline"] = {"bound": "alu", "kernel": "table_rows_kernel<QS>, table_rows_kernel<BW>", "achieved": ach / 1e12,
+                           "peak": peak / 1e12, "unit": "T warp-instructions/s (FP64 pipe)", "frac": ach / peak, "traffic": None,
+                           "peak_kind": "derived: 148 SMs x 4 sub-partitions x 1 FP64 warp instruction per 2 cycles x %.0f MHz" % sm_mhz,
+                           "instruction_count_source": TABLES_FP64_SOURCE}
+    if not args.no_cpu_baseline:
+        import oracle
+        op = oracle.TableParams(**w.table_params(4))
+        rows = [0, 512, 1024, 1536, 2047]
+        t0 = time.perf_counter()
+        for r in rows:
+            oracle.build_qs_rows(op, r, r + 1)
+            oracle.build_bw_rows(op, r, r + 1)
+        sec = time.perf_counter() - t0
+        est_ms = 1e3 * sec / len(rows) * 2048      # both tables: 2048 row pairs (the 1D tables add 4096 + 4096 totals)
+        leg["cpu_baseline"] = {"value": est_ms, "unit": "ms", "cores": oracle.num_threads(), "kind": "oracle",
+                               "sample": "rows %s of both 2D tables by the oracle's adaptive quadrature, %.1f s, scaled to 2048 "
+                                         "rows per table" % (rows, sec)}
+    ctx.close()
+    return leg
 
 
 # ------------------------------------------------------------------------------------------------
@@ -297,6 +543,7 @@ def run_ours(args):
     # (SURVEY.md 8(d)); the 48-byte records it stages for the ~5 % that fire are not counted as algorithmic
     evolve_bytes = BYTES_PER_PARTICLE_EVOLVE * n
     achieved = evolve_bytes / (ms_evolve * 1e-3) / 1e9
+    step_bytes = evolve_bytes + event_bytes(0, 8, 8, True) * fired_last
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -312,14 +559,15 @@ def run_ours(args):
                      "achieved": achieved,
                      "peak": peaks["hbm_gbs"], "peak_kind": peak_kind + " (MEASURED_PEAKS.json hbm_gbs, copy)",
                      "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
-                     "traffic": EVOLVE_DRAM_TRAFFIC_BYTES, "algorithmic_bytes_per_launch": evolve_bytes,
+                     "traffic": EVOLVE_DRAM_TRAFFIC_BYTES if n == 1 << 24 else None, "traffic_source": EVOLVE_TRAFFIC_SOURCE,
+                     "algorithmic_bytes_per_launch": evolve_bytes,
                      "ms_per_launch": ms_evolve, "share_of_step": ms_evolve * args.steps / ms_total,
-                     # the whole step against the same peak: 88 B per particle + 168 B per event (48 B record written and
-                     # read back once = 96, 32 B photon + 8 B parent index, four 8-byte parent stores = 32: DESIGN.md 6)
-                     "whole_step": {"algorithmic_bytes": evolve_bytes + 168 * fired_last,
-                                    "achieved": (evolve_bytes + 168 * fired_last) / (ms_total / args.steps * 1e-3) / 1e9,
-                                    "frac": (evolve_bytes + 168 * fired_last) / (ms_total / args.steps * 1e-3) / 1e9
-                                            / peaks["hbm_gbs"]}},
+                     # the whole step against the same peak: 88 B per particle + 72 B per event (the parent's
+                     # momentum and optical depth rewritten = 32, the photon = 32, its parent index = 8; the records the two
+                     # passes exchange are the implementation's traffic, not the method's)
+                     "whole_step": {"algorithmic_bytes": step_bytes,
+                                    "achieved": step_bytes / (ms_total / args.steps * 1e-3) / 1e9,
+                                    "frac": step_bytes / (ms_total / args.steps * 1e-3) / 1e9 / peaks["hbm_gbs"]}},
         "kernels_ms": {"qed_step": {"evolve_pass": ms_evolve, "event_pass": ms_events},
                        "two_call_path": {"evolve_optical_depth": ms_evolve2, "generate_photons": ms_events2}},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -335,6 +583,22 @@ def run_ours(args):
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
                                 "sample": "first %d particles of the workload x %d steps (evolve + photon emission), "
                                           "%.1f s" % (ns, steps_cpu, sec)}
+    if world == 1 and not args.no_other_configs:
+        # the fp32 half of the metric (configs 3 and 5) and the table build (config 4), measured in the same run
+        del p, fields, tau, ph_p, ph_tau, ph_parent, p_pin, field_pin, tau_pin, p_e2e, sec_pin
+        torch.cuda.empty_cache()
+        others = []
+        for fn in (run_config3, run_config5):
+            ctx_o = q.Context(local)
+            for kv in args.opt:
+                name, value = kv.split("=")
+                ctx_o.set_option(name, int(value))
+            ctx_o.build_tables(q.TableParams(**w.table_params(3)))
+            others.append(fn(args, torch, q, w, ctx_o, dev, peaks, peak_kind))
+            ctx_o.close()
+            torch.cuda.empty_cache()
+        others.append(run_config4(args, torch, q, w, peaks))
+        line["other_configs"] = others
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -50,7 +50,7 @@ extern "C" {
 
 /* which table, for export: */
 #define PICSARQED_TAB_LNG 0    /* ln G(chi_i),           n = qs_n_chi     */
-#define PICSARQED_TAB_QS_LNP 1 /* ln P_QS[chi_n][xi_m],  n = qs_n_chi*qs_n_xi, row-major */
+#define PICSARQED_TAB_QS_LNP 1 /* ln P_QS[chi_n][xi_m],  n = rows*qs_n_xi, row-major; rows = qs_n_chi_2d or qs_n_chi */
 #define PICSARQED_TAB_LNT 2    /* ln T(chi_gamma,i),     n = bw_n_chi     */
 #define PICSARQED_TAB_BW_P 3   /* P_BW[chi_n][xi_m],     n = bw_n_chi*bw_n_xi, row-major */
 
@@ -68,6 +68,11 @@ typedef struct {
     double bw_chi_min, bw_chi_max;
     int bw_n_chi;
     int bw_n_xi;
+    /* Rows of the two 2D tables when they differ from the 1D counts above (BASELINE configuration 4: 4096-point 1D
+     * tables with 2048 x 2048 CDF tables): log-spaced on the same [chi_min, chi_max], both ends included.  0 = the same
+     * grid as the 1D table (the paper's own sets). */
+    int qs_n_chi_2d;
+    int bw_n_chi_2d;
 } picsarqed_table_params;
 
 /* ---- context ------------------------------------------------------------------------
@@ -122,8 +127,9 @@ int picsarqed_get_timing(picsarqed_ctx* ctx, double* host_ms, long long* host_ca
  *     P_QS(chi, xi) = int_0^xi S/u du / G                              (eq.18)
  * from the K_{1/3}, K_{2/3} Bessel quadratures, and stores ln T, ln G, P_BW and ln P_QS
  * in fp64 plus an fp32-rounded copy.  Synchronises.
- * rel_tol: requested relative accuracy of T, G, P (1e-9 is the design point; <= 0 = default). */
-int picsarqed_build_tables(picsarqed_ctx* ctx, const picsarqed_table_params* host_params, double rel_tol);
+ * Accuracy: fixed by the scheme (panelled 8-point Gauss-Legendre over trapezoid-rule Bessel integrals), about 1e-11
+ * relative on T, G, P against the oracle's adaptive quadrature; there is no tolerance knob.  n_xi <= 25600. */
+int picsarqed_build_tables(picsarqed_ctx* ctx, const picsarqed_table_params* host_params);
 /* Copies table `which` to host memory as fp64 (n_elems must equal the table's size).  Synchronises. */
 int picsarqed_export_tables(picsarqed_ctx* ctx, int which, double* host_dst, size_t n_elems);
 /* Replaces the tables by caller-provided values (host, fp64, layouts as above).  Synchronises. */

@@ -36,6 +36,7 @@ class _CTables(C.Structure):
         ("bw_n_xi", C.c_int),
         ("lnG", _dp), ("qs_lnP", _dp), ("lnT", _dp), ("bw_P", _dp),
         ("read_fp32", C.c_int),
+        ("qs_n_chi_2d", C.c_int), ("bw_n_chi_2d", C.c_int),   # rows of the 2D tables (0: as the 1D tables)
     ]
 
 
@@ -164,6 +165,11 @@ class TableParams:
     bw_chi_max: float = 1e3
     bw_n_chi: int = 256
     bw_n_xi: int = 256
+    qs_n_chi_2d: int = 0   # rows of the 2D tables when they are on a grid of their own (0: the grid of the 1D table)
+    bw_n_chi_2d: int = 0
+
+    def rows_2d(self):
+        return (self.qs_n_chi_2d or self.qs_n_chi, self.bw_n_chi_2d or self.bw_n_chi)
 
 
 class Tables:
@@ -172,9 +178,9 @@ class Tables:
     def __init__(self, params, lnG, qs_lnP, lnT, bw_P, read_fp32=False):
         self.params = params
         self.lnG = _f64(lnG)
-        self.qs_lnP = _f64(qs_lnP).reshape(params.qs_n_chi, params.qs_n_xi)
+        self.qs_lnP = _f64(qs_lnP).reshape(params.rows_2d()[0], params.qs_n_xi)
         self.lnT = _f64(lnT)
-        self.bw_P = _f64(bw_P).reshape(params.bw_n_chi, params.bw_n_xi)
+        self.bw_P = _f64(bw_P).reshape(params.rows_2d()[1], params.bw_n_xi)
         assert self.lnG.shape == (params.qs_n_chi,) and self.lnT.shape == (params.bw_n_chi,)
         self.read_fp32 = bool(read_fp32)
 
@@ -186,13 +192,13 @@ class Tables:
         return _CTables(p.qs_chi_min, p.qs_chi_max, p.qs_n_chi, p.qs_xi_min, p.qs_n_xi,
                         p.bw_chi_min, p.bw_chi_max, p.bw_n_chi, p.bw_n_xi,
                         _p(self.lnG), _p(self.qs_lnP), _p(self.lnT), _p(self.bw_P),
-                        int(self.read_fp32))
+                        int(self.read_fp32), p.qs_n_chi_2d, p.bw_n_chi_2d)
 
 
 def build_bw_rows(p, row0, row1, return_half=False):
     out = np.empty((row1 - row0, p.bw_n_xi))
     half = np.empty(row1 - row0)
-    lib().orc_build_bw_cdf_rows(p.bw_chi_min, p.bw_chi_max, p.bw_n_chi, p.bw_n_xi, row0, row1,
+    lib().orc_build_bw_cdf_rows(p.bw_chi_min, p.bw_chi_max, p.rows_2d()[1], p.bw_n_xi, row0, row1,
                                 _p(out), _p(half))
     return (out, half) if return_half else out
 
@@ -200,7 +206,7 @@ def build_bw_rows(p, row0, row1, return_half=False):
 def build_qs_rows(p, row0, row1, return_total=False):
     out = np.empty((row1 - row0, p.qs_n_xi))
     tot = np.empty(row1 - row0)
-    lib().orc_build_qs_cdf_rows(p.qs_chi_min, p.qs_chi_max, p.qs_n_chi, p.qs_xi_min, p.qs_n_xi,
+    lib().orc_build_qs_cdf_rows(p.qs_chi_min, p.qs_chi_max, p.rows_2d()[0], p.qs_xi_min, p.qs_n_xi,
                                 row0, row1, _p(out), _p(tot))
     return (out, tot) if return_total else out
 
@@ -218,8 +224,8 @@ def build_lnG(p):
 
 
 def build_tables(p):
-    return Tables(p, build_lnG(p), build_qs_rows(p, 0, p.qs_n_chi), build_lnT(p),
-                  build_bw_rows(p, 0, p.bw_n_chi))
+    return Tables(p, build_lnG(p), build_qs_rows(p, 0, p.rows_2d()[0]), build_lnT(p),
+                  build_bw_rows(p, 0, p.rows_2d()[1]))
 
 
 __all__ += ["build_lnT", "build_lnG"]

@@ -422,7 +422,12 @@ struct OrcTables {
     double bw_chi_min, bw_chi_max; int bw_n_chi; int bw_n_xi;
     const double* lnG; const double* qs_lnP; const double* lnT; const double* bw_P;
     int read_fp32;  // 1: every table value is read through fp32 rounding
+    // rows of the 2D tables when they sit on a chi grid of their own (0: the grid of the 1D table).  PAPER.md:203/:246 (1D)
+    // and :210/:251 (2D) define the two grids separately; BASELINE configuration 4 asks for 4096 and 2048 points.
+    int qs_n_chi_2d, bw_n_chi_2d;
 };
+static inline int qs_rows(const OrcTables* t) { return t->qs_n_chi_2d > 0 ? t->qs_n_chi_2d : t->qs_n_chi; }
+static inline int bw_rows(const OrcTables* t) { return t->bw_n_chi_2d > 0 ? t->bw_n_chi_2d : t->bw_n_chi; }
 static inline real tab(const OrcTables* t, const double* a, size_t i) {
     return t->read_fp32 ? (real)(float)a[i] : (real)a[i];
 }
@@ -505,7 +510,7 @@ static void row_bracket(real chi, real vmin, real vmax, int n, int* k_out, real*
 // eqs.28-30: xi = chi_gamma/chi of the emitted photon for uniform r
 static real qs_sample_xi(const OrcTables* t, real chi, real r) {
     int k; real w;
-    row_bracket(chi, t->qs_chi_min, t->qs_chi_max, t->qs_n_chi, &k, &w);
+    row_bracket(chi, t->qs_chi_min, t->qs_chi_max, qs_rows(t), &k, &w);
     const int M = t->qs_n_xi;
     const double* r0 = t->qs_lnP + (size_t)k * M;
     const double* r1 = r0 + M;
@@ -529,7 +534,7 @@ static real qs_sample_xi(const OrcTables* t, real chi, real r) {
 // eqs.24-26 on r' = min(r, 1-r) in [0, 1/2]: xi = chi/chi_gamma in [0, 1/2]
 static real bw_sample_xi(const OrcTables* t, real chi, real rp) {
     int k; real w;
-    row_bracket(chi, t->bw_chi_min, t->bw_chi_max, t->bw_n_chi, &k, &w);
+    row_bracket(chi, t->bw_chi_min, t->bw_chi_max, bw_rows(t), &k, &w);
     const int M = t->bw_n_xi;
     const double* r0 = t->bw_P + (size_t)k * M;
     const double* r1 = r0 + M;

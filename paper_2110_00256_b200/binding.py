@@ -28,7 +28,7 @@ class _CSpecies(C.Structure):
 class _CParams(C.Structure):
     _fields_ = [("qs_chi_min", _d), ("qs_chi_max", _d), ("qs_n_chi", _i), ("qs_xi_min", _d),
                 ("qs_n_xi", _i), ("bw_chi_min", _d), ("bw_chi_max", _d), ("bw_n_chi", _i),
-                ("bw_n_xi", _i)]
+                ("bw_n_xi", _i), ("qs_n_chi_2d", _i), ("bw_n_chi_2d", _i)]
 
 
 @dataclass
@@ -43,13 +43,19 @@ class TableParams:
     bw_chi_max: float = 1e3
     bw_n_chi: int = 256
     bw_n_xi: int = 256
+    qs_n_chi_2d: int = 0      # rows of the 2D tables when they differ from the 1D counts (0 = the same grid)
+    bw_n_chi_2d: int = 0
 
     def _c(self):
         return _CParams(self.qs_chi_min, self.qs_chi_max, self.qs_n_chi, self.qs_xi_min, self.qs_n_xi,
-                        self.bw_chi_min, self.bw_chi_max, self.bw_n_chi, self.bw_n_xi)
+                        self.bw_chi_min, self.bw_chi_max, self.bw_n_chi, self.bw_n_xi, self.qs_n_chi_2d, self.bw_n_chi_2d)
+
+    def rows_2d(self):
+        return (self.qs_n_chi_2d or self.qs_n_chi, self.bw_n_chi_2d or self.bw_n_chi)
 
     def sizes(self):
-        return (self.qs_n_chi, self.qs_n_chi * self.qs_n_xi, self.bw_n_chi, self.bw_n_chi * self.bw_n_xi)
+        rq, rb = self.rows_2d()
+        return (self.qs_n_chi, rq * self.qs_n_xi, self.bw_n_chi, rb * self.bw_n_xi)
 
 
 _SIGNATURES = {
@@ -61,7 +67,7 @@ _SIGNATURES = {
     "picsarqed_set_units": (_i, [_vp, _i, _d]),
     "picsarqed_get_unit_scales": (_i, [_vp, C.POINTER(_d)]),
     "picsarqed_get_timing": (_i, [_vp, C.POINTER(_d), C.POINTER(_i64)]),
-    "picsarqed_build_tables": (_i, [_vp, C.POINTER(_CParams), _d]),
+    "picsarqed_build_tables": (_i, [_vp, C.POINTER(_CParams)]),
     "picsarqed_export_tables": (_i, [_vp, _i, _vp, C.c_size_t]),
     "picsarqed_import_tables": (_i, [_vp, C.POINTER(_CParams), _vp, _vp, _vp, _vp]),
     "picsarqed_chi": (_i, [_vp, _i, _i, _i64] + [_vp] * 10),
@@ -163,9 +169,9 @@ class Context:
         self._check(lib().picsarqed_get_timing(self._h, ms, C.byref(calls)))
         return float(ms[0]), float(ms[1]), int(calls.value)
 
-    def build_tables(self, params, rel_tol=0.0):
+    def build_tables(self, params):
         cp = params._c()
-        self._check(lib().picsarqed_build_tables(self._h, C.byref(cp), float(rel_tol)))
+        self._check(lib().picsarqed_build_tables(self._h, C.byref(cp)))
         self.params = params
 
     def import_tables(self, params, lnG, qs_lnP, lnT, bw_P):
@@ -183,9 +189,9 @@ class Context:
         self._check(lib().picsarqed_export_tables(self._h, which, out.ctypes.data, n))
         p = self.params
         if which == TAB_QS_LNP:
-            return out.reshape(p.qs_n_chi, p.qs_n_xi)
+            return out.reshape(p.rows_2d()[0], p.qs_n_xi)
         if which == TAB_BW_P:
-            return out.reshape(p.bw_n_chi, p.bw_n_xi)
+            return out.reshape(p.rows_2d()[1], p.bw_n_xi)
         return out
 
     # ---- runtime calls (device tensors) ---------------------------------------------------

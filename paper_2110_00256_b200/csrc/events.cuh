@@ -156,12 +156,13 @@ __device__ __forceinline__ double event_c2(double px, double py, double pz, doub
 
 template <typename R, typename TR, int KIND>
 __device__ __forceinline__ void event_commit(const EventArgs<R, TR>& a, long long i, long long slot,
-                                             const EventOut<R, TR>& o) {
+                                             const EventOut<R, TR>& o, bool parent_done = false) {
 #pragma unroll
     for (int c = 0; c < (KIND == 0 ? 3 : 6); ++c) a.out_p[c][slot] = o.sec[c];
     a.out_tau[0][slot] = o.sec_tau[0];
     if (KIND == 1) a.out_tau[1][slot] = o.sec_tau[1];
     if (a.parent) a.parent[slot] = a.parent_base + i;
+    if (parent_done) return;   // (a photon the evolve pass removed itself)
 #pragma unroll
     for (int c = 0; c < 3; ++c) a.p[c][i] = o.parent_p[c];
     a.tau[i] = o.parent_tau;
@@ -329,6 +330,7 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
     const unsigned int rescan_mask =
         __ballot_sync(0xffffffffu, cnt > 0 && (cnt > (unsigned)kStageCap || (flags & kStageNoRecords) != 0));
     const unsigned int done_mask = __ballot_sync(0xffffffffu, cnt > 0 && (flags & kStageDone) != 0);
+    const unsigned int pdone_mask = __ballot_sync(0xffffffffu, cnt > 0 && (flags & kStageParentDone) != 0);
     if (rescan_mask) {  // chunks without records: find their fired particles again (tau < 0), in index order
         __syncthreads();  // (every warp is done with the list of the previous tile that needed one)
         for (int j = warp; j < CHUNKS; j += WARPS) {
@@ -383,7 +385,8 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
             }
             continue;
         }
-        if (slot >= a.capacity) continue;  // capacity rule (R16): later parents untouched
+        const bool pdone = (pdone_mask >> j) & 1u;
+        if (slot >= a.capacity && !pdone) continue;  // capacity rule (R16): later parents untouched
         const bool staged = !((rescan_mask >> j) & 1u);
         double px, py, pz, c2;
         long long i;
@@ -393,6 +396,13 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
             union { uint4 raw[StageRecord<R>::kVecs]; StageRecord<R> rec; } u;
 #pragma unroll
             for (int k = 0; k < StageRecord<R>::kVecs; ++k) u.raw[k] = __ldg(src + k);
+            if (slot >= a.capacity) {   // (pdone) the evolve pass removed this photon already: put it back as it left it
+                const long long ib = cbase + u.rec.idx;
+#pragma unroll
+                for (int c = 0; c < 3; ++c) a.p[c][ib] = u.rec.p[c];
+                a.tau[ib] = (TR)u.rec.tau_ev;
+                continue;
+            }
             const double sp = a.units.p;
             px = u.rec.p[0] * sp; py = u.rec.p[1] * sp; pz = u.rec.p[2] * sp;   // (records hold the caller's units)
             c2 = u.rec.c2;
@@ -406,7 +416,7 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
         }
         const EventOut<R, TR> out = KIND == 0 ? qs_event_compute<R, TR>(a, i, px, py, pz, c2)
                                               : bw_event_compute<R, TR>(a, i, px, py, pz, c2);
-        event_commit<R, TR, KIND>(a, i, slot, out);
+        event_commit<R, TR, KIND>(a, i, slot, out, pdone);
     }
     }  // tiles
 #undef PXQ_TILE_OF

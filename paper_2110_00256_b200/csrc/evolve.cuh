@@ -45,9 +45,12 @@ constexpr int kStageCap = 24;               // records per chunk segment (mean a
 // records (segment overflow, or counted by count_chunks_kernel: generate_* calls and the ragged last tile)
 // bit 14 = the events of the chunk have been generated already (fused step, step.cuh): its segment holds StepResult
 // records -- the secondaries, waiting for their slots
-constexpr unsigned short kStageCountMask = 0x3FFFu;
+// bit 13 = the chunk's records are those of photons the evolve pass has removed already (p = 0, tau = +inf written with
+// its own stores, while the sectors were in L2): the event pass only creates the pairs
+constexpr unsigned short kStageCountMask = 0x1FFFu;
 constexpr unsigned short kStageNoRecords = 0x8000u;
 constexpr unsigned short kStageDone = 0x4000u;
+constexpr unsigned short kStageParentDone = 0x2000u;
 
 // one staged record: what event generation needs of a particle that fired -- its momentum, chi^2 (computed by the
 // evolve pass anyway) and its index inside the chunk.  Sizes are multiples of 16 bytes so that records move as
@@ -56,12 +59,13 @@ constexpr unsigned short kStageDone = 0x4000u;
 // bytes for the capacity rule -- were measured: the first made the evolve pass slower by more than the event pass
 // gained; the last gave evolve +12 us, events -16 us: 1 % of the step for 5 points of the evolve pass's HBM fraction.)
 template <typename R> struct StageRecord;
+// tau_ev: the evolved optical depth (what undoes a removed photon that falls beyond the capacity of the output)
 template <> struct alignas(16) StageRecord<double> {
-    double p[3]; double c2; unsigned idx; unsigned pad[3];
+    double p[3]; double c2; unsigned idx; unsigned pad; double tau_ev;
     static constexpr int kBytes = 48, kVecs = 3;
 };
 template <> struct alignas(16) StageRecord<float> {
-    float p[3]; unsigned idx; double c2; double pad;
+    float p[3]; unsigned idx; double c2; double tau_ev;
     static constexpr int kBytes = 32, kVecs = 2;
 };
 static_assert(sizeof(StageRecord<double>) == 48 && sizeof(StageRecord<float>) == 32, "record layout");
@@ -339,7 +343,9 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                 }
                 const long long chunk = (base + (long long)warp * WCH) / kChunk;
                 if (lane == 0) {
-                    a.stage_cnt[chunk] = (unsigned short)(total <= (unsigned)kStageCap ? total : (total | kStageNoRecords));
+                    a.stage_cnt[chunk] = (unsigned short)(total <= (unsigned)kStageCap
+                                                              ? (SPECIES == 1 && total > 0 ? (total | kStageParentDone) : total)
+                                                              : (total | kStageNoRecords));
                     if (total > 0) atomicAdd(a.tile_sum + chunk / a.chunks_per_tile, total);
                 }
                 if (total > 0 && total <= (unsigned)kStageCap) {  // (overflow: the event kernel re-scans the chunk)
@@ -358,7 +364,30 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                                 rec.p[2] = q[2][u].v[v];
                                 rec.c2 = c2s[u * V + v];
                                 rec.idx = (unsigned)((u * 32 + lane) * V + v);
+                                rec.tau_ev = (double)t[u].v[v];
                                 ++r;
+                            }
+                        }
+                    }
+                    if constexpr (SPECIES == 1) {
+                        // a photon that decays is removed whatever the split of its energy: p = 0, tau = +inf
+                        // go out from here, with the stores of the evolve pass and while the momentum sectors are in L2 --
+                        // the event pass has no scattered store left (it undoes this for events beyond the capacity)
+#pragma unroll
+                        for (int u = 0; u < U; ++u) {
+                            if ((fired_bits >> (u * V)) & ((1u << V) - 1u)) {
+                                const long long i = base + (long long)warp * WCH + (u * 32 + lane) * V;
+#pragma unroll
+                                for (int c = 0; c < 3; ++c) {
+                                    Vec<R, V> z = q[c][u];
+#pragma unroll
+                                    for (int v = 0; v < V; ++v)
+                                        if ((fired_bits >> (u * V + v)) & 1u) z.v[v] = (R)0;
+                                    st_vec<R, V>(const_cast<R*>(a.p[c]) + i, z);
+                                }
+#pragma unroll
+                                for (int v = 0; v < V; ++v)
+                                    if ((fired_bits >> (u * V + v)) & 1u) t[u].v[v] = (TR)INFINITY;
                             }
                         }
                     }

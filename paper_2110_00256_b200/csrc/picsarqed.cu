@@ -82,6 +82,8 @@ struct picsarqed_ctx {
     unsigned long long* d_cas = nullptr;  // 16 counters
     unsigned long long* h_cas = nullptr;
     double build_ms = 0.0;
+    cudaStream_t aux_stream = nullptr;       // build_tables: the second process
+    cudaEvent_t aux_event[2] = {nullptr, nullptr};
 };
 
 namespace {
@@ -99,17 +101,23 @@ int fail(picsarqed_ctx* c, int code, const std::string& msg) {
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+// rows of the 2D tables (0 in the params = the 1D count)
+int rows_2d(const picsarqed_table_params& p, int kind) {
+    const int r = kind == 0 ? p.qs_n_chi_2d : p.bw_n_chi_2d;
+    return r > 0 ? r : (kind == 0 ? p.qs_n_chi : p.bw_n_chi);
+}
+
 bool params_ok(const picsarqed_table_params* p) {
-    return p && p->qs_n_chi >= 2 && p->qs_n_xi >= 2 && p->bw_n_chi >= 2 && p->bw_n_xi >= 2 &&
+    return p && (p->qs_n_chi_2d == 0 || p->qs_n_chi_2d >= 2) && (p->bw_n_chi_2d == 0 || p->bw_n_chi_2d >= 2) && p->qs_n_chi >= 2 && p->qs_n_xi >= 2 && p->bw_n_chi >= 2 && p->bw_n_xi >= 2 &&
            p->qs_chi_min > 0 && p->qs_chi_max > p->qs_chi_min && p->bw_chi_min > 0 &&
            p->bw_chi_max > p->bw_chi_min && p->qs_xi_min > 0 && p->qs_xi_min < 1;
 }
 
 void table_sizes(const picsarqed_table_params& p, size_t n[4]) {
     n[0] = (size_t)p.qs_n_chi;
-    n[1] = (size_t)p.qs_n_chi * p.qs_n_xi;
+    n[1] = (size_t)rows_2d(p, 0) * p.qs_n_xi;
     n[2] = (size_t)p.bw_n_chi;
-    n[3] = (size_t)p.bw_n_chi * p.bw_n_xi;
+    n[3] = (size_t)rows_2d(p, 1) * p.bw_n_xi;
 }
 
 __global__ void narrow_kernel(const double* __restrict__ src, float* __restrict__ dst, size_t n) {
@@ -183,7 +191,7 @@ int build_guides(picsarqed_ctx* c) {
     for (int kind = 0; kind < 2; ++kind) {
         if (c->guide[kind]) cudaFree(c->guide[kind]);
         c->guide[kind] = nullptr;
-        const int rows = kind == 0 ? c->tp.qs_n_chi : c->tp.bw_n_chi, cols = kind == 0 ? c->tp.qs_n_xi : c->tp.bw_n_xi;
+        const int rows = rows_2d(c->tp, kind), cols = kind == 0 ? c->tp.qs_n_xi : c->tp.bw_n_xi;
         if (cols > 65535) continue;  // indices are stored in 16 bits; wider tables are searched unguided
         const double* tab = c->tab64[kind == 0 ? PICSARQED_TAB_QS_LNP : PICSARQED_TAB_BW_P];
         double k0 = 0.0, k1 = 0.5;
@@ -229,7 +237,7 @@ Table2D<R> view_2d(const picsarqed_ctx* c, int species) {
     Table2D<R> t;
     const auto& p = c->tp;
     const double lo = species == 0 ? p.qs_chi_min : p.bw_chi_min, hi = species == 0 ? p.qs_chi_max : p.bw_chi_max;
-    t.n_chi = species == 0 ? p.qs_n_chi : p.bw_n_chi;
+    t.n_chi = rows_2d(p, species);
     t.n_xi = species == 0 ? p.qs_n_xi : p.bw_n_xi;
     t.P = table_ptr<R>(c, species == 0 ? PICSARQED_TAB_QS_LNP : PICSARQED_TAB_BW_P);
     t.ln_min = std::log(lo);
@@ -324,6 +332,8 @@ int picsarqed_destroy(picsarqed_ctx* c) {
     cudaFree(c->d_cas);
     cudaFreeHost(c->h_cas);
     for (cudaEvent_t e : c->slab_events) cudaEventDestroy(e);
+    if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
+    for (int k = 0; k < 2; ++k) if (c->aux_event[k]) cudaEventDestroy(c->aux_event[k]);
     if (c->h2d_stream) cudaStreamDestroy(c->h2d_stream);
     if (c->d2h_stream) cudaStreamDestroy(c->d2h_stream);
     delete c;
@@ -1154,35 +1164,59 @@ extern "C" int picsarqed_step_host(picsarqed_ctx* c, int species, int dtype, int
     return PICSARQED_OK;
 }
 
-extern "C" int picsarqed_build_tables(picsarqed_ctx* c, const picsarqed_table_params* p, double rel_tol) {
+extern "C" int picsarqed_build_tables(picsarqed_ctx* c, const picsarqed_table_params* p) {
     if (!c) return PICSARQED_ERR_INVALID;
     if (!params_ok(p)) return fail(c, PICSARQED_ERR_INVALID, "bad table parameters");
-    if (rel_tol > 0 && rel_tol < 1e-10)
-        return fail(c, PICSARQED_ERR_INVALID, "rel_tol below the builder's design accuracy (1e-10)");
     if ((size_t)std::max(p->qs_n_xi, p->bw_n_xi) * sizeof(double) > 200 * 1024)
         return fail(c, PICSARQED_ERR_INVALID, "n_xi too large for the row builder (max 25600)");
     PXQ_CUDA(c, cudaSetDevice(c->device));
     c->have_tables = false;
     if (int rc = alloc_tables(c, *p)) return rc;
+    // The two processes are independent: they are built on two streams, so that a small table set (256 rows each for 148
+    // SMs) fills the GPU.  A 2D table with its own row count is a second launch of the same kernel: rows without the 1D
+    // value, then the 1D values without rows.
+    if (!c->aux_stream) PXQ_CUDA(c, cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking));
+    if (!c->aux_event[0])
+        for (int k = 0; k < 2; ++k) PXQ_CUDA(c, cudaEventCreateWithFlags(&c->aux_event[k], cudaEventDisableTiming));
+    PXQ_CUDA(c, cudaEventRecord(c->aux_event[0], c->stream));            // (the tables were just cleared on c->stream)
+    PXQ_CUDA(c, cudaStreamWaitEvent(c->aux_stream, c->aux_event[0], 0));
     for (int kind = 0; kind < 2; ++kind) {
+        cudaStream_t st = kind == 0 ? c->stream : c->aux_stream;
+        const int n1 = kind == 0 ? p->qs_n_chi : p->bw_n_chi, n2 = rows_2d(*p, kind);
         TableBuildArgs a;
         a.chi_min = kind == 0 ? p->qs_chi_min : p->bw_chi_min;
         a.chi_max = kind == 0 ? p->qs_chi_max : p->bw_chi_max;
-        a.n_chi = kind == 0 ? p->qs_n_chi : p->bw_n_chi;
         a.n_xi = kind == 0 ? p->qs_n_xi : p->bw_n_xi;
         a.xi_min = p->qs_xi_min;
-        a.rows = c->tab64[kind == 0 ? PICSARQED_TAB_QS_LNP : PICSARQED_TAB_BW_P];
-        a.ln1d = c->tab64[kind == 0 ? PICSARQED_TAB_LNG : PICSARQED_TAB_LNT];
+        double* rows = c->tab64[kind == 0 ? PICSARQED_TAB_QS_LNP : PICSARQED_TAB_BW_P];
+        double* ln1d = c->tab64[kind == 0 ? PICSARQED_TAB_LNG : PICSARQED_TAB_LNT];
         const size_t smem = (size_t)a.n_xi * sizeof(double);
-        if (kind == 0) {
-            if (smem > 48 * 1024) PXQ_CUDA(c, cudaFuncSetAttribute(table_rows_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            table_rows_kernel<0><<<a.n_chi, kTabThreads, smem, c->stream>>>(a);
+        auto launch = [&](int n_chi, double* r, double* l) -> cudaError_t {
+            a.n_chi = n_chi;
+            a.rows = r;
+            a.ln1d = l;
+            if (kind == 0) {
+                if (smem > 48 * 1024) cudaFuncSetAttribute(table_rows_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+                table_rows_kernel<0><<<n_chi, kTabThreads, smem, st>>>(a);
+            } else {
+                if (smem > 48 * 1024) cudaFuncSetAttribute(table_rows_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+                table_rows_kernel<1><<<n_chi, kTabThreads, smem, st>>>(a);
+            }
+            return cudaGetLastError();
+        };
+        if (n1 == n2) {
+            PXQ_CUDA(c, launch(n1, rows, ln1d));
         } else {
-            if (smem > 48 * 1024) PXQ_CUDA(c, cudaFuncSetAttribute(table_rows_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            table_rows_kernel<1><<<a.n_chi, kTabThreads, smem, c->stream>>>(a);
+            PXQ_CUDA(c, launch(n2, rows, nullptr));
+            // the 1D values alone: the row total does not need the table's columns -- the cell routines cut every cell
+            // into panels over which the integrand varies by a bounded factor, so 64 wide cells cost a thirtieth of 2048
+            // narrow ones and give the same integral (to ~1e-12; the two differ only in where the panels end)
+            a.n_xi = std::min(a.n_xi, 64);
+            PXQ_CUDA(c, launch(n1, nullptr, ln1d));
         }
-        PXQ_CUDA(c, cudaGetLastError());
     }
+    PXQ_CUDA(c, cudaEventRecord(c->aux_event[1], c->aux_stream));
+    PXQ_CUDA(c, cudaStreamWaitEvent(c->stream, c->aux_event[1], 0));
     if (int rc = narrow_tables(c)) return rc;
     if (int rc = build_guides(c)) return rc;
     PXQ_CUDA(c, cudaStreamSynchronize(c->stream));

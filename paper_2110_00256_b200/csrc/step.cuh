@@ -287,6 +287,7 @@ __global__ void __launch_bounds__((SW + EW) * 32, 1) step_kernel(const StepArgs<
                             g->p[2] = q[2].v[v];
                             g->c2 = c2s[v];
                             g->idx = idx;
+                            g->tau_ev = (double)t.v[v];
                         }
                         ++r;
                     }

@@ -165,8 +165,8 @@ struct TableBuildArgs {
     double chi_min, chi_max;
     int n_chi, n_xi;
     double xi_min;   // QS only
-    double* rows;    // n_chi * n_xi: ln P_QS or P_BW
-    double* ln1d;    // n_chi: ln G or ln T
+    double* rows;    // n_chi * n_xi: ln P_QS or P_BW (NULL: only the 1D values are wanted)
+    double* ln1d;    // n_chi: ln G or ln T (NULL: only the rows are wanted)
 };
 
 __device__ __forceinline__ double log_grid(double vmin, double vmax, int n, int i) {
@@ -250,9 +250,11 @@ __global__ void __launch_bounds__(kTabThreads) table_rows_kernel(const TableBuil
     double floor_v = __shfl_up_sync(0xffffffffu, wm, 1);
     if (lane == 0) floor_v = -INFINITY;
     for (int w = 0; w < warp; ++w) floor_v = fmax(floor_v, warp_tot[w]);
-    double* out = a.rows + (size_t)row * M;
-    for (int m = lo; m < hi; ++m) out[m] = fmax(cell[m], floor_v);
-    if (tid == 0) {
+    if (a.rows != nullptr) {
+        double* out = a.rows + (size_t)row * M;
+        for (int m = lo; m < hi; ++m) out[m] = fmax(cell[m], floor_v);
+    }
+    if (tid == 0 && a.ln1d != nullptr) {
         if (KIND == 0) a.ln1d[row] = log(total);                                             // ln G
         else a.ln1d[row] = log(total / (kPi * 1.7320508075688772 * chi)) - 8.0 / (3.0 * chi);  // ln T (eq.9)
     }

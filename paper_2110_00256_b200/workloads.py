@@ -40,7 +40,7 @@ def table_params(config):
                     bw_chi_min=1e-2, bw_chi_max=1e3, bw_n_chi=1024, bw_n_xi=1024)
     if config == 4:
         return dict(qs_chi_min=1e-4, qs_chi_max=1e3, qs_n_chi=4096, qs_xi_min=1e-12, qs_n_xi=2048,
-                    bw_chi_min=1e-4, bw_chi_max=1e3, bw_n_chi=4096, bw_n_xi=2048)
+                    bw_chi_min=1e-4, bw_chi_max=1e3, bw_n_chi=4096, bw_n_xi=2048, qs_n_chi_2d=2048, bw_n_chi_2d=2048)
     raise ValueError(config)
 
 

@@ -235,6 +235,73 @@ def test_events(orc, qed, ctx, mid_tables, species, dtype, tdtype):
 
 
 @pytest.mark.parametrize("species", [LEPTON, PHOTON])
+def test_events_with_2d_tables_on_their_own_row_grid(orc, qed, species):
+    """picsarqed_table_params.qs_n_chi_2d / bw_n_chi_2d (BASELINE config 4's shape): the 1D lookups use the 1D grid, the
+    row interpolation of eq.24/28 the 2D grid; GPU-built tables, their bytes given to the oracle"""
+    kw = dict(qs_chi_min=1e-3, qs_chi_max=1e3, qs_n_chi=64, qs_xi_min=1e-12, qs_n_xi=72,
+              bw_chi_min=2e-2, bw_chi_max=1e3, bw_n_chi=48, bw_n_xi=56, qs_n_chi_2d=23, bw_n_chi_2d=31)
+    c = qed.Context(0)
+    c.build_tables(qed.TableParams(**kw))
+    tabs = orc.Tables(orc.TableParams(**kw), c.export_tables(qed.TAB_LNG), c.export_tables(qed.TAB_QS_LNP),
+                      c.export_tables(qed.TAB_LNT), c.export_tables(qed.TAB_BW_P))
+    n = 2 * 4096 + 321
+    p, e, b = qed.workloads.config1(seed=14, n=n, species=species, dtype=np.float64)
+    dt = _dt_for(orc, qed, tabs, species, p, e, b)
+    tau0 = orc.init_optical_depth(species, F64, n, 3)
+    import torch
+    dtau = torch.from_numpy(tau0.copy()).cuda()
+    c.evolve_optical_depth(species, to_dev(p), to_dev(e), to_dev(b), 3 * dt, dtau)
+    o = orc.evolve_optical_depth(tabs, species, F64, p, e, b, 3 * dt, tau0)
+    ln_chi = np.log(np.maximum(orc.chi(species, p, e, b), 1e-300))
+    tau_mid = dtau.cpu().numpy()
+    check_evolve(tau_mid, tau0, o, np.float64, ln_chi)
+    g, oe = _run_events(orc, qed, c, tabs, species, np.float64, np.float64, p, e, b, tau_mid, 5, 1, 77, n)
+    assert oe["n_fired"] > 200
+    _compare_events(g, oe, species, np.float64, np.float64, n, p)
+    c.close()
+
+
+@pytest.mark.parametrize("species", [LEPTON, PHOTON])
+@pytest.mark.parametrize("dtype,tdtype", DTYPES, ids=IDS)
+def test_views_offset_by_16_bytes(orc, qed, ctx, mid_tables, species, dtype, tdtype):
+    """the ABI asks for 16-byte alignment only: every array is a view that starts 16 bytes into its allocation
+    (fp32 particles with an fp64 optical depth used to store tau with one 256-bit instruction)"""
+    import torch
+    n = 3 * 4096 + 50
+    off_p = 16 // np.dtype(dtype).itemsize
+    off_t = 16 // np.dtype(tdtype).itemsize
+    p, e, b = qed.workloads.config1(seed=15, n=n, species=species, dtype=dtype)
+    tables = _tables_for(mid_tables, dtype)
+    dt = 2 * _dt_for(orc, qed, tables, species, p, e, b)
+
+    def view(a, off):
+        buf = torch.zeros(a.size + off + 8, dtype=torch.from_numpy(a[:1]).dtype, device="cuda")
+        v = buf[off:off + a.size]
+        v.copy_(torch.from_numpy(np.ascontiguousarray(a)))
+        assert v.data_ptr() % 32 == 16
+        return v
+
+    tau0 = orc.init_optical_depth(species, code(tdtype), n, 9).astype(tdtype)
+    for fused in (False, True):
+        dp, de, db = [view(a, off_p) for a in p], [view(a, off_p) for a in e], [view(a, off_p) for a in b]
+        dtau = view(tau0, off_t)
+        nsec = 1 if species == LEPTON else 2
+        sec_p = [[view(np.zeros(n, dtype), off_p) for _ in range(3)] for _ in range(nsec)]
+        sec_t = [view(np.zeros(n, tdtype), off_t) for _ in range(nsec)]
+        n_out = torch.zeros(1, dtype=torch.int64, device="cuda")
+        if fused:
+            ctx.qed_step(species, dp, de, db, dtau, dt, 1, 0, 0, n, sec_p[0], sec_t[0], sec_p[1] if nsec == 2 else None,
+                         sec_t[1] if nsec == 2 else None, None, n_out)
+            k = ctx.read_count(n_out)
+            assert k == int((tau_mid < 0).sum())
+        else:
+            ctx.evolve_optical_depth(species, dp, de, db, dt, dtau)
+            tau_mid = dtau.cpu().numpy()
+            o = orc.evolve_optical_depth(tables, species, code(tdtype), p, e, b, dt, tau0)
+            check_evolve(tau_mid, tau0.astype(np.float64), o, dtype, np.log(np.maximum(orc.chi(species, p, e, b), 1e-300)))
+
+
+@pytest.mark.parametrize("species", [LEPTON, PHOTON])
 def test_events_capacity_rule(orc, qed, ctx, mid_tables, species):
     """only the first `capacity` fired parents are processed; the rest keep tau < 0"""
     n = 2 * 4096 + 77

@@ -33,10 +33,12 @@ def _check_rows(orc, qed, ctx, kw, rows_qs, rows_bw, one_d_idx):
     for r in rows_bw:
         ref = orc.build_bw_rows(op, r, r + 1)[0]
         assert np.all(np.abs(bw[r] - ref) <= TOL * ref + 1e-300), ("bw row", r)
+    same_grid = op.rows_2d()[0] == op.qs_n_chi
     for r in rows_qs:
         ref, tot = orc.build_qs_rows(op, r, r + 1, return_total=True)
         assert np.all(np.abs(qs[r] - ref[0]) <= TOL), ("qs row", r)
-        assert abs(lnG[r] - np.log(tot[0])) <= TOL
+        if same_grid:
+            assert abs(lnG[r] - np.log(tot[0])) <= TOL
     chi_bw = _chi_grid(kw["bw_chi_min"], kw["bw_chi_max"], kw["bw_n_chi"])
     chi_qs = _chi_grid(kw["qs_chi_min"], kw["qs_chi_max"], kw["qs_n_chi"])
     for i in one_d_idx:
@@ -79,15 +81,37 @@ def test_config1_tables(orc, qed):
 
 
 def test_config4_tables(orc, qed):
-    """BASELINE config 4: 4096-point ln G / ln T on [1e-4, 1e3], 2048-column CDF tables (here with all 4096 rows)"""
+    """BASELINE config 4: 4096-point ln G / ln T on [1e-4, 1e3] and 2048 x 2048 CDF tables (their own row grid): every
+    64th row of both 2D tables (and the last) and every 64th 1D node (and the last) against the oracle quadrature"""
     kw = qed.workloads.table_params(4)
     ctx = qed.Context(0)
     ctx.build_tables(qed.TableParams(**kw))
-    lnG, lnT, qs, bw = _check_rows(orc, qed, ctx, kw, [0, 1500, 4095], [0, 777, 2600, 4095], [0, 1, 2047, 4094, 4095])
+    assert ctx.export_tables(qed.TAB_QS_LNP).shape == (2048, 2048) and ctx.export_tables(qed.TAB_LNG).shape == (4096,)
+    rows = list(range(0, 2048, 64)) + [2047]
+    nodes = list(range(0, 4096, 64)) + [1, 4094, 4095]
+    lnG, lnT, qs, bw = _check_rows(orc, qed, ctx, kw, rows, rows, nodes)
     # pins of the paper/mathematics on the GPU tables themselves: T e^{8/(3 chi)} -> 3 sqrt3/(16 sqrt2) (chi -> 0),
     # G/chi -> 5 sqrt3/4 (chi -> 0)  [SURVEY.md 8(c) P3]
     assert abs(np.exp(lnT[0] + 8 / (3 * 1e-4)) / 0.2296396634 - 1) < 2e-4
     assert abs(np.exp(lnG[0]) / 1e-4 / 2.1650635095 - 1) < 2e-4
+    ctx.close()
+
+
+def test_own_row_grid_matches_shared_grid(qed):
+    """a 2D table with its own row count holds the rows a table built on that grid alone would hold, bit for bit, and
+    the 1D values are those of the 1D grid"""
+    base = dict(qs_chi_min=1e-3, qs_chi_max=1e3, qs_xi_min=1e-9, qs_n_xi=33, bw_chi_min=2e-2, bw_chi_max=1e3, bw_n_xi=29)
+    ctx = qed.Context(0)
+    ctx.build_tables(qed.TableParams(qs_n_chi=21, bw_n_chi=17, qs_n_chi_2d=9, bw_n_chi_2d=11, **base))
+    mixed = [ctx.export_tables(k) for k in range(4)]
+    ctx.build_tables(qed.TableParams(qs_n_chi=21, bw_n_chi=17, **base))
+    one_d = [ctx.export_tables(k) for k in range(4)]
+    ctx.build_tables(qed.TableParams(qs_n_chi=9, bw_n_chi=11, **base))
+    two_d = [ctx.export_tables(k) for k in range(4)]
+    assert mixed[1].shape == (9, 33) and mixed[3].shape == (11, 29)
+    # (1D values alone are integrated over at most 64 wide cells: the same integral, other panel ends)
+    assert np.allclose(mixed[0], one_d[0], rtol=0, atol=1e-11) and np.allclose(mixed[2], one_d[2], rtol=0, atol=1e-11)
+    assert np.array_equal(mixed[1], two_d[1]) and np.array_equal(mixed[3], two_d[3])
     ctx.close()
 
 

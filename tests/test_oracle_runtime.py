@@ -383,6 +383,19 @@ def test_row_interpolation_weight_is_linear_in_ln_chi(orc):
         assert orc.bw_sample_xi(t, chi, rp) == pytest.approx(0.5 * (4 + 0.7) / 8, abs=1e-13)
 
 
+def test_row_interpolation_on_a_row_grid_of_its_own(orc):
+    """2D tables whose rows sit on another chi grid than the 1D tables (BASELINE config 4: 4096 and 2048 points): the
+    row bracket uses the 2D grid -- the same closed forms hold with 9 (QS) / 7 (BW) 1D points over 5 rows"""
+    t, a_of, c_of = _row_dependent_tables(orc)
+    p = orc.TableParams(**dict(t.params.__dict__, qs_n_chi=9, bw_n_chi=7, qs_n_chi_2d=5, bw_n_chi_2d=5))
+    t2 = orc.Tables(p, np.zeros(9), t.qs_lnP, np.zeros(7), t.bw_P)
+    for chi in (0.013, 2.7, 31.0):
+        assert orc.qs_sample_xi(t2, chi, 0.4) == pytest.approx(0.4 ** (1 / a_of(math.log(chi))), rel=1e-12)
+        assert orc.qs_sample_xi(t2, chi, 0.4) == orc.qs_sample_xi(t, chi, 0.4)
+    for chi in (0.17, 40.0):
+        assert orc.bw_sample_xi(t2, chi, 0.21) == orc.bw_sample_xi(t, chi, 0.21)
+
+
 def test_row_interpolation_between_rows_of_a_built_table(orc):
     """at chi strictly between two closely spaced rows of an oracle-built table, the sampled xi has the exact CDF
     value r (eq.11 / eq.18 by quadrature at THAT chi) up to the interpolation error of the table"""
