@@ -1,7 +1,7 @@
 """BASELINE.json configurations on the GPU, at full size where the oracle can follow on samples.
 
 * config 1: every element (65 536 leptons + 65 536 photons, fp64, 256 / 256x256 tables).
-* config 2 (the one bench.py times), config 3, config 5 (full size; 1/8 of it with PICSARQED_SMALL_C5=1): the launch
+* config 2 (the one bench.py times), config 3, config 5 (an eighth of it; full size with PICSARQED_FULL_C5=1): the launch
   configuration of bench.py (picsarqed_qed_step on the whole population, GPU-built tables exported to the oracle),
   checked on sampled particles the oracle recomputes one by one, plus properties that hold at any size: ascending
   parent list, count = number of negative optical depths, energy conservation of every event, nothing touched
@@ -231,10 +231,10 @@ def test_config3_pair_production_fp32(orc, qed):
 
 def test_config5_mixed_precision(orc, qed):
     """BASELINE config 5: fp32 particles with fp64 optical depth, laser-plasma-like fields, both species.
-    Full size by default: 256 Mi leptons + 64 Mi photons (about 75 s, 10 GB of host arrays); PICSARQED_SMALL_C5=1
-    runs 1/8 of it."""
+    An eighth of the size by default (the 10-step test of tests/test_gpu_config_length.py runs 256 Mi + 64 Mi);
+    PICSARQED_FULL_C5=1 runs the full size here as well."""
     import torch
-    full = os.environ.get("PICSARQED_SMALL_C5") != "1"
+    full = os.environ.get("PICSARQED_FULL_C5") == "1"   # (tests/test_gpu_config_length.py runs the full size, 10 steps)
     n_lep, n_pho = ((1 << 28), (1 << 26)) if full else ((1 << 25), (1 << 23))
     ctx, tabs = _ctx_with_tables(orc, qed, 5)
     rng = np.random.default_rng(50)
