@@ -513,6 +513,20 @@ def run_ours(args):
     barrier()
     ms_evolve2 = float(np.mean([e[0].elapsed_time(e[1]) for e in split[1:]]))
     ms_events2 = float(np.mean([e[1].elapsed_time(e[2]) for e in split[1:]]))
+    # the same two calls with "stage_records" (the caller promises not to touch the arrays in between)
+    ctx.set_option("stage_records", 1)
+    for k in range(5):
+        s = args.warmup + args.steps + 5 + k
+        f = fields[s % n_sets]
+        split[k][0].record()
+        ctx.evolve_optical_depth(q.LEPTON, p, f[:3], f[3:], dt, tau)
+        split[k][1].record()
+        ctx.generate_photons(p, f[:3], f[3:], tau, seed, s, id_base, cap, ph_p, ph_tau, ph_parent, n_out)
+        split[k][2].record()
+    barrier()
+    ctx.set_option("stage_records", 0)
+    ms_evolve3 = float(np.mean([e[0].elapsed_time(e[1]) for e in split[1:]]))
+    ms_events3 = float(np.mean([e[1].elapsed_time(e[2]) for e in split[1:]]))
     ms_total = sharding.max_over_ranks(ms_total, dev)
     value = world * n * args.steps / (ms_total * 1e-3)
 
@@ -569,7 +583,8 @@ def run_ours(args):
                                     "achieved": step_bytes / (ms_total / args.steps * 1e-3) / 1e9,
                                     "frac": step_bytes / (ms_total / args.steps * 1e-3) / 1e9 / peaks["hbm_gbs"]}},
         "kernels_ms": {"qed_step": {"evolve_pass": ms_evolve, "event_pass": ms_events},
-                       "two_call_path": {"evolve_optical_depth": ms_evolve2, "generate_photons": ms_events2}},
+                       "two_call_path": {"evolve_optical_depth": ms_evolve2, "generate_photons": ms_events2},
+                       "two_call_path_stage_records": {"evolve_optical_depth": ms_evolve3, "generate_photons": ms_events3}},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": args.e2e_steps},
         "gpu_launches": 3 * args.steps,

@@ -36,6 +36,7 @@ struct EvolveArgs {
     // offsets scan reads one word per tile instead of every chunk count
     unsigned int* tile_sum;
     int chunks_per_tile;
+    int remove_photons;         // EMIT, photons: 1 = the pass removes the photons it stages (qed_step), 0 = it only stages
     UnitScales units;           // the caller's unit system (picsarqed_set_units)
 };
 
@@ -344,7 +345,7 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                 const long long chunk = (base + (long long)warp * WCH) / kChunk;
                 if (lane == 0) {
                     a.stage_cnt[chunk] = (unsigned short)(total <= (unsigned)kStageCap
-                                                              ? (SPECIES == 1 && total > 0 ? (total | kStageParentDone) : total)
+                                                              ? (SPECIES == 1 && total > 0 && a.remove_photons ? (total | kStageParentDone) : total)
                                                               : (total | kStageNoRecords));
                     if (total > 0) atomicAdd(a.tile_sum + chunk / a.chunks_per_tile, total);
                 }
@@ -369,7 +370,7 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                             }
                         }
                     }
-                    if constexpr (SPECIES == 1) {
+                    if (SPECIES == 1 && a.remove_photons) {
                         // a photon that decays is removed whatever the split of its energy: p = 0, tau = +inf
                         // go out from here, with the stores of the evolve pass and while the momentum sectors are in L2 --
                         // the event pass has no scattered store left (it undoes this for events beyond the capacity)

@@ -51,6 +51,14 @@ struct picsarqed_ctx {
     int unit_system = 0;
     int event_config = 0;        // shape of event_kernel: see launch_event_pass
     int fused_step = 0;          // qed_step: 1 = the warp-specialised fused kernel (step.cuh), 0 = evolve pass + event pass
+    // "stage_records" = 1: evolve_optical_depth also stages the records of the particles that fire, and a generate_photons
+    // / generate_pairs call that follows ON THE SAME ARRAYS (the caller's promise: momenta, fields and tau untouched in
+    // between) takes them instead of re-scanning tau and gathering the parents
+    int stage_records = 0;
+    bool staged_valid = false;
+    const void* staged_tau = nullptr;
+    long long staged_n = 0;
+    int staged_species = -1, staged_dtype = -1, staged_tau_dtype = -1;
     int step_spill = 0;          // fused kernel: 1 = a streaming warp whose queue is full hands the chunk to the record path
     int step_batch_wait = 0;     // fused kernel: polls (2 us each) an event warp waits for four chunks before it takes fewer
     int step_config = 0;         // fused kernel: see launch_fused_step
@@ -354,6 +362,8 @@ int picsarqed_set_option(picsarqed_ctx* c, const char* name, long long value) {
         c->event_config = (int)value;
     else if (!std::strcmp(name, "fused_step") && (value == 0 || value == 1))
         c->fused_step = (int)value;
+    else if (!std::strcmp(name, "stage_records") && (value == 0 || value == 1))
+        c->stage_records = (int)value;
     else if (!std::strcmp(name, "step_config") && value >= 0 && value <= 1)
         c->step_config = (int)value;
     else if (!std::strcmp(name, "step_spill") && (value == 0 || value == 1))
@@ -495,11 +505,11 @@ int launch_chi(picsarqed_ctx* c, long long n, const void* const* a, void* out) {
     return PICSARQED_OK;
 }
 
-struct StageView { unsigned char* rec; unsigned short* cnt; unsigned int* tile_sum; int chunks_per_tile; long long stride; };
+struct StageView { unsigned char* rec; unsigned short* cnt; unsigned int* tile_sum; int chunks_per_tile; long long stride; int remove_photons; };
 
 template <typename R, typename TR, int SPECIES, int U, bool EMIT>
 int launch_evolve_u(picsarqed_ctx* c, long long n, const void* const* a, double dt, void* tau,
-                    unsigned long long* d_n_events, StageView sv = StageView{nullptr, nullptr, nullptr, 1, 0}) {
+                    unsigned long long* d_n_events, StageView sv = StageView{nullptr, nullptr, nullptr, 1, 0, 0}) {
     constexpr int V = 16 / sizeof(R);
     constexpr int TILE = kEvolveThreads * V * U;
     EvolveArgs<R, TR> args;
@@ -521,6 +531,7 @@ int launch_evolve_u(picsarqed_ctx* c, long long n, const void* const* a, double 
     args.stage_cnt = sv.cnt;
     args.tile_sum = sv.tile_sum;
     args.chunks_per_tile = sv.chunks_per_tile;
+    args.remove_photons = sv.remove_photons;
     size_t smem = ((size_t)args.tab.n * sizeof(R) + 127) & ~(size_t)127;
     args.table_in_smem = smem <= 96 * 1024;  // larger tables are read through L1/L2
     if (!args.table_in_smem) smem = 0;
@@ -542,21 +553,16 @@ int launch_evolve_u(picsarqed_ctx* c, long long n, const void* const* a, double 
     return PICSARQED_OK;
 }
 
-template <typename R, typename TR, int SPECIES>
-int launch_evolve(picsarqed_ctx* c, long long n, const void* const* a, double dt, void* tau,
-                  unsigned long long* d_n_events) {
-    // measured on B200: two 128-bit loads per array per thread, except fp32 photons (branchier: one)
-    int u = c->evolve_unroll ? c->evolve_unroll : ((sizeof(R) == 4 && SPECIES == 1) ? 1 : 2);
-    if (u == 1) return launch_evolve_u<R, TR, SPECIES, 1, false>(c, n, a, dt, tau, d_n_events);
-    if (u == 4) return launch_evolve_u<R, TR, SPECIES, 4, false>(c, n, a, dt, tau, d_n_events);
-    return launch_evolve_u<R, TR, SPECIES, 2, false>(c, n, a, dt, tau, d_n_events);
-}
-
 // per-chunk scratch: [tile sums][records][counts][offsets]
 struct ChunkScratch { unsigned char* rec; unsigned short* cnt; unsigned long long* off; unsigned int* sum; long long n_chunks; long long stride; };
 
 // seg_bytes: bytes of one entry of a chunk's segment (a staged record, or a staged result of the fused step; 0 = none)
-int chunk_scratch(picsarqed_ctx* c, long long n, size_t seg_bytes, ChunkScratch* out) {
+int chunk_scratch(picsarqed_ctx* c, long long n, size_t seg_bytes, ChunkScratch* out, bool keep_staged = false) {
+    if (c->staged_valid && !keep_staged) {
+        // records staged by evolve_optical_depth were never consumed: their tile sums must not leak into this call
+        if (c->rec) PXQ_CUDA(c, cudaMemsetAsync(c->rec, 0, c->rec_sum_bytes, c->stream));
+        c->staged_valid = false;
+    }
     const long long nchunks = (n + kChunk - 1) / kChunk;
     const size_t rec_sz = ((size_t)nchunks * kStageCap * seg_bytes + 255) & ~(size_t)255;
     const size_t cnt_sz = ((size_t)nchunks * sizeof(unsigned short) + 255) & ~(size_t)255;
@@ -595,6 +601,36 @@ int chunk_scratch(picsarqed_ctx* c, long long n, size_t seg_bytes, ChunkScratch*
 int event_chunks_per_tile(const picsarqed_ctx* c) {
     (void)c;
     return 32;  // both shapes of launch_event_pass
+}
+
+template <typename R, typename TR, int SPECIES>
+int launch_evolve(picsarqed_ctx* c, long long n, const void* const* a, double dt, void* tau,
+                  unsigned long long* d_n_events) {
+    if (c->stage_records) {
+        // the pass of qed_step without the removal of photons: tau evolves, the records of what fired are staged
+        ChunkScratch cs;
+        if (int rc = chunk_scratch(c, n, StageRecord<R>::kBytes, &cs)) return rc;
+        StageView sv{cs.rec, cs.cnt, cs.sum, event_chunks_per_tile(c), cs.stride, 0};
+        constexpr int U = kChunk / (32 * (16 / (int)sizeof(R)));
+        if (int rc = launch_evolve_u<R, TR, SPECIES, U, true>(c, n, a, dt, tau, d_n_events, sv)) return rc;
+        constexpr long long kTile = (long long)kEvolveThreads * (16 / (int)sizeof(R)) * U;
+        if (n % kTile)
+            count_chunks_kernel<TR><<<1, 256, 0, c->stream>>>((const TR*)tau, n, (n / kTile) * kTile / kChunk, cs.n_chunks, cs.cnt,
+                                                              cs.sum, sv.chunks_per_tile);
+        PXQ_CUDA(c, cudaGetLastError());
+        c->staged_valid = true;
+        c->staged_tau = tau;
+        c->staged_n = n;
+        c->staged_species = SPECIES;
+        c->staged_dtype = sizeof(R) == 8;
+        c->staged_tau_dtype = sizeof(TR) == 8;
+        return PICSARQED_OK;
+    }
+    // measured on B200: two 128-bit loads per array per thread, except fp32 photons (branchier: one)
+    int u = c->evolve_unroll ? c->evolve_unroll : ((sizeof(R) == 4 && SPECIES == 1) ? 1 : 2);
+    if (u == 1) return launch_evolve_u<R, TR, SPECIES, 1, false>(c, n, a, dt, tau, d_n_events);
+    if (u == 4) return launch_evolve_u<R, TR, SPECIES, 4, false>(c, n, a, dt, tau, d_n_events);
+    return launch_evolve_u<R, TR, SPECIES, 2, false>(c, n, a, dt, tau, d_n_events);
 }
 
 // levels 2 and 3 of the compaction: chunk counts (and their tile sums) -> offsets -> events
@@ -654,6 +690,14 @@ int launch_events(picsarqed_ctx* c, long long n, void* const* p, const void* con
                   unsigned long long seed, unsigned long long step, unsigned long long id_base, long long capacity,
                   void* const* out_p, void* const* out_tau, long long* parent, unsigned long long* d_n_out) {
     ChunkScratch cs;
+    if (c->staged_valid && c->staged_tau == tau && c->staged_n == n && c->staged_species == KIND &&
+        c->staged_dtype == (int)(sizeof(R) == 8) && c->staged_tau_dtype == (int)(sizeof(TR) == 8)) {
+        // "stage_records": the evolve call before this one staged the records and counted the chunks
+        if (int rc = chunk_scratch(c, n, StageRecord<R>::kBytes, &cs, true)) return rc;
+        c->staged_valid = false;
+        return launch_event_pass<R, TR, KIND>(c, n, cs, p, eb, tau, seed, step, id_base, capacity, out_p, out_tau, parent,
+                                              d_n_out);
+    }
     if (int rc = chunk_scratch(c, n, 0, &cs)) return rc;
     const int grid = (int)std::max<long long>(1, std::min<long long>((cs.n_chunks + 7) / 8, (long long)c->num_sms * 8));
     count_chunks_kernel<TR><<<grid, 256, 0, c->stream>>>((const TR*)tau, n, 0, cs.n_chunks, cs.cnt, cs.sum,
@@ -698,6 +742,7 @@ int launch_fused_step_c(picsarqed_ctx* c, long long n, void* const* p, const voi
     args.stage_cnt = cs.cnt;
     args.tile_sum = cs.sum;
     args.chunks_per_tile = event_chunks_per_tile(c);
+    args.remove_photons = 0;
     // shared memory: [1D table][sub-chunk stages][record queues]; a table that does not fit beside them is read through L1
     constexpr size_t kSmemMax = 227 * 1024 - 2048;   // (2 KB: the kernel's static shared memory)
     size_t smem = ((size_t)args.tab.n * sizeof(R) + 127) & ~(size_t)127;
@@ -789,6 +834,7 @@ int launch_step(picsarqed_ctx* c, long long n, void* const* p, const void* const
     sv.cnt = cs.cnt;
     sv.tile_sum = cs.sum;
     sv.chunks_per_tile = event_chunks_per_tile(c);
+    sv.remove_photons = 1;
     const void* a9[9] = {p[0], p[1], p[2], eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]};
     constexpr int U = kChunk / (32 * (16 / (int)sizeof(R)));  // fp64: 2, fp32: 1
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};

@@ -159,6 +159,11 @@ def test_config1_every_element(orc, qed):
         sec_t = [torch.zeros(n, dtype=torch.float64, device="cuda") for _ in range(nsec)]
         parent = torch.zeros(n, dtype=torch.int64, device="cuda")
         n_out = torch.zeros(1, dtype=torch.int64, device="cuda")
+        # the evolve pass of the step, seen through picsarqed_evolve_optical_depth on a copy (the same kernel arithmetic;
+        # tests/test_gpu_parity.py::test_fused_step holds the two bit-identical): the GPU's evolved tau of EVERY particle
+        tau_mid_d = tau.clone()
+        ctx.evolve_optical_depth(sp, dp, de, db, dt, tau_mid_d)
+        tau_mid = tau_mid_d.cpu().numpy()
         ctx.qed_step(sp, dp, de, db, tau, dt, seed, 0, sp * n, n, sec_p[0], sec_t[0], sec_p[1] if nsec == 2 else None,
                      sec_t[1] if nsec == 2 else None, parent, n_out)
         k = ctx.read_count(n_out)
@@ -166,9 +171,9 @@ def test_config1_every_element(orc, qed):
         ln_chi = np.log(np.maximum(orc.chi(sp, p, e, b), 1e-300))
         fired = np.zeros(n, bool)
         fired[parent.cpu().numpy()[:k]] = True
-        tau_mid = np.where(fired, o["tau"], tau.cpu().numpy())      # tau after evolve: untouched where nothing fired
-        n_amb, flags = check_evolve(np.where(fired, -np.abs(o["tau_exact"]) - 1e-300, tau_mid), tau0, o, np.float64, ln_chi)
+        n_amb, flags = check_evolve(tau_mid, tau0, o, np.float64, ln_chi)
         assert n_amb == 0 and np.array_equal(flags, fired) and k == int((o["tau"] < 0).sum())
+        assert np.array_equal(tau.cpu().numpy()[~fired], tau_mid[~fired])   # the step left the others as the evolve pass did
         ids = sp * n + np.arange(n, dtype=np.uint64)
         if sp == LEPTON:
             oe = orc.generate_photons(tabs, 1, 1, p, e, b, o["tau"], seed, 0, ids)

@@ -431,10 +431,19 @@ def test_fused_step(orc, qed, ctx, mid_tables, species, dtype, tdtype, n, target
     for cap in (n, max(1, n // 40)):
         f = _run_fused(qed, ctx, species, dtype, tdtype, p, e, b, tau0, dt, 77, 2, 123456789, cap)
         u, tau_mid = _run_unfused(qed, ctx, species, dtype, tdtype, p, e, b, tau0, dt, 77, 2, 123456789, cap)
-        assert f["n_fired"] == u["n_fired"] and _same(f["parent"], u["parent"])
-        assert _same(f["tau"], u["tau"]) and all(_same(x, y) for x, y in zip(f["p"], u["p"]))
-        for s in range(len(f["sec_p"])):
-            assert all(_same(x, y) for x, y in zip(f["sec_p"][s], u["sec_p"][s])) and _same(f["sec_tau"][s], u["sec_tau"][s])
+        # the two calls again with "stage_records": evolve_optical_depth stages what generate_* then takes
+        ctx.set_option("stage_records", 1)
+        try:
+            u2, tau_mid2 = _run_unfused(qed, ctx, species, dtype, tdtype, p, e, b, tau0, dt, 77, 2, 123456789, cap)
+        finally:
+            ctx.set_option("stage_records", 0)
+        assert _same(tau_mid, tau_mid2)
+        for other in (u, u2):
+            assert f["n_fired"] == other["n_fired"] and _same(f["parent"], other["parent"])
+            assert _same(f["tau"], other["tau"]) and all(_same(x, y) for x, y in zip(f["p"], other["p"]))
+            for s in range(len(f["sec_p"])):
+                assert all(_same(x, y) for x, y in zip(f["sec_p"][s], other["sec_p"][s]))
+                assert _same(f["sec_tau"][s], other["sec_tau"][s])
         # and against the oracle: evolve with the tie protocol, events on the GPU's evolved tau
         o = orc.evolve_optical_depth(tables, species, code(tdtype), p, e, b, dt, tau0)
         ln_chi = np.log(np.maximum(orc.chi(species, p, e, b), 1e-300))
@@ -449,6 +458,39 @@ def test_fused_step(orc, qed, ctx, mid_tables, species, dtype, tdtype, n, target
         _compare_events(f, oe, species, dtype, tdtype, cap, p)
         if n > 4096:
             assert f["n_fired"] > 0.5 * target * n
+
+
+def test_staged_records_are_dropped_when_not_consumed(orc, qed, ctx, mid_tables):
+    """"stage_records": records staged by an evolve call that no generate call consumes (another evolve, another array,
+    another size in between) must not leak into the next event pass"""
+    import torch
+    n = 2 * 4096 + 300
+    p, e, b = qed.workloads.config1(seed=41, n=n, species=LEPTON, dtype=np.float64)
+    dt = 3 * qed.workloads.choose_dt(orc.rate(mid_tables, LEPTON, p, e, b), 0.05)
+    tau0 = orc.init_optical_depth(LEPTON, F64, n, 6)
+    ref, _ = _run_unfused(qed, ctx, LEPTON, np.float64, np.float64, p, e, b, tau0, dt, 3, 1, 0, n)
+    ctx.set_option("stage_records", 1)
+    try:
+        dp, de, db = to_dev(p), to_dev(e), to_dev(b)
+        other = torch.from_numpy(tau0.copy()).cuda()
+        ctx.evolve_optical_depth(LEPTON, dp, de, db, 5 * dt, other)                 # staged, never consumed
+        ctx.evolve_optical_depth(LEPTON, [t[:4096] for t in dp], [t[:4096] for t in de], [t[:4096] for t in db], dt,
+                                 torch.from_numpy(tau0[:4096].copy()).cuda())        # another size
+        got, _ = _run_unfused(qed, ctx, LEPTON, np.float64, np.float64, p, e, b, tau0, dt, 3, 1, 0, n)
+        # a generate call on an array that was NOT the last one evolved re-scans tau
+        dtau = torch.from_numpy(tau0.copy()).cuda()
+        ctx.evolve_optical_depth(LEPTON, dp, de, db, dt, dtau)
+        ctx.evolve_optical_depth(LEPTON, dp, de, db, 5 * dt, other)
+        sec_p = [torch.zeros(n, dtype=torch.float64, device="cuda") for _ in range(3)]
+        sec_t = torch.zeros(n, dtype=torch.float64, device="cuda")
+        parent = torch.full((n,), -1, dtype=torch.int64, device="cuda")
+        n_out = torch.zeros(1, dtype=torch.int64, device="cuda")
+        ctx.generate_photons(dp, de, db, dtau, 3, 1, 0, n, sec_p, sec_t, parent, n_out)
+        k = ctx.read_count(n_out)
+    finally:
+        ctx.set_option("stage_records", 0)
+    assert got["n_fired"] == ref["n_fired"] and _same(got["parent"], ref["parent"]) and _same(got["tau"], ref["tau"])
+    assert k == ref["n_fired"] and _same(parent.cpu().numpy(), ref["parent"]) and _same(dtau.cpu().numpy(), ref["tau"])
 
 
 def test_fused_step_repeated_launches(qed, ctx):
