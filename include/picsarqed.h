@@ -130,6 +130,9 @@ int picsarqed_get_timing(picsarqed_ctx* ctx, double* host_ms, long long* host_ca
  * Accuracy: fixed by the scheme (panelled 8-point Gauss-Legendre over trapezoid-rule Bessel integrals), about 1e-11
  * relative on T, G, P against the oracle's adaptive quadrature; there is no tolerance knob.  n_xi <= 25600. */
 int picsarqed_build_tables(picsarqed_ctx* ctx, const picsarqed_table_params* host_params);
+/* Device time of the quadrature kernels of the last build_tables (CUDA events on the context's stream around the two
+ * processes' launches; milliseconds).  The call's wall time adds allocation, the fp32 copies and the search guides. */
+int picsarqed_get_table_build_ms(picsarqed_ctx* ctx, double* host_ms);
 /* Copies table `which` to host memory as fp64 (n_elems must equal the table's size).  Synchronises. */
 int picsarqed_export_tables(picsarqed_ctx* ctx, int which, double* host_dst, size_t n_elems);
 /* Replaces the tables by caller-provided values (host, fp64, layouts as above).  Synchronises. */

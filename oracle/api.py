@@ -37,6 +37,7 @@ class _CTables(C.Structure):
         ("lnG", _dp), ("qs_lnP", _dp), ("lnT", _dp), ("bw_P", _dp),
         ("read_fp32", C.c_int),
         ("qs_n_chi_2d", C.c_int), ("bw_n_chi_2d", C.c_int),   # rows of the 2D tables (0: as the 1D tables)
+        ("chi_event_min", C.c_double),                        # no event below this chi (0: off)
     ]
 
 
@@ -75,6 +76,7 @@ def lib():
             _dp, _dp, _dp, _dp, _i64p, _dp)
         sig("orc_generate_pairs", i64, tp, i, i, i64, *([_dp] * 10), u64, u64, _u64p, i64,
             *([_dp] * 8), _i64p, _dp)
+        sig("orc_classical_loss", None, i, i64, *([_dp] * 9), d, d)
         sig("orc_schwinger_prefactor", d)
         sig("orc_schwinger_rate", None, i64, *([_dp] * 7))
         sig("orc_qs_sample_xi", d, tp, d, d)
@@ -183,16 +185,25 @@ class Tables:
         self.bw_P = _f64(bw_P).reshape(params.rows_2d()[1], params.bw_n_xi)
         assert self.lnG.shape == (params.qs_n_chi,) and self.lnT.shape == (params.bw_n_chi,)
         self.read_fp32 = bool(read_fp32)
+        self.chi_event_min = 0.0
 
     def with_fp32_reads(self, flag=True):
-        return Tables(self.params, self.lnG, self.qs_lnP, self.lnT, self.bw_P, flag)
+        t = Tables(self.params, self.lnG, self.qs_lnP, self.lnT, self.bw_P, flag)
+        t.chi_event_min = self.chi_event_min
+        return t
+
+    def with_chi_event_min(self, chi_min):
+        """below chi_min neither process is an event (rate := 0)"""
+        t = Tables(self.params, self.lnG, self.qs_lnP, self.lnT, self.bw_P, self.read_fp32)
+        t.chi_event_min = float(chi_min)
+        return t
 
     def _c(self):
         p = self.params
         return _CTables(p.qs_chi_min, p.qs_chi_max, p.qs_n_chi, p.qs_xi_min, p.qs_n_xi,
                         p.bw_chi_min, p.bw_chi_max, p.bw_n_chi, p.bw_n_xi,
                         _p(self.lnG), _p(self.qs_lnP), _p(self.lnT), _p(self.bw_P),
-                        int(self.read_fp32), p.qs_n_chi_2d, p.bw_n_chi_2d)
+                        int(self.read_fp32), p.qs_n_chi_2d, p.bw_n_chi_2d, float(self.chi_event_min))
 
 
 def build_bw_rows(p, row0, row1, return_half=False):
@@ -331,6 +342,15 @@ def generate_pairs(tables, dtype, tau_dtype, p, e, b, tau, seed, step, ids=None,
                 po_p=[a[:k] for a in out[4:7]], po_tau=out[7][:k], parent=parent[:k], xi_el=xi[:k])
 
 
+def classical_loss(dtype, p, e, b, dt, chi_min):
+    """PAPER.md:340 / DESIGN.md R24: leptons with chi < chi_min lose (2/3)(alpha/tau_C) chi^2 (gamma-1)/gamma dt of kinetic
+    energy; returns the three momentum arrays after the step"""
+    pp = [_f64(a).copy() for a in p]
+    ff = [_f64(a) for a in (*e, *b)]
+    lib().orc_classical_loss(dtype, pp[0].size, *[_p(a) for a in pp], *[_p(a) for a in ff], float(dt), float(chi_min))
+    return pp
+
+
 def qs_sample_xi(tables, chi_v, r):
     ct = tables._c()
     return lib().orc_qs_sample_xi(C.byref(ct), chi_v, r)
@@ -354,4 +374,4 @@ def schwinger_rate(e, b):
     return out
 
 
-__all__ += ["schwinger_prefactor", "schwinger_rate"]
+__all__ += ["schwinger_prefactor", "schwinger_rate", "classical_loss"]

@@ -425,6 +425,10 @@ struct OrcTables {
     // rows of the 2D tables when they sit on a chi grid of their own (0: the grid of the 1D table).  PAPER.md:203/:246 (1D)
     // and :210/:251 (2D) define the two grids separately; BASELINE configuration 4 asks for 4096 and 2048 points.
     int qs_n_chi_2d, bw_n_chi_2d;
+    // PAPER.md:340 (WarpX): "a minimum quantum parameter threshold below which Breit-Wheeler pair production is ignored and
+    // photon emission is simulated with a classical model" -- below chi_event_min neither process is an event (rate := 0;
+    // DESIGN.md R24).  0 = off.  The classical model itself is orc_classical_loss below.
+    double chi_event_min;
 };
 static inline int qs_rows(const OrcTables* t) { return t->qs_n_chi_2d > 0 ? t->qs_n_chi_2d : t->qs_n_chi; }
 static inline int bw_rows(const OrcTables* t) { return t->bw_n_chi_2d > 0 ? t->bw_n_chi_2d : t->bw_n_chi; }
@@ -474,7 +478,9 @@ static real erber_T(real chi) {
 // dN/dt in 1/s (eq.15 for leptons, eq.8 for photons); also the ln of the tabulated factor
 static real qed_rate(const OrcTables* t, int species, real chi, real g, real* L_out, real* slope_out) {
     real L = 0, slope = 0, rate = 0;
-    if (species == 0) {
+    if (chi < (real)t->chi_event_min) {
+        // below the threshold of PAPER.md:340: no event of either kind
+    } else if (species == 0) {
         real lc = logl(chi);  // chi = 0 -> -inf -> clamped to the first value
         lc = std::max(logl((real)t->qs_chi_min), std::min(logl((real)t->qs_chi_max), lc));
         L = lookup_ln(t, t->lnG, t->qs_chi_min, t->qs_chi_max, t->qs_n_chi, lc, &slope);
@@ -626,6 +632,35 @@ void orc_evolve_optical_depth(const OrcTables* t, int species, int tau_dtype, in
         if (decr) decr[i] = (double)d;
         if (lnval) lnval[i] = (double)L;
         if (slope) slope[i] = (double)sl;
+    }
+}
+
+// Classical radiation reaction below the threshold of PAPER.md:340 (R24; refs [58, 59] of the paper are not in
+// the container).  Reading: a lepton with chi < chi_min loses energy continuously at the classical radiated power, which
+// is the chi -> 0 limit of the mean loss of the Monte Carlo emission: the emission rate (2/3)(alpha/tau_C) G/gamma (eq.15)
+// times the mean photon energy (gamma - 1) <xi>, <xi> = int S dxi / G, with int S dxi -> chi^2 (classical synchrotron power):
+//     d(gamma - 1)/dt = -(2/3) (alpha/tau_C) chi^2 (gamma - 1)/gamma,
+// one explicit step per call, direction kept, norm(p') from gamma' (as for an emission, R15), the kinetic energy
+// not below zero.  Leptons at or above the threshold are left alone.
+void orc_classical_loss(int dtype, int64_t n, double* px, double* py, double* pz, const double* ex, const double* ey,
+                        const double* ez, const double* bx, const double* by, const double* bz, double dt,
+                        double chi_min) {
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        const double p[3] = {px[i], py[i], pz[i]}, e[3] = {ex[i], ey[i], ez[i]}, b[3] = {bx[i], by[i], bz[i]};
+        __float128 gq;
+        const real chi = (real)chi_q(0, p, e, b, &gq);
+        if (!(chi < (real)chi_min)) continue;
+        const real g = (real)gq;
+        const real pn = sqrtl((real)p[0] * p[0] + (real)p[1] * p[1] + (real)p[2] * p[2]);
+        if (!(pn > 0)) continue;
+        const real k = pn * pn / (g + 1);  // gamma - 1
+        real k2 = k - (2.0L / 3) * rate_prefactor() * chi * chi * (k / g) * (real)dt;
+        if (k2 < 0) k2 = 0;
+        const real s = sqrtl(k2 * (k2 + 2)) / pn;
+        px[i] = round_to(s * p[0], dtype);
+        py[i] = round_to(s * p[1], dtype);
+        pz[i] = round_to(s * p[2], dtype);
     }
 }
 

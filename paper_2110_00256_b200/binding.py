@@ -68,6 +68,7 @@ _SIGNATURES = {
     "picsarqed_get_unit_scales": (_i, [_vp, C.POINTER(_d)]),
     "picsarqed_get_timing": (_i, [_vp, C.POINTER(_d), C.POINTER(_i64)]),
     "picsarqed_build_tables": (_i, [_vp, C.POINTER(_CParams)]),
+    "picsarqed_get_table_build_ms": (_i, [_vp, C.POINTER(_d)]),
     "picsarqed_export_tables": (_i, [_vp, _i, _vp, C.c_size_t]),
     "picsarqed_import_tables": (_i, [_vp, C.POINTER(_CParams), _vp, _vp, _vp, _vp]),
     "picsarqed_chi": (_i, [_vp, _i, _i, _i64] + [_vp] * 10),
@@ -173,6 +174,12 @@ class Context:
         cp = params._c()
         self._check(lib().picsarqed_build_tables(self._h, C.byref(cp)))
         self.params = params
+
+    def table_build_ms(self):
+        """device time of the quadrature kernels of the last build_tables, in milliseconds"""
+        ms = _d(0.0)
+        self._check(lib().picsarqed_get_table_build_ms(self._h, C.byref(ms)))
+        return ms.value
 
     def import_tables(self, params, lnG, qs_lnP, lnT, bw_P):
         arrs = [np.ascontiguousarray(a, dtype=np.float64).ravel() for a in (lnG, qs_lnP, lnT, bw_P)]

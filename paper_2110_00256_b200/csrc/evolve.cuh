@@ -119,6 +119,65 @@ __host__ __device__ constexpr double hankel13(int k) {
     return a;
 }
 
+// Outside the T table: chi T = 0.16 K_{1/3}(x)^2, x = 4/(3 chi) (eq.10 with the argument of DESIGN.md R2).
+// A routine of its own: for fp32 particles it is called (not inlined), so that the registers of the streaming kernel are
+// those of its common path (in-table photons) and three CTAs fit on an SM.
+template <typename R>
+__device__ __forceinline__ R erber_decrement_body(double c2, double inv_g, double rate_dt) {
+    typedef R A;
+        // chi T = 0.16 K_{1/3}(x)^2, x = 4/(3 chi) (eq.10 with the argument of DESIGN.md R2)
+        if (c2 < 1.7777e-4) return (A)0;  // x > 100: K^2 < e^-200, the decrement is below 1e-80 of any optical depth
+        if constexpr (sizeof(R) == 4) {
+            if (c2 > 7.2e2) {  // x < 0.05, fp32 particles: the same series in float (two terms: y < 7e-4)
+                const float y = (4.0f / 9.0f) / (float)c2;
+                const float sm = (float)(1.0 / 1.3541179394264004) * fmaf(y, 1.5f, 1.0f);
+                const float sp = (float)(1.0 / 0.8929795115692492) * fmaf(y, 0.75f, 1.0f);
+                const float h2 = cbrtf(y);
+                const float k = sm - sp * h2;
+                return (float)rate_dt * (0.16f * 3.2898681336964524f) * (k * k / h2) * (float)inv_g;  // (pi/sqrt3)^2
+            }
+        }
+        double k2;                        // K_{1/3}(x)^2
+        if (c2 > 7.2e2) {                 // x < 0.05
+            // ascending series (DLMF 10.27.4, 10.25.2), four terms: relative error < (x^2/4)^4 < 2e-13.
+            // K = (pi/sqrt3) (sm/h - sp h), h = (x/2)^(1/3); with y = x^2/4 = 4/(9 chi^2): h^2 = cbrt(y)
+            // (coefficients 1/(k (k -+ nu)) are written as constants: no divisions in the series)
+            const double y = (4.0 / 9.0) / c2;
+            constexpr double am1 = 1.0 / (1.0 * (1.0 - 1.0 / 3.0)), am2 = 1.0 / (2.0 * (2.0 - 1.0 / 3.0)),
+                             am3 = 1.0 / (3.0 * (3.0 - 1.0 / 3.0));
+            constexpr double ap1 = 1.0 / (1.0 * (1.0 + 1.0 / 3.0)), ap2 = 1.0 / (2.0 * (2.0 + 1.0 / 3.0)),
+                             ap3 = 1.0 / (3.0 * (3.0 + 1.0 / 3.0));
+            const double sm = (1.0 / 1.3541179394264004) * fma(y * am1, fma(y * am2, fma(y, am3, 1.0), 1.0), 1.0);
+            const double sp = (1.0 / 0.8929795115692492) * fma(y * ap1, fma(y * ap2, fma(y, ap3, 1.0), 1.0), 1.0);
+            const double h2 = cbrt(y);
+            const double k = sm - sp * h2;  // K h sqrt3/pi
+            k2 = (1.5707963267948966 / 0.8660254037844386) * (1.5707963267948966 / 0.8660254037844386) * k * k / h2;
+        } else if (c2 < 2.8444e-3) {      // x > 25: the window just below a T table that starts at chi ~ 1e-2
+            // Hankel expansion (DLMF 10.40.2): K^2 = (pi/2x) e^{-2x} (sum_k a_k x^-k)^2, sixteen terms in
+            // Horner form with constant coefficients (the first term left out is < 1e-16 at x = 25); 1/x =
+            // (3/4) chi comes from one rsqrt: no division, no logarithm
+            const double rs = rsqrt_fast(c2);
+            const double x = (4.0 / 3.0) * rs, r = 0.75 * (c2 * rs);
+            double sum = hankel13(16);
+#pragma unroll
+            for (int k = 15; k >= 1; --k) sum = fma(sum, r, hankel13(k));
+            sum = fma(sum, r, 1.0);
+            k2 = 1.5707963267948966 * r * sum * sum * exp_fast(-2.0 * x);
+        } else {
+            const double x = 4.0 / (3.0 * sqrt(c2));
+            k2 = exp(2.0 * (ln_bessel_k13_scaled(x) - x));
+        }
+        return (A)(rate_dt * 0.16 * k2 * inv_g);
+}
+__device__ __noinline__ float erber_decrement_f32(double c2, double inv_g, double rate_dt) {
+    return erber_decrement_body<float>(c2, inv_g, rate_dt);
+}
+template <typename R>
+__device__ __forceinline__ R erber_decrement(double c2, double inv_g, double rate_dt) {
+    if constexpr (sizeof(R) == 4) return erber_decrement_f32(c2, inv_g, rate_dt);
+    else return erber_decrement_body<R>(c2, inv_g, rate_dt);
+}
+
 // The decrement dN/dt * dt from chi^2 (all cases, one particle), in the particle arithmetic type A = R.
 template <typename R, int SPECIES>
 __device__ __forceinline__ R rate_from_c2(double c2, double inv_g, double g2, const R* tab, const Table1D<R>& T,
@@ -137,49 +196,8 @@ __device__ __forceinline__ R rate_from_c2(double c2, double inv_g, double g2, co
         // eq.8 with T from eq.23; Erber form outside; gamma_gamma <= 2 cannot decay (R12)
         if (!(g2 > 4.0) || !(c2 > 0.0)) return (A)0;
         if (c2 < T.chi_min * T.chi_min || c2 > T.chi_max * T.chi_max) {
-            // chi T = 0.16 K_{1/3}(x)^2, x = 4/(3 chi) (eq.10 with the argument of DESIGN.md R2)
-            if (c2 < 1.7777e-4) return (A)0;  // x > 100: K^2 < e^-200, the decrement is below 1e-80 of any optical depth
-            if constexpr (sizeof(R) == 4) {
-                if (c2 > 7.2e2) {  // x < 0.05, fp32 particles: the same series in float (two terms: y < 7e-4)
-                    const float y = (4.0f / 9.0f) / (float)c2;
-                    const float sm = (float)(1.0 / 1.3541179394264004) * fmaf(y, 1.5f, 1.0f);
-                    const float sp = (float)(1.0 / 0.8929795115692492) * fmaf(y, 0.75f, 1.0f);
-                    const float h2 = cbrtf(y);
-                    const float k = sm - sp * h2;
-                    return (float)rate_dt * (0.16f * 3.2898681336964524f) * (k * k / h2) * (float)inv_g;  // (pi/sqrt3)^2
-                }
-            }
-            double k2;                        // K_{1/3}(x)^2
-            if (c2 > 7.2e2) {                 // x < 0.05
-                // ascending series (DLMF 10.27.4, 10.25.2), four terms: relative error < (x^2/4)^4 < 2e-13.
-                // K = (pi/sqrt3) (sm/h - sp h), h = (x/2)^(1/3); with y = x^2/4 = 4/(9 chi^2): h^2 = cbrt(y)
-                // (coefficients 1/(k (k -+ nu)) are written as constants: no divisions in the series)
-                const double y = (4.0 / 9.0) / c2;
-                constexpr double am1 = 1.0 / (1.0 * (1.0 - 1.0 / 3.0)), am2 = 1.0 / (2.0 * (2.0 - 1.0 / 3.0)),
-                                 am3 = 1.0 / (3.0 * (3.0 - 1.0 / 3.0));
-                constexpr double ap1 = 1.0 / (1.0 * (1.0 + 1.0 / 3.0)), ap2 = 1.0 / (2.0 * (2.0 + 1.0 / 3.0)),
-                                 ap3 = 1.0 / (3.0 * (3.0 + 1.0 / 3.0));
-                const double sm = (1.0 / 1.3541179394264004) * fma(y * am1, fma(y * am2, fma(y, am3, 1.0), 1.0), 1.0);
-                const double sp = (1.0 / 0.8929795115692492) * fma(y * ap1, fma(y * ap2, fma(y, ap3, 1.0), 1.0), 1.0);
-                const double h2 = cbrt(y);
-                const double k = sm - sp * h2;  // K h sqrt3/pi
-                k2 = (1.5707963267948966 / 0.8660254037844386) * (1.5707963267948966 / 0.8660254037844386) * k * k / h2;
-            } else if (c2 < 2.8444e-3) {      // x > 25: the window just below a T table that starts at chi ~ 1e-2
-                // Hankel expansion (DLMF 10.40.2): K^2 = (pi/2x) e^{-2x} (sum_k a_k x^-k)^2, sixteen terms in
-                // Horner form with constant coefficients (the first term left out is < 1e-16 at x = 25); 1/x =
-                // (3/4) chi comes from one rsqrt: no division, no logarithm
-                const double rs = rsqrt_fast(c2);
-                const double x = (4.0 / 3.0) * rs, r = 0.75 * (c2 * rs);
-                double sum = hankel13(16);
-#pragma unroll
-                for (int k = 15; k >= 1; --k) sum = fma(sum, r, hankel13(k));
-                sum = fma(sum, r, 1.0);
-                k2 = 1.5707963267948966 * r * sum * sum * exp_fast(-2.0 * x);
-            } else {
-                const double x = 4.0 / (3.0 * sqrt(c2));
-                k2 = exp(2.0 * (ln_bessel_k13_scaled(x) - x));
-            }
-            return (A)(rate_dt * 0.16 * k2 * inv_g);
+            if (c2 < 1.7777e-4) return (A)0;  // (the routine's own first test, kept here: no call for the photons far below)
+            return erber_decrement<R>(c2, inv_g, rate_dt);
         }
         lc = lc < ln_min ? ln_min : (lc > ln_max ? ln_max : lc);
         const A L = lookup_ln<R, A>(tab, T.n, lc, ln_min, inv_delta);
@@ -263,7 +281,7 @@ __device__ __forceinline__ void decrement_vec(const R (&in)[9][V], const R* tab,
 // segment of its 128-particle chunk, in index order (warp ballot/popc; no CTA barrier), for event_kernel.
 // Requires U*32*V == kChunk.
 template <typename R, typename TR, int SPECIES, int U, bool EMIT, bool SCALED>
-__global__ void __launch_bounds__(kEvolveThreads, U > 2 ? 1 : ((sizeof(R) == 4 && U == 1 && SPECIES == 0) ? 3 : 2))
+__global__ void __launch_bounds__(kEvolveThreads, U > 2 ? 1 : ((sizeof(R) == 4 && U == 1) ? 3 : 2))
 evolve_kernel(const EvolveArgs<R, TR> a) {
     constexpr int V = 16 / sizeof(R);
     constexpr int TILE = kEvolveThreads * V * U;

@@ -92,6 +92,7 @@ struct picsarqed_ctx {
     double build_ms = 0.0;
     cudaStream_t aux_stream = nullptr;       // build_tables: the second process
     cudaEvent_t aux_event[2] = {nullptr, nullptr};
+    cudaEvent_t build_event[2] = {nullptr, nullptr};   // around the quadrature kernels of the last build_tables
 };
 
 namespace {
@@ -138,12 +139,15 @@ int alloc_tables(picsarqed_ctx* c, const picsarqed_table_params& p) {
     size_t n[4];
     table_sizes(p, n);
     for (int k = 0; k < 4; ++k) {
-        if (c->tab64[k]) cudaFree(c->tab64[k]);
-        if (c->tab32[k]) cudaFree(c->tab32[k]);
-        c->tab64[k] = nullptr;
-        c->tab32[k] = nullptr;
-        PXQ_CUDA(c, cudaMalloc(&c->tab64[k], (n[k] + 4) * sizeof(double)));
-        PXQ_CUDA(c, cudaMalloc(&c->tab32[k], (n[k] + 4) * sizeof(float)));
+        if (c->tab_n[k] != n[k] || !c->tab64[k] || !c->tab32[k]) {   // (a rebuild of the same geometry keeps its buffers)
+            if (c->tab64[k]) cudaFree(c->tab64[k]);
+            if (c->tab32[k]) cudaFree(c->tab32[k]);
+            c->tab64[k] = nullptr;
+            c->tab32[k] = nullptr;
+            c->tab_n[k] = 0;
+            PXQ_CUDA(c, cudaMalloc(&c->tab64[k], (n[k] + 4) * sizeof(double)));
+            PXQ_CUDA(c, cudaMalloc(&c->tab32[k], (n[k] + 4) * sizeof(float)));
+        }
         PXQ_CUDA(c, cudaMemsetAsync(c->tab64[k], 0, (n[k] + 4) * sizeof(double), c->stream));
         PXQ_CUDA(c, cudaMemsetAsync(c->tab32[k], 0, (n[k] + 4) * sizeof(float), c->stream));
         c->tab_n[k] = n[k];
@@ -342,6 +346,7 @@ int picsarqed_destroy(picsarqed_ctx* c) {
     for (cudaEvent_t e : c->slab_events) cudaEventDestroy(e);
     if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
     for (int k = 0; k < 2; ++k) if (c->aux_event[k]) cudaEventDestroy(c->aux_event[k]);
+    for (int k = 0; k < 2; ++k) if (c->build_event[k]) cudaEventDestroy(c->build_event[k]);
     if (c->h2d_stream) cudaStreamDestroy(c->h2d_stream);
     if (c->d2h_stream) cudaStreamDestroy(c->d2h_stream);
     delete c;
@@ -1224,6 +1229,9 @@ extern "C" int picsarqed_build_tables(picsarqed_ctx* c, const picsarqed_table_pa
     if (!c->aux_stream) PXQ_CUDA(c, cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking));
     if (!c->aux_event[0])
         for (int k = 0; k < 2; ++k) PXQ_CUDA(c, cudaEventCreateWithFlags(&c->aux_event[k], cudaEventDisableTiming));
+    if (!c->build_event[0])
+        for (int k = 0; k < 2; ++k) PXQ_CUDA(c, cudaEventCreate(&c->build_event[k]));
+    PXQ_CUDA(c, cudaEventRecord(c->build_event[0], c->stream));
     PXQ_CUDA(c, cudaEventRecord(c->aux_event[0], c->stream));            // (the tables were just cleared on c->stream)
     PXQ_CUDA(c, cudaStreamWaitEvent(c->aux_stream, c->aux_event[0], 0));
     for (int kind = 0; kind < 2; ++kind) {
@@ -1263,10 +1271,20 @@ extern "C" int picsarqed_build_tables(picsarqed_ctx* c, const picsarqed_table_pa
     }
     PXQ_CUDA(c, cudaEventRecord(c->aux_event[1], c->aux_stream));
     PXQ_CUDA(c, cudaStreamWaitEvent(c->stream, c->aux_event[1], 0));
+    PXQ_CUDA(c, cudaEventRecord(c->build_event[1], c->stream));          // (the quadrature kernels of both processes end here)
     if (int rc = narrow_tables(c)) return rc;
     if (int rc = build_guides(c)) return rc;
     PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    float ms = 0.f;
+    PXQ_CUDA(c, cudaEventElapsedTime(&ms, c->build_event[0], c->build_event[1]));
+    c->build_ms = ms;
     c->have_tables = true;
+    return PICSARQED_OK;
+}
+
+extern "C" int picsarqed_get_table_build_ms(picsarqed_ctx* c, double* host_ms) {
+    if (!c || !host_ms) return PICSARQED_ERR_INVALID;
+    *host_ms = c->build_ms;
     return PICSARQED_OK;
 }
 

@@ -444,6 +444,71 @@ def test_children_and_parent_streams(orc, small_tables):
     assert orc.uniform(seed, base + 9, step, 2, PHOTON, 1, F64) == _stream_uniform(orc, seed, base + 9, step, 2, PHOTON, 1)
 
 
+# ----------------------------------------------------------------------------- chi threshold and classical model
+def test_chi_threshold_switches_both_processes_off(orc):
+    """below the threshold neither process is an event: the rate is exactly 0, at and above it the rate is unchanged"""
+    t = _power_law_tables(orc)
+    tt = t.with_chi_event_min(0.5)
+    for sp, pm in ((LEPTON, 1000.0), (PHOTON, 500.0)):
+        for chi_want, below in ((0.2, True), (0.4999, True), (0.5001, False), (7.0, False)):
+            args = (vec((pm, 0, 0)), vec((0, 0, 0)), vec((0, chi_want / pm, 0)))
+            r0, r1 = orc.rate(t, sp, *args)[0], orc.rate(tt, sp, *args)[0]
+            assert r0 > 0 and (r1 == 0.0 if below else r1 == r0)
+    # evolve: optical depths of the particles below the threshold do not move
+    n = 1000
+    rng = np.random.default_rng(5)
+    p, e, b, g = _population(rng, n, LEPTON)
+    chi = orc.chi(LEPTON, p, e, b)
+    tau = rng.exponential(size=n)
+    o = orc.evolve_optical_depth(tt, LEPTON, F64, p, e, b, 1e-15, tau)
+    assert np.array_equal(o["tau"][chi < 0.5], tau[chi < 0.5]) and np.all(o["tau"][chi >= 0.5] < tau[chi >= 0.5])
+
+
+def test_classical_loss_closed_form_and_bookkeeping(orc):
+    """p perp b: chi = |p||b|; one step removes (2/3)(alpha/tau_C) chi^2 (gamma-1)/gamma dt of kinetic energy, keeps the
+    direction, leaves the leptons at or above the threshold alone and never takes the kinetic energy below zero"""
+    pm, bb, dt = 300.0, 1e-6, 2e-13
+    g = math.sqrt(1 + pm * pm)
+    chi = pm * bb
+    p2 = orc.classical_loss(F64, vec((0, pm, 0)), vec((0, 0, 0)), vec((bb, 0, 0)), dt, 1e-3)
+    k_after = math.sqrt(1 + p2[1][0] ** 2) - 1
+    want = (g - 1) - 2 / 3 * ALPHA_OVER_TAUC * chi * chi * (g - 1) / g * dt
+    assert p2[0][0] == 0 and p2[2][0] == 0 and p2[1][0] > 0
+    assert k_after == pytest.approx(want, rel=1e-12) and 0 < 1 - want / (g - 1) < 0.5
+    # at / above the threshold: untouched, bit for bit
+    same = orc.classical_loss(F64, vec((0, pm, 0)), vec((0, 0, 0)), vec((bb, 0, 0)), dt, chi)
+    assert same[1][0] == pm
+    # a step that would take more than there is stops at rest
+    rest = orc.classical_loss(F64, vec((0, pm, 0)), vec((0, 0, 0)), vec((bb, 0, 0)), 1e-6, 1e-3)
+    assert rest[1][0] == 0.0
+    # a random population: direction kept, energy never gained, fp32 storage rounds once
+    rng = np.random.default_rng(8)
+    p, e, b, g = _population(rng, 500, LEPTON)
+    chi = orc.chi(LEPTON, p, e, b)
+    q = orc.classical_loss(F64, p, e, b, 1e-16, 0.05)
+    low = chi < 0.05
+    assert 0 < low.sum() < 500 and all(np.array_equal(a[~low], c[~low]) for a, c in zip(p, q))
+    n0, n1 = np.sqrt(sum(a * a for a in p)), np.sqrt(sum(a * a for a in q))
+    assert np.all(n1[low] < n0[low])
+    for a, c in zip(p, q):
+        assert np.allclose(c[low] / n1[low], a[low] / n0[low], atol=1e-13)
+    q32 = orc.classical_loss(F32, p, e, b, 1e-16, 0.05)
+    assert all(np.array_equal(c[low], c[low].astype(np.float32).astype(np.float64)) for c in q32)
+
+
+def test_classical_loss_is_the_small_chi_limit_of_the_mean_emission(orc):
+    """continuity across the threshold: the mean energy a lepton loses per unit time to the Monte Carlo emission,
+    rate x (gamma-1) x <xi> with <xi> = int S dxi / G (exact quadratures), tends to the classical power as chi -> 0"""
+    pm, dt = 2000.0, 1e-18
+    g = math.sqrt(1 + pm * pm)
+    for chi, tol in ((1e-3, 1e-2), (1e-2, 6e-2)):        # the quantum correction is 1 - 5.95 chi + ...
+        mc = 2 / 3 * ALPHA_OVER_TAUC * orc.qs_first_moment(chi) * (g - 1) / g          # rate x <xi> x (gamma-1), G cancels
+        p2 = orc.classical_loss(F64, vec((0, pm, 0)), vec((0, 0, 0)), vec((chi / pm, 0, 0)), dt, 1.0)
+        cl = ((g - 1) - (math.sqrt(1 + p2[1][0] ** 2) - 1)) / dt
+        assert cl == pytest.approx(2 / 3 * ALPHA_OVER_TAUC * chi * chi * (g - 1) / g, rel=1e-6)
+        assert mc < cl and mc == pytest.approx(cl, rel=tol)
+
+
 # ----------------------------------------------------------------------------- Schwinger rate (SURVEY.md 8(f)-3)
 def test_schwinger_rate_closed_forms(orc):
     """PAPER.md:171-183 eqs.19-22: prefactor from CODATA, pure-E textbook limit, E parallel B, null fields"""
