@@ -271,6 +271,20 @@ int picsarqed_step_host(picsarqed_ctx* ctx, int species, int dtype, int tau_dtyp
 int picsarqed_boris_push_uniform(picsarqed_ctx* ctx, int dtype, long long n, void* px, void* py, void* pz,
                                  int charge_sign, const double* e, const double* b, double dt);
 
+/* ---- chi threshold and classical radiation reaction (R24) -------------------------------
+ * "WarpX offers the possibility to select a minimum quantum parameter threshold below which Breit-Wheeler pair production
+ * is ignored and photon emission is simulated with a classical model."  set_chi_threshold(chi_min > 0): a particle with
+ * chi < chi_min has no event of either kind -- its optical depth is not decremented by chi, evolve_optical_depth,
+ * qed_step, step_host or cascade_step (0, the default, switches the threshold off).  classical_loss: one explicit step of
+ * the classical model for the leptons below the threshold, d(gamma-1)/dt = -(2/3)(alpha/tau_C) chi^2 (gamma-1)/gamma
+ * (the chi -> 0 limit of the mean loss of the Monte Carlo emission), direction kept, momenta rewritten in place; leptons
+ * at or above the threshold are not touched; a no-op while the threshold is 0.  Library units only.  cascade_step calls
+ * it for both lepton species after the push when the threshold is set. */
+int picsarqed_set_chi_threshold(picsarqed_ctx* ctx, double chi_min);
+int picsarqed_classical_loss(picsarqed_ctx* ctx, int dtype, long long n, void* px, void* py, void* pz,
+                             const void* ex, const void* ey, const void* ez,
+                             const void* bx, const void* by, const void* bz, double dt);
+
 /* Ordered, filtering append (R20, R22): of the first m = min(*d_count, m_max) entries
  * of the source arrays s_* (device; *d_count is a device counter such as qed_step's d_n_out),
  * those with sqrt(px^2+py^2+pz^2) >= min_energy (photons below the threshold are

@@ -123,7 +123,9 @@ def qed_step_species(tables, species, dtype, tau_dtype, pop, e, b, dt, seed, ste
 
 def cascade_step(tables, dtype, tau_dtype, pops, e, b, dt, seed, step, photon_min_energy=0.0, push=True):
     """one time step in the order of R20.  pops: dict electrons / positrons / photons -> Population (modified).
-    Returns the numbers of events (electrons, positrons, photons) and of photons kept."""
+    Returns the numbers of events (electrons, positrons, photons) and of photons kept.
+    With tables.chi_event_min > 0 (R24) the leptons below the threshold take one step of the classical
+    radiation reaction after the push, and no particle below it has an event."""
     el, po, ph = pops["electrons"], pops["positrons"], pops["photons"]
     if push:
         el.p = boris_push_uniform(el.p, -1, e, b, dt)
@@ -131,6 +133,11 @@ def cascade_step(tables, dtype, tau_dtype, pops, e, b, dt, seed, step, photon_mi
         if dtype == api.F32:
             el.p = [a.astype(np.float32).astype(np.float64) for a in el.p]
             po.p = [a.astype(np.float32).astype(np.float64) for a in po.p]
+    if tables.chi_event_min > 0:
+        for pop in (el, po):
+            ee = [np.full(pop.n, float(v)) for v in e]
+            bb = [np.full(pop.n, float(v)) for v in b]
+            pop.p = api.classical_loss(dtype, pop.p, ee, bb, dt, tables.chi_event_min)
     oe = qed_step_species(tables, api.LEPTON, dtype, tau_dtype, el, e, b, dt, seed, step, ID_BASE["electrons"])
     op = qed_step_species(tables, api.LEPTON, dtype, tau_dtype, po, e, b, dt, seed, step, ID_BASE["positrons"])
     og = qed_step_species(tables, api.PHOTON, dtype, tau_dtype, ph, e, b, dt, seed, step, ID_BASE["photons"])

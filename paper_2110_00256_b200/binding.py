@@ -69,6 +69,8 @@ _SIGNATURES = {
     "picsarqed_get_timing": (_i, [_vp, C.POINTER(_d), C.POINTER(_i64)]),
     "picsarqed_build_tables": (_i, [_vp, C.POINTER(_CParams)]),
     "picsarqed_get_table_build_ms": (_i, [_vp, C.POINTER(_d)]),
+    "picsarqed_set_chi_threshold": (_i, [_vp, _d]),
+    "picsarqed_classical_loss": (_i, [_vp, _i, _i64] + [_vp] * 9 + [_d]),
     "picsarqed_export_tables": (_i, [_vp, _i, _vp, C.c_size_t]),
     "picsarqed_import_tables": (_i, [_vp, C.POINTER(_CParams), _vp, _vp, _vp, _vp]),
     "picsarqed_chi": (_i, [_vp, _i, _i, _i64] + [_vp] * 10),
@@ -305,6 +307,16 @@ class Context:
                                               _dev(r, chi.dtype), _dev(xi, chi.dtype)))
 
     # ---- closed loop in a uniform field ------------------------------
+    def set_chi_threshold(self, chi_min):
+        """no event of either kind below chi_min (0 = off)"""
+        self._check(lib().picsarqed_set_chi_threshold(self._h, float(chi_min)))
+
+    def classical_loss(self, p, e, b, dt):
+        """one step of the classical radiation reaction for the leptons below the chi threshold (momenta in place)"""
+        d = p[0].dtype
+        self._check(lib().picsarqed_classical_loss(self._h, _code(d), p[0].numel(), *[_dev(t, d) for t in (*p, *e, *b)],
+                                                   float(dt)))
+
     def boris_push_uniform(self, p, charge_sign, e, b, dt):
         d = p[0].dtype
         self._check(lib().picsarqed_boris_push_uniform(

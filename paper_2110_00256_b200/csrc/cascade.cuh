@@ -17,6 +17,55 @@ namespace pxq {
 
 constexpr double kInvTauC = kElectronMass * kLightSpeed * kLightSpeed / (kPlanck / (2.0 * kPi));  // m c^2/hbar, 1/s
 
+// ---- classical radiation reaction below the chi threshold (R24) ---------------------------------
+// A lepton with chi < chi_min loses kinetic energy at the classical radiated power, the chi -> 0 limit of the mean loss of
+// the Monte Carlo emission: d(gamma-1)/dt = -(2/3)(alpha/tau_C) chi^2 (gamma-1)/gamma; direction kept, norm(p') from gamma'.
+// One streaming pass: nine 128-bit loads per thread, chi^2 in fp64 registers (the routine of the evolve pass), and the three
+// momentum vectors stored back only where a lepton of the vector was below the threshold.
+template <typename R>
+__global__ void __launch_bounds__(256) classical_loss_kernel(R* __restrict__ px, R* __restrict__ py, R* __restrict__ pz,
+                                                             const R* __restrict__ ex, const R* __restrict__ ey,
+                                                             const R* __restrict__ ez, const R* __restrict__ bx,
+                                                             const R* __restrict__ by, const R* __restrict__ bz, long long n,
+                                                             double c2_min, double loss_dt /* (2/3)(alpha/tau_C) dt */) {
+    constexpr int V = 16 / sizeof(R);
+    const long long nvec = n / V;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const unsigned long long pol = l2_policy_evict_first();
+    auto one = [&](R& x, R& y, R& z, R e0, R e1, R e2, R b0, R b1, R b2) -> bool {
+        double inv_g, g2;
+        const double c2 = chi_squared_of<0>(x, y, z, e0, e1, e2, b0, b1, b2, &inv_g, &g2);
+        const double p2 = g2 - 1.0;
+        if (!(c2 < c2_min) || !(p2 > 1e-300)) return false;
+        const double g = g2 * inv_g;
+        const double k = p2 * rcp_fast(g + 1.0);                       // gamma - 1
+        double k2 = k - loss_dt * c2 * (k * inv_g);
+        k2 = k2 > 0.0 ? k2 : 0.0;
+        const double q2 = k2 * (k2 + 2.0);
+        const double s = q2 > 1e-300 ? q2 * rsqrt_fast(q2) * rsqrt_fast(p2) : 0.0;
+        x = (R)(s * x); y = (R)(s * y); z = (R)(s * z);
+        return true;
+    };
+    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < nvec; j += stride) {
+        const long long i = j * V;
+        Vec<R, V> x = ld_stream_rw<R, V>(px + i, pol), y = ld_stream_rw<R, V>(py + i, pol), z = ld_stream_rw<R, V>(pz + i, pol);
+        const Vec<R, V> a3 = ld_stream<R, V>(ex + i, pol), a4 = ld_stream<R, V>(ey + i, pol), a5 = ld_stream<R, V>(ez + i, pol),
+                        a6 = ld_stream<R, V>(bx + i, pol), a7 = ld_stream<R, V>(by + i, pol), a8 = ld_stream<R, V>(bz + i, pol);
+        bool any = false;
+#pragma unroll
+        for (int v = 0; v < V; ++v) any = one(x.v[v], y.v[v], z.v[v], a3.v[v], a4.v[v], a5.v[v], a6.v[v], a7.v[v], a8.v[v]) || any;
+        if (any) {
+            st_vec<R, V>(px + i, x);
+            st_vec<R, V>(py + i, y);
+            st_vec<R, V>(pz + i, z);
+        }
+    }
+    for (long long i = nvec * V + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        R x = px[i], y = py[i], z = pz[i];
+        if (one(x, y, z, ex[i], ey[i], ez[i], bx[i], by[i], bz[i])) { px[i] = x; py[i] = y; pz[i] = z; }
+    }
+}
+
 // ---- Boris push in a uniform field (R19) ---------------------------------------------------------------
 // ke = s dt/(2 tau_C) e, kb = s dt/(2 tau_C) b (host, fp64).  Arithmetic in fp64 registers whatever R.
 struct BorisArgs {

@@ -183,6 +183,7 @@ template <typename R, int SPECIES>
 __device__ __forceinline__ R rate_from_c2(double c2, double inv_g, double g2, const R* tab, const Table1D<R>& T,
                                           double rate_dt) {
     typedef R A;
+    if (c2 < T.c2_event_min) return (A)0;   // below the chi threshold of PAPER.md:340 neither process is an event (R24)
     A lc;
     if constexpr (sizeof(R) == 8) lc = 0.5 * log_pos(c2); else lc = 0.5f * logf((float)c2);
     const A ln_min = (A)T.ln_min, ln_max = (A)T.ln_max, inv_delta = (A)T.inv_delta;
@@ -261,7 +262,7 @@ __device__ __forceinline__ void decrement_vec(const R (&in)[9][V], const R* tab,
         }
         exp_fast_v<V>(L, ex);
 #pragma unroll
-        for (int v = 0; v < V; ++v) d[v] = rate_dt * ex[v] * inv_g[v];
+        for (int v = 0; v < V; ++v) d[v] = c2[v] < T.c2_event_min ? 0.0 : rate_dt * ex[v] * inv_g[v];
     } else {
         const float ln_min = (float)T.ln_min, ln_max = (float)T.ln_max, inv_delta = (float)T.inv_delta;
 #pragma unroll
@@ -269,7 +270,7 @@ __device__ __forceinline__ void decrement_vec(const R (&in)[9][V], const R* tab,
             float lc = 0.5f * logf((float)c2[v]);
             lc = lc < ln_min ? ln_min : (lc > ln_max ? ln_max : lc);
             const float L = lookup_ln<R, float>(tab, T.n, lc, ln_min, inv_delta);
-            d[v] = (float)rate_dt * expf(SPECIES == 1 ? L + lc : L) * (float)inv_g[v];
+            d[v] = c2[v] < T.c2_event_min ? 0.0f : (float)rate_dt * expf(SPECIES == 1 ? L + lc : L) * (float)inv_g[v];
         }
     }
 }

@@ -59,6 +59,7 @@ struct picsarqed_ctx {
     const void* staged_tau = nullptr;
     long long staged_n = 0;
     int staged_species = -1, staged_dtype = -1, staged_tau_dtype = -1;
+    double chi_event_min = 0.0;   // PAPER.md:340 (picsarqed_set_chi_threshold): no event below it; 0 = off
     int step_spill = 0;          // fused kernel: 1 = a streaming warp whose queue is full hands the chunk to the record path
     int step_batch_wait = 0;     // fused kernel: polls (2 us each) an event warp waits for four chunks before it takes fewer
     int step_config = 0;         // fused kernel: see launch_fused_step
@@ -241,6 +242,7 @@ Table1D<R> view_1d(const picsarqed_ctx* c, int species) {
     t.inv_delta = (t.n - 1) / (t.ln_max - t.ln_min);
     t.chi_min = lo;
     t.chi_max = hi;
+    t.c2_event_min = c->chi_event_min * c->chi_event_min;
     return t;
 }
 
@@ -1317,6 +1319,38 @@ extern "C" int picsarqed_boris_push_uniform(picsarqed_ctx* c, int dtype, long lo
     return PICSARQED_OK;
 }
 
+extern "C" int picsarqed_set_chi_threshold(picsarqed_ctx* c, double chi_min) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (!(chi_min >= 0.0) || !std::isfinite(chi_min)) return fail(c, PICSARQED_ERR_INVALID, "set_chi_threshold: chi_min must be >= 0");
+    c->chi_event_min = chi_min;
+    return PICSARQED_OK;
+}
+
+extern "C" int picsarqed_classical_loss(picsarqed_ctx* c, int dtype, long long n, void* px, void* py, void* pz, const void* ex,
+                                        const void* ey, const void* ez, const void* bx, const void* by, const void* bz,
+                                        double dt) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (c->unit_system != PICSARQED_UNITS_LIBRARY)
+        return fail(c, PICSARQED_ERR_INVALID, "the closed-loop calls take the library's own units");
+    if (n < 0) return fail(c, PICSARQED_ERR_INVALID, "bad n");
+    if (dtype != PICSARQED_F64 && dtype != PICSARQED_F32) return fail(c, PICSARQED_ERR_DTYPE, "bad dtype");
+    if (n == 0 || c->chi_event_min == 0.0) return PICSARQED_OK;
+    const void* a[9] = {px, py, pz, ex, ey, ez, bx, by, bz};
+    if (int rc = check_arrays(c, a, 9)) return rc;
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    const double c2_min = c->chi_event_min * c->chi_event_min, loss_dt = (2.0 / 3.0) * kAlphaOverTauC * dt;
+    if (dtype == PICSARQED_F64)
+        classical_loss_kernel<double><<<stream_grid(c, (n + 1) / 2, 256), 256, 0, c->stream>>>(
+            (double*)px, (double*)py, (double*)pz, (const double*)ex, (const double*)ey, (const double*)ez, (const double*)bx,
+            (const double*)by, (const double*)bz, n, c2_min, loss_dt);
+    else
+        classical_loss_kernel<float><<<stream_grid(c, (n + 3) / 4, 256), 256, 0, c->stream>>>(
+            (float*)px, (float*)py, (float*)pz, (const float*)ex, (const float*)ey, (const float*)ez, (const float*)bx,
+            (const float*)by, (const float*)bz, n, c2_min, loss_dt);
+    PXQ_CUDA(c, cudaGetLastError());
+    return PICSARQED_OK;
+}
+
 extern "C" int picsarqed_append_secondaries(picsarqed_ctx* c, int dtype, int tau_dtype, long long m_max, const void* s_px,
                                             const void* s_py, const void* s_pz, const void* s_tau,
                                             const unsigned long long* d_count, double min_energy, void* d_px, void* d_py,
@@ -1443,6 +1477,10 @@ extern "C" int picsarqed_cascade_step(picsarqed_ctx* c, int dtype, int tau_dtype
     if (push) {
         if (int rc = picsarqed_boris_push_uniform(c, dtype, n_e, el->px, el->py, el->pz, -1, e, b, dt)) return rc;
         if (int rc = picsarqed_boris_push_uniform(c, dtype, n_p, po->px, po->py, po->pz, +1, e, b, dt)) return rc;
+    }
+    if (c->chi_event_min > 0.0) {   // below the threshold the leptons radiate classically (R24)
+        if (int rc = picsarqed_classical_loss(c, dtype, n_e, el->px, el->py, el->pz, f[0], f[1], f[2], f[3], f[4], f[5], dt)) return rc;
+        if (int rc = picsarqed_classical_loss(c, dtype, n_p, po->px, po->py, po->pz, f[0], f[1], f[2], f[3], f[4], f[5], dt)) return rc;
     }
     if (n_e > 0)
         if (int rc = picsarqed_qed_step(c, 0, dtype, tau_dtype, n_e, el->px, el->py, el->pz, f[0], f[1], f[2], f[3], f[4], f[5],

@@ -39,6 +39,7 @@ struct Table1D {      // ln G or ln T on a log-spaced chi grid
     double ln_max;    // ln chi_{n-1}
     double inv_delta; // (n-1)/(ln_max - ln_min)
     double chi_min, chi_max;
+    double c2_event_min;  // square of the chi threshold of PAPER.md:340 (picsarqed_set_chi_threshold; 0 = off): no event below
 };
 
 template <typename R>

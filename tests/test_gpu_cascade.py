@@ -225,3 +225,78 @@ def test_cascade_capacity_overflow_is_reported(orc, qed, ctx, cas):
         for s in range(40):
             ctx.cascade_step(pops, (0, 0, 0), (0, 0, 9e-3), 1e-17, 23, s)
     assert pops["photons"].n == pops["photons"].capacity
+
+
+# ----------------------------------------------------------------------------- chi threshold + classical model
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("n", [70001, 3])
+def test_classical_loss_and_threshold(orc, qed, ctx, mid_tables, dtype, n):
+    """picsarqed_set_chi_threshold / picsarqed_classical_loss against the oracle: below the threshold the optical depth
+    does not move and the momentum shrinks by the classical power; at or above it nothing changes"""
+    import torch
+    species = LEPTON
+    p, e, b = qed.workloads.config1(seed=61, n=n, species=species, dtype=dtype)
+    thr, dt = 0.05, 4e-16
+    tabs = mid_tables.with_fp32_reads(np.dtype(dtype) == np.float32).with_chi_event_min(thr)
+    chi = orc.chi(species, p, e, b)
+    near = np.abs(chi - thr) <= 1e-6 * thr                      # (fp32: which side of the threshold is a rounding matter)
+    low = (chi < thr) & ~near
+    dp, de, db = to_dev(p), to_dev(e), to_dev(b)
+    ctx.set_chi_threshold(thr)
+    try:
+        ctx.classical_loss(dp, de, db, dt)
+        got = to_host(dp)
+        ref = orc.classical_loss(code(dtype), p, e, b, dt, thr)
+        tol = 1e-9 if dtype == np.float64 else 1e-5
+        norm = np.sqrt(sum(np.asarray(a, np.float64) ** 2 for a in p))
+        for g_, r_, p_ in zip(got, ref, p):
+            ok = ~near
+            assert np.all(np.abs(g_[ok].astype(np.float64) - r_[ok]) <= tol * norm[ok])
+            assert np.array_equal(g_[~low & ~near], p_[~low & ~near])                 # untouched, bit for bit
+        if n > 10:
+            assert 0.1 * n < low.sum() < 0.9 * n
+        # the evolve pass with the threshold: tau of the particles below it does not move
+        for sp in (LEPTON, PHOTON):
+            p2, e2, b2 = qed.workloads.config1(seed=62, n=n, species=sp, dtype=dtype)
+            chi2 = orc.chi(sp, p2, e2, b2)
+            tau0 = orc.init_optical_depth(sp, code(dtype), n, 4).astype(dtype)
+            dtau = torch.from_numpy(tau0.copy()).cuda()
+            ctx.evolve_optical_depth(sp, to_dev(p2), to_dev(e2), to_dev(b2), 1e-15, dtau)
+            o = orc.evolve_optical_depth(tabs, sp, code(dtype), p2, e2, b2, 1e-15, tau0)
+            g_tau = dtau.cpu().numpy()
+            clear = np.abs(chi2 - thr) > 1e-6 * thr
+            assert np.array_equal(g_tau[(chi2 < thr) & clear], tau0[(chi2 < thr) & clear])
+            fin = clear & np.isfinite(o["tau_exact"])
+            assert np.all(np.abs(g_tau[fin].astype(np.float64) - o["tau_exact"][fin]) <= tol * (np.abs(tau0[fin]) + o["decr"][fin]))
+    finally:
+        ctx.set_chi_threshold(0.0)
+
+
+def test_cascade_with_chi_threshold_fp64(orc, qed, ctx, cas, mid_tables):
+    """the closed loop with the WarpX-side chi threshold: Ridgers case (i) with a threshold above the
+    electrons' chi = 1 would switch everything off, so the threshold sits inside the population a cascade produces"""
+    n, g0, b0, steps = 3000, 1000.0, 9e-3, 30
+    thr = 2.0                                                   # chi_0 = 9: primaries above, most secondaries below
+    pops, opops = _start(qed, ctx, orc, cas, n, g0, 23, np.float64, np.float64, 40 * n)
+    tabs = mid_tables.with_chi_event_min(thr)
+    e, b = (0.0, 0.0, 0.0), (0.0, 0.0, b0)
+    dt = 1e-16 / steps
+    ctx.set_chi_threshold(thr)
+    try:
+        for s in range(steps):
+            ev = ctx.cascade_step(pops, e, b, dt, 23, s, photon_min_energy=2.0)
+            r = cas.cascade_step(tabs, orc.F64, orc.F64, opops, e, b, dt, 23, s, photon_min_energy=2.0)
+            assert ev == tuple(r["events"]), (s, ev, r["events"])
+    finally:
+        ctx.set_chi_threshold(0.0)
+    for k in pops:
+        assert pops[k].n == opops[k].n
+        gp, gt = _state(pops[k])
+        op = opops[k].p
+        norm = np.sqrt(sum(a * a for a in op))
+        for c in range(3):
+            assert np.all(np.abs(gp[c] - op[c]) <= 1e-9 * norm), (k, c)
+    # the classical model acted: some electrons sit below the threshold and lost energy without emitting
+    el_p, _ = _state(pops["electrons"])
+    g = np.sqrt(1 + sum(a * a for a in el_p))
+    assert (g * b0 < thr).any()
