@@ -42,6 +42,11 @@ extern "C" {
 #define PICSARQED_ERR_CUDA 2     /* a CUDA runtime call failed; see picsarqed_last_error        */
 #define PICSARQED_ERR_NO_TABLES 4 /* build_tables / import_tables has not been called           */
 #define PICSARQED_ERR_DTYPE 5    /* unsupported dtype combination                              */
+/* There is no "capacity exceeded" status (SURVEY.md 8(b) proposed an all-or-nothing status 3): when more particles fire than
+ * the output buffers hold, the first `capacity` fired parents (in index order) are processed, the later ones are left
+ * exactly as the evolve pass left them (optical depth still negative, momentum untouched) and *d_n_out receives the TOTAL
+ * number that fired, so the caller sees the overflow by comparing it with `capacity` and can run generate_* again on the
+ * same arrays with fresh buffers (R16). */
 
 #define PICSARQED_F32 0
 #define PICSARQED_F64 1
@@ -85,7 +90,9 @@ const char* picsarqed_last_error(const picsarqed_ctx* ctx);
 int picsarqed_version(void);
 /* Tuning knobs (integers): "evolve_unroll" in {0 (default), 1, 2, 4} = independent 128-bit
  * loads per array per thread in the evolve kernel; "evolve_ctas_per_sm" (0 = occupancy limit);
- * "event_config" 0..7 = (threads, chunks per tile) of the event kernel; "time_kernels" 0/1;
+ * "event_config" 0..1 = shape of the event kernel; "time_kernels" 0/1; "stage_records" 0/1 (see
+ * evolve_optical_depth); "fused_step" 0/1 = qed_step as one warp-specialised kernel (experimental, slower today: DESIGN.md 11),
+ * with "step_config", "step_spill", "step_batch_wait" its tuning knobs;
  * "host_slabs" 0..64 = number of slabs step_host pipelines (0 = automatic: slabs of at least
  * 2^20 particles, at most 32; 1 = copy in, step, copy out, one after the other). */
 int picsarqed_set_option(picsarqed_ctx* ctx, const char* name, long long value);
@@ -168,7 +175,12 @@ int picsarqed_init_optical_depth(picsarqed_ctx* ctx, int species, int tau_dtype,
  *            eq.23 inside the table, the Erber form of eq.10 outside (R2);
  *            photons with gamma_gamma <= 2 or tau = +inf never decay (R12).
  * *d_n_events (device, 8 bytes, may be NULL) is overwritten with the number of tau[i] < 0
- * after the update (R1). */
+ * after the update (R1).
+ * Option "stage_records" = 1: the call also stages, in context scratch, the record (momentum, chi^2, index) of every
+ * particle that fired, and the next generate_photons / generate_pairs call on the SAME tau pointer, n, species and
+ * dtypes takes them instead of re-scanning tau and gathering the parents (the two calls then cost what qed_step costs).
+ * The caller promises that momenta, fields and optical depths are not modified between the two calls; any other call
+ * in between drops the staged records. */
 int picsarqed_evolve_optical_depth(picsarqed_ctx* ctx, int species, int dtype, int tau_dtype, long long n,
                                    const void* px, const void* py, const void* pz,
                                    const void* ex, const void* ey, const void* ez,
@@ -324,7 +336,9 @@ typedef struct picsarqed_species_arrays {
  * (one 24-byte device-to-host read per step) and writes the event counts (electrons, positrons,
  * photons) to h_events[3] if it is not NULL.  Scratch (constant field arrays, secondary buffers) is
  * owned by the context.  PICSARQED_ERR_INVALID if a species would exceed its capacity (its n is
- * then clipped to the capacity and the entries that did not fit are lost). */
+ * then clipped to the capacity and the entries that did not fit are lost).  * The Philox counter distinguishes leptons from photons only, so electrons and positrons must own disjoint id ranges
+ * [id_base, id_base + capacity) (e.g. 0 and 2^40; R21): cascade_step returns PICSARQED_ERR_INVALID otherwise.
+ */
 int picsarqed_cascade_step(picsarqed_ctx* ctx, int dtype, int tau_dtype,
                            picsarqed_species_arrays* electrons, picsarqed_species_arrays* positrons,
                            picsarqed_species_arrays* photons, const double* e, const double* b, double dt,

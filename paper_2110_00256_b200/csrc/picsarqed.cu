@@ -35,6 +35,7 @@ struct picsarqed_ctx {
     size_t tab_n[4] = {0, 0, 0, 0};
     // search guides of the two CDF tables (see Table2D::guide), [0] photon emission, [1] pair production
     unsigned short* guide[2] = {nullptr, nullptr};
+    size_t guide_bytes[2] = {0, 0};
     double guide_k0[2] = {0.0, 0.0}, guide_inv_dk[2] = {0.0, 0.0};
     double* d_scalar = nullptr;
 
@@ -202,10 +203,16 @@ __global__ void guide_kernel(const double* __restrict__ tab, int n_rows, int n_c
 
 int build_guides(picsarqed_ctx* c) {
     for (int kind = 0; kind < 2; ++kind) {
-        if (c->guide[kind]) cudaFree(c->guide[kind]);
-        c->guide[kind] = nullptr;
         const int rows = rows_2d(c->tp, kind), cols = kind == 0 ? c->tp.qs_n_xi : c->tp.bw_n_xi;
-        if (cols > 65535) continue;  // indices are stored in 16 bits; wider tables are searched unguided
+        const size_t want = (size_t)rows * (kGuideBins + 1) * sizeof(unsigned short);
+        if (c->guide[kind] && c->guide_bytes[kind] != want) {   // (a rebuild of the same geometry keeps its buffer)
+            cudaFree(c->guide[kind]);
+            c->guide[kind] = nullptr;
+        }
+        unsigned short* keep = c->guide[kind];
+        c->guide[kind] = nullptr;                                // (no guide while it is being rebuilt, or if it cannot be built)
+        auto drop = [&]() { if (keep) cudaFree(keep); keep = nullptr; c->guide_bytes[kind] = 0; };
+        if (cols > 65535) { drop(); continue; }  // indices are stored in 16 bits; wider tables are searched unguided
         const double* tab = c->tab64[kind == 0 ? PICSARQED_TAB_QS_LNP : PICSARQED_TAB_BW_P];
         double k0 = 0.0, k1 = 0.5;
         if (kind == 0) {
@@ -214,10 +221,12 @@ int build_guides(picsarqed_ctx* c) {
             PXQ_CUDA(c, cudaMemcpyAsync(&k0, c->d_scalar, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
             PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
             k1 = 0.0;
-            if (!std::isfinite(k0) || !(k0 < 0.0)) continue;
+            if (!std::isfinite(k0) || !(k0 < 0.0)) { drop(); continue; }
         }
         const double dk = (k1 - k0) / kGuideBins;
-        PXQ_CUDA(c, cudaMalloc(&c->guide[kind], (size_t)rows * (kGuideBins + 1) * sizeof(unsigned short)));
+        if (!keep) PXQ_CUDA(c, cudaMalloc(&keep, want));
+        c->guide_bytes[kind] = want;
+        c->guide[kind] = keep;
         guide_kernel<<<c->num_sms * 4, 256, 0, c->stream>>>(tab, rows, cols, k0, dk, kGuideBins, c->guide[kind]);
         PXQ_CUDA(c, cudaGetLastError());
         c->guide_k0[kind] = k0;
@@ -304,7 +313,7 @@ int picsarqed_create(picsarqed_ctx** out, int cuda_device, void* cuda_stream) {
     if (e == cudaSuccess) e = cudaMalloc(&c->d_cas, 16 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_cas, 16 * sizeof(unsigned long long));
     if (e != cudaSuccess) {
-        delete c;
+        picsarqed_destroy(c);   // (frees whatever was allocated: every pointer starts as NULL)
         return PICSARQED_ERR_CUDA;
     }
     *out = c;
@@ -713,6 +722,17 @@ int launch_events(picsarqed_ctx* c, long long n, void* const* p, const void* con
                                           d_n_out);
 }
 
+// the three timing events of a step ("time_kernels"): handed to the context when the step was enqueued, destroyed otherwise
+struct StepEvents {
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    bool kept = false;
+    ~StepEvents() {
+        if (!kept)
+            for (cudaEvent_t e : ev)
+                if (e) cudaEventDestroy(e);
+    }
+};
+
 // qed_step, fused (step.cuh): streaming warps evolve, event warps of the same CTA generate the events and rewrite the
 // parents while their sectors are in L2; then the offsets scan and the placement of the staged secondaries
 template <typename R, typename TR, int SPECIES, int EW, int D, int REG_S, int REG_E>
@@ -791,7 +811,8 @@ int launch_fused_step_c(picsarqed_ctx* c, long long n, void* const* p, const voi
     PXQ_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const long long ntiles = n / kTile;
     const int grid = (int)std::max<long long>(1, std::min<long long>(ntiles, (long long)c->num_sms));
-    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    StepEvents se;
+    cudaEvent_t* ev = se.ev;
     if (c->time_kernels) {
         for (int k = 0; k < 3; ++k) PXQ_CUDA(c, cudaEventCreate(&ev[k]));
         PXQ_CUDA(c, cudaEventRecord(ev[0], c->stream));
@@ -808,6 +829,7 @@ int launch_fused_step_c(picsarqed_ctx* c, long long n, void* const* p, const voi
     if (c->time_kernels) {
         PXQ_CUDA(c, cudaEventRecord(ev[2], c->stream));
         for (int k = 0; k < 3; ++k) c->timing_events.push_back(ev[k]);
+        se.kept = true;
     }
     return PICSARQED_OK;
 }
@@ -844,7 +866,8 @@ int launch_step(picsarqed_ctx* c, long long n, void* const* p, const void* const
     sv.remove_photons = 1;
     const void* a9[9] = {p[0], p[1], p[2], eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]};
     constexpr int U = kChunk / (32 * (16 / (int)sizeof(R)));  // fp64: 2, fp32: 1
-    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    StepEvents se;
+    cudaEvent_t* ev = se.ev;
     if (c->time_kernels) {
         for (int k = 0; k < 3; ++k) PXQ_CUDA(c, cudaEventCreate(&ev[k]));
         PXQ_CUDA(c, cudaEventRecord(ev[0], c->stream));
@@ -861,6 +884,7 @@ int launch_step(picsarqed_ctx* c, long long n, void* const* p, const void* const
     if (c->time_kernels) {
         PXQ_CUDA(c, cudaEventRecord(ev[2], c->stream));
         for (int k = 0; k < 3; ++k) c->timing_events.push_back(ev[k]);
+        se.kept = true;
     }
     return PICSARQED_OK;
 }
@@ -1158,9 +1182,15 @@ extern "C" int picsarqed_step_host(picsarqed_ctx* c, int species, int dtype, int
         PXQ_CUDA(c, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
         c->slab_events.push_back(e);
     }
-    struct LinkReset {  // the link must not outlive this call, whatever path leaves it
-        picsarqed_ctx* c;
-        ~LinkReset() { c->link_slot_base = nullptr; c->link_parent_base = 0; }
+    struct LinkReset {  // the link must not outlive this call, whatever path leaves it -- and no copy into or out of the
+        picsarqed_ctx* c;   // caller's host buffers may still be in flight when the call returns, error or not
+        ~LinkReset() {
+            c->link_slot_base = nullptr;
+            c->link_parent_base = 0;
+            cudaStreamSynchronize(c->h2d_stream);
+            cudaStreamSynchronize(c->stream);
+            cudaStreamSynchronize(c->d2h_stream);
+        }
     } link_reset{c};
     PXQ_CUDA(c, cudaMemsetAsync(c->d_counts, 0, sizeof(unsigned long long), c->stream));
     for (int s = 0; s < n_slabs; ++s) {
@@ -1420,6 +1450,14 @@ extern "C" int picsarqed_cascade_step(picsarqed_ctx* c, int dtype, int tau_dtype
     for (int k = 0; k < 3; ++k)
         if (sp[k]->n < 0 || sp[k]->capacity < sp[k]->n) return fail(c, PICSARQED_ERR_INVALID, "species: bad n or capacity");
     if (!c->have_tables) return fail(c, PICSARQED_ERR_NO_TABLES, "no tables: call build_tables or import_tables");
+    {
+        // the Philox counter holds the species only as lepton / photon: an electron and a positron with the
+        // same id would draw the same numbers, so the two arrays must own disjoint id ranges (R21: 0 and 2^40)
+        const unsigned long long e0 = el->id_base, e1 = e0 + (unsigned long long)el->capacity;
+        const unsigned long long p0 = po->id_base, p1 = p0 + (unsigned long long)po->capacity;
+        if (el->capacity > 0 && po->capacity > 0 && e0 < p1 && p0 < e1)
+            return fail(c, PICSARQED_ERR_INVALID, "cascade_step: the id ranges [id_base, id_base + capacity) of electrons and positrons overlap");
+    }
     PXQ_CUDA(c, cudaSetDevice(c->device));
     const size_t es = dtype ? 8 : 4, ts = tau_dtype ? 8 : 4;
     auto pad = [](size_t x) { return (x + 255) & ~(size_t)255; };

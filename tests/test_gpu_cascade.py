@@ -300,3 +300,13 @@ def test_cascade_with_chi_threshold_fp64(orc, qed, ctx, cas, mid_tables):
     el_p, _ = _state(pops["electrons"])
     g = np.sqrt(1 + sum(a * a for a in el_p))
     assert (g * b0 < thr).any()
+
+
+def test_cascade_rejects_overlapping_lepton_id_ranges(qed, ctx):
+    """electrons and positrons share the lepton Philox stream: equal id ranges would give pair partners the same draws"""
+    import torch
+    pops = {k: qed.Species(1024, torch.float64, torch.float64, 0 if k != "photons" else 1 << 41)
+            for k in ("electrons", "positrons", "photons")}
+    pops["electrons"].n = 8
+    with pytest.raises(qed.PicsarQedError):
+        ctx.cascade_step(pops, (0.0, 0.0, 0.0), (0.0, 0.0, 1e-3), 1e-17, 1, 0)
