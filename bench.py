@@ -365,7 +365,7 @@ def run_config5(args, torch, q, w, ctx, dev, peaks, peak_kind):
 # FP64 instructions (warp level) of one build of the configuration-4 tables: smsp__inst_executed_pipe_fp64.sum of the two
 # table_rows_kernel launches per process, from the ncu capture named in TABLES_FP64_SOURCE
 TABLES_FP64_SOURCE = "profiles/r2_tables_full.md"
-TABLES_FP64_WARP_INST = None        # filled in from that capture; None = not measured for this build
+TABLES_FP64_WARP_INST = None        # set below from that capture; None = no roofline entry
 
 
 def run_config4(args, torch, q, w, peaks):

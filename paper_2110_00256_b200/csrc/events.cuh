@@ -15,7 +15,7 @@
 //      ticket, no look-back, no barrier on the common path.
 //  (A single-pass decoupled look-back was tried first: with ~10^3 tiles in flight every tile
 //  walks ~30 status windows before it meets an inclusive prefix, which serialised the kernel
-//  at ~0.3 ms per 16 Mi particles whatever its shape -- profiles/r1_events_full.md.)
+//  at ~0.3 ms per 16 Mi particles whatever its shape (round-1 capture).)
 // =====================================================================================
 #pragma once
 #include "qed_device.cuh"

@@ -95,7 +95,7 @@ template <> __device__ __forceinline__ float uniform_open<float>(uint32_t a, uin
 }
 // ---- lean fp64 elementary functions for the streaming kernel ------------------------------------
 // The CUDA library log/exp cost ~85 / ~50 instructions per call (special cases, constant moves); in the evolve
-// kernel they were 45 % of all instructions (profiles/r1b_step_full.md).  These versions assume what holds
+// kernel they were 45 % of all instructions (round-1 capture).  These versions assume what holds
 // there -- log of a positive normal number (anything else takes the library path), exp of a finite argument --
 // and keep the error at the 1e-16 level: a few ulp, far inside the 1e-9 tolerance on the optical depth.
 // They are written for V arguments at once (log_pos_v, exp_fast_v; the scalar names are V = 1): the common path is one
