@@ -179,7 +179,7 @@ __device__ __forceinline__ double log_grid(double vmin, double vmax, int n, int 
 }
 
 template <int KIND>  // 0: photon emission (QS), 1: Breit-Wheeler
-__global__ void __launch_bounds__(kTabThreads) table_rows_kernel(const TableBuildArgs a) {
+__global__ void __launch_bounds__(kTabThreads, 3) table_rows_kernel(const TableBuildArgs a) {
     extern __shared__ double cell[];  // n_xi cell integrals, then the cumulative row
     __shared__ double warp_tot[kTabThreads / 32];
     const int row = blockIdx.x, M = a.n_xi;
