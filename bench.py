@@ -155,14 +155,20 @@ def run_reference(args):
     dt = w.choose_dt(oracle.rate(oracle_tables_from(tp, tables), 0, p0, e0, b0), 0.05)  # the 5 % rule
     for _ in range(max(0, min(args.warmup, 1))):
         time_oracle(tp, tables, min(n, 1 << 16), 1, dt)
-    # bound the run: at ~4e6 particle-steps/s an 8 Mi sample takes ~2 s per step
-    steps_run = min(steps, 8)
+    # bound the run: the oracle does ~4e6 particle-steps/s on 16 cores; the arm honours --particles (through --cpu-sample)
+    # and --steps up to a wall-time cap, and says what it ran
+    wall_cap_s = 60.0
+    probe_n = min(n, 1 << 20)
+    _, probe_sec, _ = time_oracle(tp, tables, probe_n, 1, dt)
+    per_step = probe_sec * n / probe_n
+    steps_run = int(max(1, min(steps, wall_cap_s // max(per_step, 1e-9))))
     value, sec, threads = time_oracle(tp, tables, n, steps_run, dt)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps_run,
             "warmup": args.warmup, "ms_per_step": 1e3 * sec / steps_run, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "config 2 (synchrotron emission, fp64), oracle on host cores", "particles": n,
-                       "tables": "1024 / 1024x1024 (stand-in values, same shape)"},
+                       "tables": "1024 / 1024x1024 (stand-in values, same shape)", "steps_asked": steps,
+                       "steps_run": steps_run, "wall_cap_s": wall_cap_s},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
                              "sample": "%d particles x %d steps (evolve + photon emission)" % (n, steps_run)},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}

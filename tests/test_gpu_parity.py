@@ -460,6 +460,36 @@ def test_fused_step(orc, qed, ctx, mid_tables, species, dtype, tdtype, n, target
             assert f["n_fired"] > 0.5 * target * n
 
 
+@pytest.mark.parametrize("species", [LEPTON, PHOTON])
+@pytest.mark.parametrize("dtype,tdtype", DTYPES, ids=IDS)
+@pytest.mark.parametrize("config", [0, 1])
+def test_fused_kernel_matches_the_two_kernel_step(orc, qed, ctx, mid_tables, species, dtype, tdtype, config):
+    """option "fused_step" (step.cuh: TMA-staged streaming warps + event warps, parents rewritten while their sectors are in
+    L2): bit for bit what the default evolve pass + event pass give -- all tiles, a ragged end, chunks with more than 24
+    events, a capacity below the number of events (the undo path of the placement), both register configurations"""
+    for n, target in ((9 * 2048 + 777, 0.06), (2 * 2048 + 5, 0.5), (300, 0.06)):
+        p, e, b = qed.workloads.config1(seed=51, n=n, species=species, dtype=dtype)
+        tables = _tables_for(mid_tables, dtype)
+        dt = qed.workloads.choose_dt(orc.rate(tables, species, p, e, b), target)
+        tau0 = orc.init_optical_depth(species, code(tdtype), n, 7).astype(tdtype)
+        for cap in (n, max(1, n // 50)):
+            ref = _run_fused(qed, ctx, species, dtype, tdtype, p, e, b, tau0, dt, 5, 3, 1 << 35, cap)
+            ctx.set_option("fused_step", 1)
+            ctx.set_option("step_config", config)
+            try:
+                got = _run_fused(qed, ctx, species, dtype, tdtype, p, e, b, tau0, dt, 5, 3, 1 << 35, cap)
+            finally:
+                ctx.set_option("fused_step", 0)
+                ctx.set_option("step_config", 0)
+            assert got["n_fired"] == ref["n_fired"] and _same(got["parent"], ref["parent"])
+            assert _same(got["tau"], ref["tau"]) and all(_same(x, y) for x, y in zip(got["p"], ref["p"]))
+            for s_ in range(len(ref["sec_p"])):
+                assert all(_same(x, y) for x, y in zip(got["sec_p"][s_], ref["sec_p"][s_]))
+                assert _same(got["sec_tau"][s_], ref["sec_tau"][s_])
+            if n > 2048:
+                assert ref["n_fired"] > 0.5 * target * n
+
+
 def test_staged_records_are_dropped_when_not_consumed(orc, qed, ctx, mid_tables):
     """"stage_records": records staged by an evolve call that no generate call consumes (another evolve, another array,
     another size in between) must not leak into the next event pass"""
