@@ -368,10 +368,11 @@ def run_config5(args, torch, q, w, ctx, dev, peaks, peak_kind):
     return leg
 
 
-# FP64 instructions (warp level) of one build of the configuration-4 tables: smsp__inst_executed_pipe_fp64.sum of the two
-# table_rows_kernel launches per process, from the ncu capture named in TABLES_FP64_SOURCE
+# FP64 warp instructions (DFMA + DMUL + DADD + DSETP, counted on the source page) of one build of the configuration-4 tables,
+# summed over the four table_rows_kernel launches, from the ncu capture named in TABLES_FP64_SOURCE.  A profile figure of
+# that build of the library; the live part of the roofline entry is the duration (CUDA events inside the library).
 TABLES_FP64_SOURCE = "profiles/r2_tables_full.md"
-TABLES_FP64_WARP_INST = None        # set below from that capture; None = no roofline entry
+TABLES_FP64_WARP_INST = 5036057619
 
 
 def run_config4(args, torch, q, w, peaks):
@@ -668,28 +669,22 @@ def run_cascade(args):
 
 
 def run_tables(args):
-    """BASELINE config 4: picsarqed_build_tables on 4096 log-spaced chi points over [1e-4, 1e3], 2048 xi columns,
-    both processes (the 2D tables carry all 4096 rows: DESIGN.md 4).  Time per build, median of `steps`."""
+    """BASELINE config 4 alone (the entry `other_configs` carries in the default run), as its own JSON line"""
     import torch
 
     import paper_2110_00256_b200 as q
     from paper_2110_00256_b200 import workloads as w
     torch.cuda.set_device(0)
-    ctx = q.Context(0)
-    tp = q.TableParams(**w.table_params(4))
-    times = []
-    for _ in range(max(1, args.warmup) + max(1, min(args.steps, 10))):
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        ctx.build_tables(tp)                      # synchronises
-        times.append(time.perf_counter() - t0)
-    ms = 1e3 * float(np.median(times[max(1, args.warmup):]))
-    cells = 2 * tp.qs_n_chi * tp.qs_n_xi
-    print(json.dumps({"metric": "table build time (BASELINE config 4)", "value": ms, "unit": "ms", "n_gpus": 1,
-                      "steps": len(times) - max(1, args.warmup), "warmup": max(1, args.warmup), "ms_per_step": ms,
-                      "higher_is_better": False, "dtype": "f64", "data": "synthetic",
-                      "config": {"workload": "4096-point lnG, lnT on [1e-4, 1e3]; two 4096 x 2048 CDF tables",
-                                 "cells": cells, "cells_per_s": cells / (ms * 1e-3)}}), flush=True)
+    peaks, _ = measured_peaks()
+    leg = run_config4(args, torch, q, w, peaks)
+    line = {"metric": "table build time (BASELINE config 4)", "value": leg["value"], "unit": "ms", "n_gpus": 1, "steps": 5,
+            "warmup": 2, "ms_per_step": leg["value"], "higher_is_better": False, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": leg["workload"], "cells": leg["cells"], "cells_per_s": leg["cells_per_s"],
+                       "quadrature_kernels_ms": leg["quadrature_kernels_ms"]}}
+    for k in ("roofline", "cpu_baseline"):
+        if k in leg:
+            line[k] = leg[k]
+    print(json.dumps(line), flush=True)
 
 
 def main():
