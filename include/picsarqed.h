@@ -208,6 +208,31 @@ int picsarqed_generate_photons(picsarqed_ctx* ctx, int dtype, int tau_dtype, lon
                                void* ph_px, void* ph_py, void* ph_pz, void* ph_tau,
                                long long* ph_parent, unsigned long long* d_n_out);
 
+/* generate_photons_noalloc: picsarqed_generate_photons for callers that must not allocate (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Same operation (PAPER.md:165,
+ * :255-267 eqs.28-30), same arguments, same results bit for bit, same ordering, capacity rule and d_n_out;
+ * the caller still passes every input and output.  What differs is the scratch of the compaction (chunk
+ * counts, tile sums, tile offsets): it is a file-scope device array of 459 264 bytes inside the library, which
+ * every GPU that loads the library holds until the process exits, instead of a buffer the context grows with
+ * cudaMalloc.  The call issues no cudaMalloc, cudaFree or allocating library routine: one cudaMemsetAsync of
+ * the tile sums (they must start at zero; the array keeps the last call's contents) and three kernels on the
+ * context's stream.  (The tables must be there already: build_tables / import_tables allocate.)
+ * Limit: n <= PICSARQED_NOALLOC_MAX_N (16 Mi particles per call); a larger n returns
+ * PICSARQED_ERR_INVALID with a message naming the limit, and nothing is enqueued.
+ * EVERY call on a device -- from any context, any stream -- shares the one array: calls that overlap on the
+ * GPU race.  Calls on one stream, or ordered by events, are safe.  If the context holds records staged by
+ * evolve_optical_depth ("stage_records"), they are dropped. */
+#define PICSARQED_NOALLOC_MAX_N (1ll << 24)
+int picsarqed_generate_photons_noalloc(picsarqed_ctx* ctx, int dtype, int tau_dtype, long long n,
+                                       void* px, void* py, void* pz, /* in/out */
+                                       const void* ex, const void* ey, const void* ez,
+                                       const void* bx, const void* by, const void* bz,
+                                       void* tau, /* in/out */
+                                       unsigned long long seed, unsigned long long step,
+                                       unsigned long long id_base, long long capacity,
+                                       void* ph_px, void* ph_py, void* ph_pz, void* ph_tau,
+                                       long long* ph_parent, unsigned long long* d_n_out);
+
 /* generate_pairs (eqs.24-26): every photon with tau < 0 becomes an
  * electron-positron pair, chi_-/chi_gamma = xi by inverse-CDF lookup in P_BW on
  * r' = min(r, 1-r) (r <= 1/2: the electron takes xi, else 1-xi),

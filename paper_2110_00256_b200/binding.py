@@ -16,6 +16,7 @@ F32, F64 = 0, 1
 LEPTON, PHOTON = 0, 1
 UNITS_LIBRARY, UNITS_SI, UNITS_NORM_OMEGA, UNITS_NORM_LAMBDA, UNITS_HL_MEV = 0, 1, 2, 3, 4
 TAB_LNG, TAB_QS_LNP, TAB_LNT, TAB_BW_P = 0, 1, 2, 3
+NOALLOC_MAX_N = 1 << 24   # PICSARQED_NOALLOC_MAX_N
 
 _vp, _u64, _i64, _i, _d = C.c_void_p, C.c_uint64, C.c_longlong, C.c_int, C.c_double
 
@@ -78,6 +79,7 @@ _SIGNATURES = {
     "picsarqed_init_optical_depth": (_i, [_vp, _i, _i, _i64, _u64, _u64, _vp]),
     "picsarqed_evolve_optical_depth": (_i, [_vp, _i, _i, _i, _i64] + [_vp] * 9 + [_d, _vp, _vp]),
     "picsarqed_generate_photons": (_i, [_vp, _i, _i, _i64] + [_vp] * 10 + [_u64, _u64, _u64, _i64] + [_vp] * 6),
+    "picsarqed_generate_photons_noalloc": (_i, [_vp, _i, _i, _i64] + [_vp] * 10 + [_u64, _u64, _u64, _i64] + [_vp] * 6),
     "picsarqed_generate_pairs": (_i, [_vp, _i, _i, _i64] + [_vp] * 10 + [_u64, _u64, _u64, _i64] + [_vp] * 10),
     "picsarqed_qed_step": (_i, [_vp, _i, _i, _i, _i64] + [_vp] * 10 + [_d, _u64, _u64, _u64, _i64] + [_vp] * 10),
     "picsarqed_read_count": (_i, [_vp, _vp, C.POINTER(_u64)]),
@@ -239,6 +241,15 @@ class Context:
         d = p[0].dtype
         ptrs = [_dev(t, d) for t in (*p, *e, *b)]
         self._check(lib().picsarqed_generate_photons(
+            self._h, _code(d), _code(tau.dtype), tau.numel(), *ptrs, _dev(tau), seed, step, id_base, capacity,
+            *[_dev(t, d) for t in ph_p], _dev(ph_tau, tau.dtype),
+            _dev(ph_parent, torch.int64) if ph_parent is not None else None, _dev(n_out, torch.int64)))
+
+    def generate_photons_noalloc(self, p, e, b, tau, seed, step, id_base, capacity, ph_p, ph_tau, ph_parent, n_out):
+        """generate_photons on the library's static scratch: allocates nothing, n <= NOALLOC_MAX_N"""
+        d = p[0].dtype
+        ptrs = [_dev(t, d) for t in (*p, *e, *b)]
+        self._check(lib().picsarqed_generate_photons_noalloc(
             self._h, _code(d), _code(tau.dtype), tau.numel(), *ptrs, _dev(tau), seed, step, id_base, capacity,
             *[_dev(t, d) for t in ph_p], _dev(ph_tau, tau.dtype),
             _dev(ph_parent, torch.int64) if ph_parent is not None else None, _dev(n_out, torch.int64)))

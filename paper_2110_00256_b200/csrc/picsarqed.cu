@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -274,6 +275,37 @@ Table2D<R> view_2d(const picsarqed_ctx* c, int species) {
     return t;
 }
 
+// ---- the scratch of picsarqed_generate_photons_noalloc (include/picsarqed.h): chunk counts, tile offsets, tile sums
+// of up to kNoAllocMaxN particles, laid out as chunk_scratch lays them out, in a file-scope device array that every
+// GPU which loads the library holds until exit.  In host code the array's NAME is a host-side stand-in, not a device
+// address: the address a kernel can use comes from cudaGetSymbolAddress, once per device, with that device current.
+constexpr long long kNoAllocMaxN = 1ll << 24;
+constexpr long long kNoAllocChunks = kNoAllocMaxN / kChunk;
+constexpr size_t kNoAllocSumBytes = ((size_t)(kNoAllocChunks / 8 + 2) * sizeof(unsigned int) + 255) & ~(size_t)255;
+constexpr size_t kNoAllocCntBytes = ((size_t)kNoAllocChunks * sizeof(unsigned short) + 255) & ~(size_t)255;
+constexpr size_t kNoAllocOffBytes = ((size_t)(kNoAllocChunks / 8 + 2) * sizeof(unsigned long long) + 255) & ~(size_t)255;
+constexpr size_t kNoAllocBytes = kNoAllocSumBytes + kNoAllocCntBytes + kNoAllocOffBytes;   // 459 264 bytes
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocBytes];
+
+constexpr int kNoAllocMaxDevices = 64;
+std::mutex g_noalloc_mutex;
+void* g_noalloc_ptr[kNoAllocMaxDevices] = {};
+
+// the device address of g_noalloc_scratch on `device`, which must be the current device
+cudaError_t noalloc_scratch_address(int device, void** out) {
+    *out = nullptr;
+    if (device < 0 || device >= kNoAllocMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[device]) {
+        void* ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);
+        if (e != cudaSuccess) return e;
+        g_noalloc_ptr[device] = ptr;
+    }
+    *out = g_noalloc_ptr[device];
+    return cudaSuccess;
+}
+
 }  // namespace
 
 // =====================================================================================
@@ -317,6 +349,10 @@ int picsarqed_create(picsarqed_ctx** out, int cuda_device, void* cuda_stream) {
         return PICSARQED_ERR_CUDA;
     }
     *out = c;
+    {   // set-up of the no-alloc entry point: the device is current here (a failure is reported by that entry point)
+        void* scratch = nullptr;
+        (void)noalloc_scratch_address(cuda_device, &scratch);
+    }
     // PICSARQED_OPTIONS="name=value,name=value": set_option calls applied to every new context (tuning experiments)
     if (const char* env = std::getenv("PICSARQED_OPTIONS")) {
         std::string all(env);
@@ -722,6 +758,18 @@ int launch_events(picsarqed_ctx* c, long long n, void* const* p, const void* con
                                           d_n_out);
 }
 
+// the unstaged path of launch_events on a scratch the caller laid out (picsarqed_generate_photons_noalloc: the static array)
+template <typename R, typename TR, int KIND>
+int launch_events_on(picsarqed_ctx* c, long long n, const ChunkScratch& cs, void* const* p, const void* const* eb, void* tau,
+                     unsigned long long seed, unsigned long long step, unsigned long long id_base, long long capacity,
+                     void* const* out_p, void* const* out_tau, long long* parent, unsigned long long* d_n_out) {
+    const int grid = (int)std::max<long long>(1, std::min<long long>((cs.n_chunks + 7) / 8, (long long)c->num_sms * 8));
+    count_chunks_kernel<TR><<<grid, 256, 0, c->stream>>>((const TR*)tau, n, 0, cs.n_chunks, cs.cnt, cs.sum,
+                                                         event_chunks_per_tile(c));
+    return launch_event_pass<R, TR, KIND>(c, n, cs, p, eb, tau, seed, step, id_base, capacity, out_p, out_tau, parent,
+                                          d_n_out);
+}
+
 // the three timing events of a step ("time_kernels"): handed to the context when the step was enqueued, destroyed otherwise
 struct StepEvents {
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
@@ -1076,6 +1124,57 @@ int picsarqed_generate_pairs(picsarqed_ctx* c, int dtype, int tau_dtype, long lo
     PXQ_DISPATCH_RT(c, dtype, tau_dtype,
                     return (launch_events<R, TR, 1>(c, n, p, eb, tau, seed, step, id_base, capacity, out_p, out_tau,
                                                     parent, d_n_out)));
+}
+
+// generate_photons on the static scratch: no cudaMalloc, cudaFree or allocating library call on this path
+int picsarqed_generate_photons_noalloc(picsarqed_ctx* c, int dtype, int tau_dtype, long long n, void* px, void* py,
+                                       void* pz, const void* ex, const void* ey, const void* ez, const void* bx,
+                                       const void* by, const void* bz, void* tau, unsigned long long seed,
+                                       unsigned long long step, unsigned long long id_base, long long capacity,
+                                       void* ph_px, void* ph_py, void* ph_pz, void* ph_tau, long long* ph_parent,
+                                       unsigned long long* d_n_out) {
+    if (!c) return PICSARQED_ERR_INVALID;
+    if (n < 0 || capacity < 0 || !d_n_out) return fail(c, PICSARQED_ERR_INVALID, "bad n, capacity or d_n_out");
+    if (n > kNoAllocMaxN)
+        return fail(c, PICSARQED_ERR_INVALID,
+                    "generate_photons_noalloc: n = " + std::to_string(n) + " exceeds the static scratch (at most " +
+                        std::to_string(kNoAllocMaxN) + " particles per call); use picsarqed_generate_photons");
+    if (!c->have_tables) return fail(c, PICSARQED_ERR_NO_TABLES, "no tables: call build_tables or import_tables");
+    PXQ_CUDA(c, cudaSetDevice(c->device));
+    void* scratch = nullptr;
+    PXQ_CUDA(c, noalloc_scratch_address(c->device, &scratch));
+    if (n == 0) {
+        PXQ_CUDA(c, cudaMemsetAsync(d_n_out, 0, sizeof(unsigned long long), c->stream));
+        return PICSARQED_OK;
+    }
+    void* p[3] = {px, py, pz};
+    const void* eb[6] = {ex, ey, ez, bx, by, bz};
+    const void* chk[10] = {px, py, pz, ex, ey, ez, bx, by, bz, tau};
+    if (int rc = check_arrays(c, chk, 10)) return rc;
+    void* out_p[6] = {ph_px, ph_py, ph_pz, nullptr, nullptr, nullptr};
+    void* out_tau[2] = {ph_tau, nullptr};
+    if (capacity > 0) {
+        const void* o[4] = {ph_px, ph_py, ph_pz, ph_tau};
+        if (int rc = check_arrays(c, o, 4)) return rc;
+    }
+    if (c->staged_valid) {
+        // records staged by evolve_optical_depth ("stage_records") describe arrays this call is about to rewrite: dropped
+        if (c->rec) PXQ_CUDA(c, cudaMemsetAsync(c->rec, 0, c->rec_sum_bytes, c->stream));
+        c->staged_valid = false;
+    }
+    // [tile sums][counts][offsets]; every call shares the array and finds the last call's contents in it: the tile
+    // sums are accumulated by atomics and must start at zero (the counts and offsets are written before they are read)
+    ChunkScratch cs;
+    cs.sum = static_cast<unsigned int*>(scratch);
+    cs.rec = static_cast<unsigned char*>(scratch) + kNoAllocSumBytes;   // no staged records: never dereferenced
+    cs.cnt = reinterpret_cast<unsigned short*>(static_cast<unsigned char*>(scratch) + kNoAllocSumBytes);
+    cs.off = reinterpret_cast<unsigned long long*>(static_cast<unsigned char*>(scratch) + kNoAllocSumBytes + kNoAllocCntBytes);
+    cs.n_chunks = (n + kChunk - 1) / kChunk;
+    cs.stride = 0;
+    PXQ_CUDA(c, cudaMemsetAsync(cs.sum, 0, kNoAllocSumBytes, c->stream));
+    PXQ_DISPATCH_RT(c, dtype, tau_dtype,
+                    return (launch_events_on<R, TR, 0>(c, n, cs, p, eb, tau, seed, step, id_base, capacity, out_p, out_tau,
+                                                       ph_parent, d_n_out)));
 }
 
 }  // extern "C"
