@@ -169,7 +169,7 @@ int narrow_tables(picsarqed_ctx* c) {
     return PICSARQED_OK;
 }
 
-constexpr int kGuideBins = 256;
+constexpr int kGuideBins = 1024;
 
 // minimum of column 0 over the rows (lower end of the key range of the photon-emission guide)
 __global__ void column0_min_kernel(const double* __restrict__ tab, int n_rows, int n_cols, double* out) {

@@ -324,6 +324,7 @@ __device__ __forceinline__ void row_bracket(const Table2D<R>& T, double ln_chi, 
 // The guide entries of a key (four 16-bit loads that depend on the row and the key only: the callers issue them together
 // with whatever else they load first, one round trip instead of two).
 struct GuideBracket { int lo, hi; bool guided; };
+constexpr int kGuideFastSpan = 8;   // brackets up to this wide are closed in one round trip (search_row)
 template <typename R>
 __device__ __forceinline__ GuideBracket guide_bracket(const Table2D<R>& T, int k, double key) {
     GuideBracket g;
@@ -351,12 +352,40 @@ __device__ __forceinline__ int search_row(const Table2D<R>& T, int k, double w, 
     const R* __restrict__ r1 = r0 + M;
     auto ell = [&](int m) { const double a = (double)__ldg(r0 + m); return fma(w, (double)__ldg(r1 + m) - a, a); };
     int lo = gb.lo, hi = gb.hi;
-    bool verified = !gb.guided;
+    if (gb.guided && hi - lo >= 1 && hi - lo <= kGuideFastSpan) {
+        // the common case (99 % of the events with the 1024-bin guide): the bracket is a few columns wide, so its ends
+        // (the verification) and its interior are fetched in ONE round trip and counted
+        const int span = hi - lo;
+        double v[kGuideFastSpan + 1];
+#pragma unroll
+        for (int q = 0; q <= kGuideFastSpan; ++q) v[q] = q <= span ? ell(lo + q) : 0.0;
+        double top = v[0];
+        int cnt = 0;
+#pragma unroll
+        for (int q = 1; q <= kGuideFastSpan; ++q) {
+            if (q == span) top = v[q];
+            cnt += (q <= span && v[q] <= key) ? 1 : 0;
+        }
+        if (v[0] <= key && (top > key || hi == M - 1)) {
+            if (cnt == span) --cnt;   // key at or above the last column (only with hi == M-1): the last interval
+            double a = v[0], b = v[1];
+#pragma unroll
+            for (int q = 1; q < kGuideFastSpan; ++q)
+                if (q == cnt) { a = v[q]; b = v[q + 1]; }
+            *a_out = a;
+            *b_out = b;
+            return lo + cnt;
+        }
+        lo = 0;                   // the bracket does not hold (a rounding of the bin index): the full range
+        hi = M - 1;
+    }
+    bool verified = !gb.guided || hi - lo == M - 1;
     bool have_vb = false;         // vb = ell(hi) is known (always, once a guide bracket has been verified)
     double va = 0.0, vb = 0.0;
     if (verified) va = ell(0);    // (unguided: hi = M-1, whose value is fetched at the end if it is still the upper end)
     while (true) {
         const int span = hi - lo;
+        if (verified && span <= 1) break;   // (closed: no probe left to make)
         const int step = (span + 8) / 9;
         double v[8];
 #pragma unroll
