@@ -327,10 +327,12 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
     const unsigned int off_lane = incl - cnt;
     const unsigned int total = __shfl_sync(0xffffffffu, incl, 31);
     if (total == 0) continue;
-    const unsigned int rescan_mask =
-        __ballot_sync(0xffffffffu, cnt > 0 && (cnt > (unsigned)kStageCap || (flags & kStageNoRecords) != 0));
-    const unsigned int done_mask = __ballot_sync(0xffffffffu, cnt > 0 && (flags & kStageDone) != 0);
-    const unsigned int pdone_mask = __ballot_sync(0xffffffffu, cnt > 0 && (flags & kStageParentDone) != 0);
+    unsigned int rescan_mask = 0, done_mask = 0, pdone_mask = 0;
+    if (__any_sync(0xffffffffu, cnt > (unsigned)kStageCap || (flags & ~kStageCountMask) != 0)) {   // (rarely: most tiles are plain)
+        rescan_mask = __ballot_sync(0xffffffffu, cnt > 0 && (cnt > (unsigned)kStageCap || (flags & kStageNoRecords) != 0));
+        done_mask = __ballot_sync(0xffffffffu, cnt > 0 && (flags & kStageDone) != 0);
+        pdone_mask = __ballot_sync(0xffffffffu, cnt > 0 && (flags & kStageParentDone) != 0);
+    }
     if (rescan_mask) {  // chunks without records: find their fired particles again (tau < 0), in index order
         __syncthreads();  // (every warp is done with the list of the previous tile that needed one)
         for (int j = warp; j < CHUNKS; j += WARPS) {
@@ -350,6 +352,7 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
     }
     for (unsigned int e0 = 0; e0 < total; e0 += THREADS) {
         const unsigned int e = e0 + tid;
+        if (e0 + (unsigned)(tid & ~31) >= total) break;   // (the whole warp is past the tile's last event)
         // chunk of event e: the largest j with off_j <= e (ties are empty chunks followed by the one that holds
         // e; lanes past the last chunk carry off = total > e); the offsets live in the lanes' registers
         int j = 0;

@@ -137,6 +137,10 @@ __global__ void narrow_kernel(const double* __restrict__ src, float* __restrict_
         dst[i] = (float)src[i];
 }
 
+// elements of zero padding behind every table: 16-byte TMA copies of the 1D tables and the unconditional column loads of
+// search_row's fast path (kGuideFastSpan columns past the bracket) stay in bounds
+constexpr size_t kTablePad = 16;
+
 // (re)allocate table storage for params p; +2 elements of padding so that 16-byte TMA copies stay in bounds
 int alloc_tables(picsarqed_ctx* c, const picsarqed_table_params& p) {
     size_t n[4];
@@ -148,11 +152,11 @@ int alloc_tables(picsarqed_ctx* c, const picsarqed_table_params& p) {
             c->tab64[k] = nullptr;
             c->tab32[k] = nullptr;
             c->tab_n[k] = 0;
-            PXQ_CUDA(c, cudaMalloc(&c->tab64[k], (n[k] + 4) * sizeof(double)));
-            PXQ_CUDA(c, cudaMalloc(&c->tab32[k], (n[k] + 4) * sizeof(float)));
+            PXQ_CUDA(c, cudaMalloc(&c->tab64[k], (n[k] + kTablePad) * sizeof(double)));
+            PXQ_CUDA(c, cudaMalloc(&c->tab32[k], (n[k] + kTablePad) * sizeof(float)));
         }
-        PXQ_CUDA(c, cudaMemsetAsync(c->tab64[k], 0, (n[k] + 4) * sizeof(double), c->stream));
-        PXQ_CUDA(c, cudaMemsetAsync(c->tab32[k], 0, (n[k] + 4) * sizeof(float), c->stream));
+        PXQ_CUDA(c, cudaMemsetAsync(c->tab64[k], 0, (n[k] + kTablePad) * sizeof(double), c->stream));
+        PXQ_CUDA(c, cudaMemsetAsync(c->tab32[k], 0, (n[k] + kTablePad) * sizeof(float), c->stream));
         c->tab_n[k] = n[k];
     }
     c->tp = p;
@@ -268,6 +272,7 @@ Table2D<R> view_2d(const picsarqed_ctx* c, int species) {
     t.ln_max = std::log(hi);
     t.inv_delta = (t.n_chi - 1) / (t.ln_max - t.ln_min);
     t.ln_xi_min = species == 0 ? std::log(p.qs_xi_min) : 0.0;
+    t.xi_step = species == 0 ? -t.ln_xi_min / (double)(t.n_xi - 1) : 0.5 / (double)(t.n_xi - 1);
     t.guide = c->guide[species];
     t.guide_bins = kGuideBins;
     t.guide_k0 = c->guide_k0[species];

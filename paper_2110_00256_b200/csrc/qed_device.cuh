@@ -48,6 +48,7 @@ struct Table2D {      // rows: log-spaced chi; columns: xi grid
     int n_chi, n_xi;
     double ln_min, ln_max, inv_delta;
     double ln_xi_min; // QS only: ln(xi_min)
+    double xi_step;   // column spacing: ln xi_{m+1} - ln xi_m (QS), xi_{m+1} - xi_m (BW); the host's division
     // search guide (may be null): guide[n * (bins + 1) + j] = max{m : P[n][m] <= key_j} (0 if none, and for j = 0),
     // key_j = guide_k0 + j / guide_inv_dk: narrows the binary search of eq.25 / eq.29 without changing its result
     const unsigned short* guide;
@@ -354,19 +355,20 @@ __device__ __forceinline__ int search_row(const Table2D<R>& T, int k, double w, 
     int lo = gb.lo, hi = gb.hi;
     if (gb.guided && hi - lo >= 1 && hi - lo <= kGuideFastSpan) {
         // the common case (99 % of the events with the 1024-bin guide): the bracket is a few columns wide, so its ends
-        // (the verification) and its interior are fetched in ONE round trip and counted
+        // (the verification) and its interior are fetched in ONE round trip and counted.
         const int span = hi - lo;
         double v[kGuideFastSpan + 1];
 #pragma unroll
         for (int q = 0; q <= kGuideFastSpan; ++q) v[q] = q <= span ? ell(lo + q) : 0.0;
-        double top = v[0];
         int cnt = 0;
+        bool top_le = false;
 #pragma unroll
         for (int q = 1; q <= kGuideFastSpan; ++q) {
-            if (q == span) top = v[q];
-            cnt += (q <= span && v[q] <= key) ? 1 : 0;
+            const bool le = q <= span && v[q] <= key;
+            cnt += le ? 1 : 0;
+            if (q == span) top_le = le;
         }
-        if (v[0] <= key && (top > key || hi == M - 1)) {
+        if (v[0] <= key && (!top_le || hi == M - 1)) {
             if (cnt == span) --cnt;   // key at or above the last column (only with hi == M-1): the last interval
             double a = v[0], b = v[1];
 #pragma unroll
@@ -448,7 +450,7 @@ __device__ __forceinline__ double qs_sample_xi_ln(const Table2D<R>& T, double ln
     if (lr < fma(w, e0b - e0a, e0a)) return exp_fast(T.ln_xi_min);  // below the first column (R6)
     double a, b;
     const int ms = search_row(T, k, w, lr, gb, &a, &b);        // eq.29
-    const double step = -T.ln_xi_min / (double)(M - 1);        // ln xi_{m+1} - ln xi_m
+    const double step = T.xi_step;                             // ln xi_{m+1} - ln xi_m
     const double lx0 = T.ln_xi_min + step * (double)ms;
     if (!(b > a)) return exp_fast(lx0);
     return exp_fast(fma((lr - a) * rcp_fast(b - a), step, lx0));   // eq.30
@@ -467,7 +469,7 @@ __device__ __forceinline__ double bw_sample_xi(const Table2D<R>& T, double ln_ch
     double a, b;
     const GuideBracket gb = guide_bracket(T, k, rp);
     const int ms = search_row(T, k, w, rp, gb, &a, &b);        // eq.25 (P(0) = 0 <= r')
-    const double step = 0.5 / (double)(M - 1);
+    const double step = T.xi_step;
     const double x0 = step * (double)ms;
     if (!(b > a)) return x0;
     return fma((rp - a) * rcp_fast(b - a), step, x0);          // eq.26
