@@ -173,7 +173,7 @@ int narrow_tables(picsarqed_ctx* c) {
     return PICSARQED_OK;
 }
 
-constexpr int kGuideBins = 1024;
+constexpr int kGuideBins = 2048;   // measured: 256 -> 1024 -> 2048 -> 4096 bins: config 5 event passes 1.77 -> 1.63 -> 1.58 -> 1.55 ms
 
 // minimum of column 0 over the rows (lower end of the key range of the photon-emission guide)
 __global__ void column0_min_kernel(const double* __restrict__ tab, int n_rows, int n_cols, double* out) {
