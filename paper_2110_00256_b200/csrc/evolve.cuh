@@ -40,6 +40,8 @@ struct EvolveArgs {
     UnitScales units;           // the caller's unit system (picsarqed_set_units)
 };
 
+constexpr int kEventTileChunks = 32;        // chunks per tile of event_kernel (the tile sums are kept per 32 chunks: a shift,
+                                            // not a 64-bit division, in the kernels that count)
 constexpr int kChunk = 128;                 // particles one warp handles per tile: the unit of record staging
 constexpr int kStageCap = 24;               // records per chunk segment (mean at 5 % firing: 6.4)
 // stage_cnt[chunk]: bits 0..14 = number of particles of the chunk that fired; bit 15 = the chunk has no staged
@@ -237,18 +239,6 @@ __device__ __forceinline__ void decrement_vec(const R (&in)[9][V], const R* tab,
                                                  in[8][v] * us.b, &inv_g[v], &g2[v])
                        : chi_squared_of<SPECIES>(in[0][v], in[1][v], in[2][v], in[3][v], in[4][v], in[5][v], in[6][v],
                                                  in[7][v], in[8][v], &inv_g[v], &g2[v]);
-    if constexpr (SPECIES == 1) {
-        // photons that cannot decay or lie outside the T table (Erber form): the general routine, one by one
-        bool plain = true;
-        const double lo2 = T.chi_min * T.chi_min, hi2 = T.chi_max * T.chi_max;
-#pragma unroll
-        for (int v = 0; v < V; ++v) plain = plain && g2[v] > 4.0 && c2[v] >= lo2 && c2[v] <= hi2;
-        if (!plain) {
-#pragma unroll
-            for (int v = 0; v < V; ++v) d[v] = rate_from_c2<R, SPECIES>(c2[v], inv_g[v], g2[v], tab, T, rate_dt);
-            return;
-        }
-    }
     if constexpr (sizeof(R) == 8) {
         double lc[V], L[V], ex[V];
         log_pos_v<V>(c2, lc);
@@ -271,6 +261,18 @@ __device__ __forceinline__ void decrement_vec(const R (&in)[9][V], const R* tab,
             lc = lc < ln_min ? ln_min : (lc > ln_max ? ln_max : lc);
             const float L = lookup_ln<R, float>(tab, T.n, lc, ln_min, inv_delta);
             d[v] = c2[v] < T.c2_event_min ? 0.0f : (float)rate_dt * expf(SPECIES == 1 ? L + lc : L) * (float)inv_g[v];
+        }
+    }
+    if constexpr (SPECIES == 1) {
+        // photons that cannot decay (R12) or lie outside the T table (Erber form): their value replaces
+        // the clamped lookup's, one particle at a time -- the in-table photons of the warp pay nothing for them but the
+        // branch (as rate_from_c2 decides, in its order)
+        const double lo2 = T.chi_min * T.chi_min, hi2 = T.chi_max * T.chi_max;
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            if (!(g2[v] > 4.0) || !(c2[v] > 0.0)) d[v] = (R)0;
+            else if (c2[v] < lo2 || c2[v] > hi2)
+                d[v] = (c2[v] < T.c2_event_min || c2[v] < 1.7777e-4) ? (R)0 : erber_decrement<R>(c2[v], inv_g[v], rate_dt);
         }
     }
 }
@@ -366,7 +368,7 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                     a.stage_cnt[chunk] = (unsigned short)(total <= (unsigned)kStageCap
                                                               ? (SPECIES == 1 && total > 0 && a.remove_photons ? (total | kStageParentDone) : total)
                                                               : (total | kStageNoRecords));
-                    if (total > 0) atomicAdd(a.tile_sum + chunk / a.chunks_per_tile, total);
+                    if (total > 0) atomicAdd(a.tile_sum + chunk / kEventTileChunks, total);
                 }
                 if (total > 0 && total <= (unsigned)kStageCap) {  // (overflow: the event kernel re-scans the chunk)
                     // records are assembled in this warp's shared-memory buffer (scattered writes are cheap there)
@@ -473,7 +475,7 @@ __global__ void __launch_bounds__(256) chi_kernel(const R* __restrict__ px, cons
         const double p2 = fma(x, x, fma(y, y, z * z));
         const double g = sqrt(SPECIES == 0 ? 1.0 + p2 : p2);
         return (R)sqrt(chi_squared<SPECIES>(x, y, z, exr * us.e, eyr * us.e, ezr * us.e, bxr * us.b, byr * us.b,
-                                            bzr * us.b, g, p2));
+                                            bzr * us.b, g, p2 > 1e-300 ? rcp_fast(p2) : 0.0));
     };
     const unsigned long long pol = l2_policy_evict_first();
     for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < nvec; j += stride) {

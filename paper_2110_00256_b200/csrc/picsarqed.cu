@@ -657,7 +657,7 @@ int chunk_scratch(picsarqed_ctx* c, long long n, size_t seg_bytes, ChunkScratch*
 // chunks per tile of the configured event_kernel shape
 int event_chunks_per_tile(const picsarqed_ctx* c) {
     (void)c;
-    return 32;  // both shapes of launch_event_pass
+    return kEventTileChunks;  // both shapes of launch_event_pass (the counting kernels rely on it)
 }
 
 template <typename R, typename TR, int SPECIES>
@@ -733,8 +733,8 @@ int launch_event_pass(picsarqed_ctx* c, long long n, const ChunkScratch& cs, voi
         kern<<<grid, T, 0, c->stream>>>(ev);                                                                 \
     } while (0)
     switch (c->event_config) {
-        case 1: PXQ_LAUNCH_EVENTS(256, 32, 3); break;
-        default: PXQ_LAUNCH_EVENTS(384, 32, 2); break;  // measured best on B200 (config 2: 1-4 us ahead of (256, 24, 3))
+        case 1: PXQ_LAUNCH_EVENTS(256, kEventTileChunks, 3); break;
+        default: PXQ_LAUNCH_EVENTS(384, kEventTileChunks, 2); break;  // measured best on B200 (config 2: 1-4 us ahead of (256, 24, 3))
     }
 #undef PXQ_LAUNCH_EVENTS
     PXQ_CUDA(c, cudaGetLastError());

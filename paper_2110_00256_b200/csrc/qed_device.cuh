@@ -219,9 +219,8 @@ template <> __device__ __forceinline__ float draw_tau<float>(uint32_t a, uint32_
 // Returns chi^2; *g2_out = g^2 (= 1 + p^2 or p^2).
 template <int SPECIES>
 __device__ __forceinline__ double chi_squared(double px, double py, double pz, double ex, double ey, double ez,
-                                              double bx, double by, double bz, double g, double p2) {
+                                              double bx, double by, double bz, double g, double q) {   // q = 1/p^2 (0 for p = 0)
     const double d = fma(px, ex, fma(py, ey, pz * ez));  // p.e
-    const double q = p2 > 1e-300 ? rcp_fast(p2) : 0.0;
     const double t = d * q;
     const double fx = fma(-t, px, ex), fy = fma(-t, py, ey), fz = fma(-t, pz, ez);  // e_perp
     const double cx = fma(py, bz, -pz * by), cy = fma(pz, bx, -px * bz), cz = fma(px, by, -py * bx);
@@ -241,7 +240,9 @@ __device__ __forceinline__ double chi_squared_of(double px, double py, double pz
     const double inv_g = g2 > 1e-300 ? rsqrt_fast(g2) : 0.0;  // 1/gamma (lepton) or 1/gamma_gamma (photon)
     *inv_g_out = inv_g;
     *g2_out = g2;
-    return chi_squared<SPECIES>(px, py, pz, ex, ey, ez, bx, by, bz, g2 * inv_g, p2);
+    // 1/p^2: a photon's is (1/gamma_gamma)^2, the reciprocal square root squared (one multiplication)
+    const double q = SPECIES == 1 ? inv_g * inv_g : (p2 > 1e-300 ? rcp_fast(p2) : 0.0);
+    return chi_squared<SPECIES>(px, py, pz, ex, ey, ez, bx, by, bz, g2 * inv_g, q);
 }
 
 // ---- K_{1/3}(x), only for the Erber branch outside the T table -------------------------

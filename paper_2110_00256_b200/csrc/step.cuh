@@ -298,7 +298,7 @@ __global__ void __launch_bounds__((SW + EW) * 32, 1) step_kernel(const StepArgs<
                 if (lane == 0) {
                     a.stage_cnt[chunk] = (unsigned short)(total == 0 ? 0u : (publish ? (total | kStageDone)
                                                                                     : (queued ? total : (total | kStageNoRecords))));
-                    if (total > 0) atomicAdd(a.tile_sum + chunk / a.chunks_per_tile, total);
+                    if (total > 0) atomicAdd(a.tile_sum + chunk / kEventTileChunks, total);
                     if (publish) {
                         header[warp][n_pub % D].chunk = chunk;
                         header[warp][n_pub % D].total = total;
