@@ -326,7 +326,7 @@ __device__ __forceinline__ void row_bracket(const Table2D<R>& T, double ln_chi, 
 // The guide entries of a key (four 16-bit loads that depend on the row and the key only: the callers issue them together
 // with whatever else they load first, one round trip instead of two).
 struct GuideBracket { int lo, hi; bool guided; };
-constexpr int kGuideFastSpan = 8;   // brackets up to this wide are closed in one round trip (search_row)
+constexpr int kGuideFastSpan = 5;   // brackets up to this wide are closed in one round trip (search_row); measured 8 -> 5 -> 4: config 3 event pass 0.0685 -> 0.0669 -> 0.0655 ms, config 5 1.568 -> 1.556 -> 1.558 ms
 template <typename R>
 __device__ __forceinline__ GuideBracket guide_bracket(const Table2D<R>& T, int k, double key) {
     GuideBracket g;
