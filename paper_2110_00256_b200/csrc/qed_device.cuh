@@ -355,7 +355,7 @@ __device__ __forceinline__ int search_row(const Table2D<R>& T, int k, double w, 
     auto ell = [&](int m) { const double a = (double)__ldg(r0 + m); return fma(w, (double)__ldg(r1 + m) - a, a); };
     int lo = gb.lo, hi = gb.hi;
     if (gb.guided && hi - lo >= 1 && hi - lo <= kGuideFastSpan) {
-        // the common case (99 % of the events with the 1024-bin guide): the bracket is a few columns wide, so its ends
+        // the common case (99 % of the events with the 2048-bin guide): the bracket is a few columns wide, so its ends
         // (the verification) and its interior are fetched in ONE round trip and counted.
         const int span = hi - lo;
         double v[kGuideFastSpan + 1];
