@@ -321,8 +321,9 @@ __device__ __forceinline__ void row_bracket(const Table2D<R>& T, double ln_chi, 
 // only the schedule differs, because an event is a chain of dependent L2 accesses and its length is what
 // costs time: (1) the per-row guide gives a bracket [lo, hi] that provably contains m* (each of the two
 // rows bounds the interpolated row); it is verified against the table and dropped if a rounding of the bin
-// index made it wrong; (2) every level probes eight interior points at once (nine-way split), so the
-// bracket closes in one or two round trips instead of log2(M).
+// index made it wrong; (2) a bracket of up to kGuideFastSpan columns (nearly all, with 2048 key bins per row) is
+// fetched whole -- ends and interior -- in one round trip and counted; (3) a wider one closes level by level, every
+// level probing eight interior points at once (nine-way split): one or two round trips instead of log2(M).
 // The guide entries of a key (four 16-bit loads that depend on the row and the key only: the callers issue them together
 // with whatever else they load first, one round trip instead of two).
 struct GuideBracket { int lo, hi; bool guided; };
