@@ -316,8 +316,8 @@ __device__ __forceinline__ void row_bracket(const Table2D<R>& T, double ln_chi, 
 
 // ---- the search of eq.25 / eq.29 -------------------------------------------------------
 // Finds m* = max{m : ell(m) <= key} for the row interpolated between rows k and k+1 with weight w
-// (eq.24 / eq.28), clamped to M-2, and returns it with a = ell(m*), b = ell(m*+1).  Precondition:
-// ell(0) <= key.  The result is the one a plain bisection over [0, M-1] gives (ell is non-decreasing);
+// (eq.24 / eq.28), clamped to M-2, and returns it with a = ell(m*), b = ell(m*+1); -1 when key < ell(0)
+// (a photon-emission draw below the first column, R6; P_BW(0) = 0 never is).  The result is the one a plain bisection over [0, M-1] gives (ell is non-decreasing);
 // only the schedule differs, because an event is a chain of dependent L2 accesses and its length is what
 // costs time: (1) the per-row guide gives a bracket [lo, hi] that provably contains m* (each of the two
 // rows bounds the interpolated row); it is verified against the table and dropped if a rounding of the bin
@@ -380,13 +380,17 @@ __device__ __forceinline__ int search_row(const Table2D<R>& T, int k, double w, 
             *b_out = b;
             return lo + cnt;
         }
+        if (lo == 0 && !(v[0] <= key)) return -1;   // key below the first column
         lo = 0;                   // the bracket does not hold (a rounding of the bin index): the full range
         hi = M - 1;
     }
     bool verified = !gb.guided || hi - lo == M - 1;
     bool have_vb = false;         // vb = ell(hi) is known (always, once a guide bracket has been verified)
     double va = 0.0, vb = 0.0;
-    if (verified) va = ell(0);    // (unguided: hi = M-1, whose value is fetched at the end if it is still the upper end)
+    if (verified) {               // (unguided: hi = M-1, whose value is fetched at the end if it is still the upper end)
+        va = ell(0);
+        if (!(va <= key)) return -1;
+    }
     while (true) {
         const int span = hi - lo;
         if (verified && span <= 1) break;   // (closed: no probe left to make)
@@ -403,9 +407,11 @@ __device__ __forceinline__ int search_row(const Table2D<R>& T, int k, double w, 
             verified = true;
             have_vb = true;
             if (!(va <= key) || !(vb > key || hi == M - 1)) {  // guide bracket does not hold: full range
+                if (lo == 0 && !(va <= key)) return -1;
                 lo = 0;
                 hi = M - 1;
                 va = ell(0);
+                if (!(va <= key)) return -1;
                 have_vb = false;
                 continue;
             }
@@ -445,13 +451,10 @@ template <typename R>
 __device__ __forceinline__ double qs_sample_xi_ln(const Table2D<R>& T, double ln_chi, double lr) {
     int k; double w;
     row_bracket(T, ln_chi, &k, &w);
-    const int M = T.n_xi;
-    const R* __restrict__ r0 = T.P + (size_t)k * M;
-    const GuideBracket gb = guide_bracket(T, k, lr);           // (issued together with the first column)
-    const double e0a = (double)__ldg(r0), e0b = (double)__ldg(r0 + M);
-    if (lr < fma(w, e0b - e0a, e0a)) return exp_fast(T.ln_xi_min);  // below the first column (R6)
+    const GuideBracket gb = guide_bracket(T, k, lr);
     double a, b;
     const int ms = search_row(T, k, w, lr, gb, &a, &b);        // eq.29
+    if (ms < 0) return exp_fast(T.ln_xi_min);                  // below the first column (R6)
     const double step = T.xi_step;                             // ln xi_{m+1} - ln xi_m
     const double lx0 = T.ln_xi_min + step * (double)ms;
     if (!(b > a)) return exp_fast(lx0);
