@@ -81,7 +81,7 @@ __device__ __forceinline__ EventOut<R, TR> qs_event_compute(const EventArgs<R, T
         log_pos_v<2>(la, l2);
         lg[0] = l2[0]; lg[1] = l2[1]; lg[2] = lg[3] = 0.0;
     }
-    const double xi = qs_sample_xi_ln(a.cdf, 0.5 * lg[1], lg[0]);
+    const double xi = qs_sample_xi_ln(a.cdf, 0.5 * lg[1], lg[0], r);
     const double inv_pn = p2 > 1e-300 ? rsqrt_fast(p2) : 0.0;
     const double nx = px * inv_pn, ny = py * inv_pn, nz = pz * inv_pn;
     const double km1 = p2 * rcp_fast(g + 1.0);  // gamma - 1 without cancellation

@@ -189,13 +189,18 @@ __global__ void column0_min_kernel(const double* __restrict__ tab, int n_rows, i
     if (threadIdx.x == 0) *out = red[0];
 }
 
-// guide[n][j] = max{m : tab[n][m] <= k0 + j dk}, 0 if there is none and for j = 0 (whose lower edge is -inf)
-__global__ void guide_kernel(const double* __restrict__ tab, int n_rows, int n_cols, double k0, double dk, int bins,
+// guide[n][j] = max{m : tab[n][m] <= key_j}, 0 if there is none and for j = 0 (whose lower edge is -inf).
+// split = 0 (pair production: the table holds P, the key is r'): key_j = k0 + j dk.
+// split = 1 (photon emission: the table holds ln P, the key is ln r): the lower half of the bins is uniform in ln r on [k0, ln 1/2]
+// (dk = its spacing), the upper half uniform in r on [1/2, 1] -- with all bins uniform in ln r the last one, ln r in [-dk, 0], holds
+// the whole flat end of a low-chi row (hundreds of columns) and is hit by 0.5-1 % of the events: a quarter of the warps
+__global__ void guide_kernel(const double* __restrict__ tab, int n_rows, int n_cols, double k0, double dk, int bins, int split,
                              unsigned short* __restrict__ guide) {
     const long long total = (long long)n_rows * (bins + 1);
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
         const int n = (int)(t / (bins + 1)), j = (int)(t % (bins + 1));
-        const double key = k0 + j * dk;
+        double key = k0 + j * dk;
+        if (split && j >= bins / 2) key = j == bins ? 0.0 : log(0.5 + (j - bins / 2) * (0.5 / (bins / 2)));
         const double* row = tab + (size_t)n * n_cols;
         int lo = -1, hi = n_cols;  // row[lo] <= key < row[hi]
         while (hi - lo > 1) {
@@ -225,14 +230,15 @@ int build_guides(picsarqed_ctx* c) {
             column0_min_kernel<<<1, 256, 0, c->stream>>>(tab, rows, cols, c->d_scalar);
             PXQ_CUDA(c, cudaMemcpyAsync(&k0, c->d_scalar, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
             PXQ_CUDA(c, cudaStreamSynchronize(c->stream));
-            k1 = 0.0;
-            if (!std::isfinite(k0) || !(k0 < 0.0)) { drop(); continue; }
+            k1 = std::log(0.5);
+            if (!std::isfinite(k0) || !(k0 < k1)) { drop(); continue; }
         }
-        const double dk = (k1 - k0) / kGuideBins;
+        // (photon emission: the lower half of the bins covers [k0, ln 1/2] uniformly in ln r, the upper half [1/2, 1] uniformly in r)
+        const double dk = (k1 - k0) / (kind == 0 ? kGuideBins / 2 : kGuideBins);
         if (!keep) PXQ_CUDA(c, cudaMalloc(&keep, want));
         c->guide_bytes[kind] = want;
         c->guide[kind] = keep;
-        guide_kernel<<<c->num_sms * 4, 256, 0, c->stream>>>(tab, rows, cols, k0, dk, kGuideBins, c->guide[kind]);
+        guide_kernel<<<c->num_sms * 4, 256, 0, c->stream>>>(tab, rows, cols, k0, dk, kGuideBins, kind == 0 ? 1 : 0, c->guide[kind]);
         PXQ_CUDA(c, cudaGetLastError());
         c->guide_k0[kind] = k0;
         c->guide_inv_dk[kind] = 1.0 / dk;
@@ -275,6 +281,7 @@ Table2D<R> view_2d(const picsarqed_ctx* c, int species) {
     t.xi_step = species == 0 ? -t.ln_xi_min / (double)(t.n_xi - 1) : 0.5 / (double)(t.n_xi - 1);
     t.guide = c->guide[species];
     t.guide_bins = kGuideBins;
+    t.guide_split = species == 0 ? 1 : 0;
     t.guide_k0 = c->guide_k0[species];
     t.guide_inv_dk = c->guide_inv_dk[species];
     return t;

@@ -53,6 +53,7 @@ struct Table2D {      // rows: log-spaced chi; columns: xi grid
     // key_j = guide_k0 + j / guide_inv_dk: narrows the binary search of eq.25 / eq.29 without changing its result
     const unsigned short* guide;
     int guide_bins;
+    int guide_split;  // 1 (photon emission): lower half of the bins uniform in ln r on [guide_k0, ln 1/2], upper half uniform in r on [1/2, 1]
     double guide_k0, guide_inv_dk;
 };
 
@@ -329,7 +330,7 @@ __device__ __forceinline__ void row_bracket(const Table2D<R>& T, double ln_chi, 
 struct GuideBracket { int lo, hi; bool guided; };
 constexpr int kGuideFastSpan = 5;   // brackets up to this wide are closed in one round trip (search_row); measured 8 -> 5 -> 4: config 3 event pass 0.0685 -> 0.0669 -> 0.0655 ms, config 5 1.568 -> 1.556 -> 1.558 ms
 template <typename R>
-__device__ __forceinline__ GuideBracket guide_bracket(const Table2D<R>& T, int k, double key) {
+__device__ __forceinline__ GuideBracket guide_bracket(const Table2D<R>& T, int k, double key, double r = 0.0) {
     GuideBracket g;
     g.lo = 0;
     g.hi = T.n_xi - 1;
@@ -337,6 +338,10 @@ __device__ __forceinline__ GuideBracket guide_bracket(const Table2D<R>& T, int k
     if (g.guided) {
         const int J = T.guide_bins;
         int j = (int)((key - T.guide_k0) * T.guide_inv_dk);
+        if (T.guide_split) {   // (key = ln r; the bins above J/2 are uniform in r itself)
+            j = min(j, J / 2 - 1);
+            if (r >= 0.5) j = J / 2 + (int)((r - 0.5) * (double)J);
+        }
         j = max(0, min(j, J - 1));
         const unsigned short* g0 = T.guide + (size_t)k * (J + 1) + j;
         const unsigned short* g1 = g0 + (J + 1);
@@ -445,13 +450,13 @@ __device__ __forceinline__ int search_row(const Table2D<R>& T, int k, double w, 
     return lo;
 }
 
-// eqs.28-30: xi = chi_gamma/chi of the emitted photon for uniform r (lr = ln r).
+// eqs.28-30: xi = chi_gamma/chi of the emitted photon for uniform r (lr = ln r, both passed).
 // Event arithmetic is fp64 whatever the table element type (events are rare).
 template <typename R>
-__device__ __forceinline__ double qs_sample_xi_ln(const Table2D<R>& T, double ln_chi, double lr) {
+__device__ __forceinline__ double qs_sample_xi_ln(const Table2D<R>& T, double ln_chi, double lr, double r) {
     int k; double w;
     row_bracket(T, ln_chi, &k, &w);
-    const GuideBracket gb = guide_bracket(T, k, lr);
+    const GuideBracket gb = guide_bracket(T, k, lr, r);
     double a, b;
     const int ms = search_row(T, k, w, lr, gb, &a, &b);        // eq.29
     if (ms < 0) return exp_fast(T.ln_xi_min);                  // below the first column (R6)
@@ -462,7 +467,7 @@ __device__ __forceinline__ double qs_sample_xi_ln(const Table2D<R>& T, double ln
 }
 template <typename R>
 __device__ __forceinline__ double qs_sample_xi(const Table2D<R>& T, double ln_chi, double r) {
-    return qs_sample_xi_ln(T, ln_chi, log_pos(r));
+    return qs_sample_xi_ln(T, ln_chi, log_pos(r), r);
 }
 
 // eqs.24-26 on r' = min(r, 1-r): xi = chi_-/chi_gamma in [0, 1/2]
