@@ -93,6 +93,9 @@ int picsarqed_version(void);
  * "event_config" 0..1 = shape of the event kernel; "time_kernels" 0/1; "stage_records" 0/1 (see
  * evolve_optical_depth); "fused_step" 0/1 = qed_step as one warp-specialised kernel (experimental, slower today: DESIGN.md 11),
  * with "step_config", "step_spill", "step_batch_wait" its tuning knobs;
+ * "evolve_redraw" 0..2 = which pass of qed_step re-draws the optical depth of the leptons that emit (same Philox words, same
+ * value either way): 0 = the event pass (a fourth scattered store per event), 1 = the evolve pass for fp64 particles, 2 (default)
+ * = the evolve pass for every dtype (the new value leaves with the pass's own vector store);
  * "host_slabs" 0..64 = number of slabs step_host pipelines (0 = automatic: slabs of at least
  * 2^20 particles, at most 32; 1 = copy in, step, copy out, one after the other). */
 int picsarqed_set_option(picsarqed_ctx* ctx, const char* name, long long value);

@@ -162,10 +162,10 @@ __device__ __forceinline__ void event_commit(const EventArgs<R, TR>& a, long lon
     a.out_tau[0][slot] = o.sec_tau[0];
     if (KIND == 1) a.out_tau[1][slot] = o.sec_tau[1];
     if (a.parent) a.parent[slot] = a.parent_base + i;
-    if (parent_done) return;   // (a photon the evolve pass removed itself)
+    if (parent_done && KIND == 1) return;   // (a photon the evolve pass removed itself)
 #pragma unroll
     for (int c = 0; c < 3; ++c) a.p[c][i] = o.parent_p[c];
-    a.tau[i] = o.parent_tau;
+    if (!parent_done) a.tau[i] = o.parent_tau;   // (parent_done, lepton: the evolve pass stored the new optical depth itself)
 }
 
 // ---- level 1 for generate_*: count the fired particles of every chunk --------------------------

@@ -37,6 +37,11 @@ struct EvolveArgs {
     unsigned int* tile_sum;
     int chunks_per_tile;
     int remove_photons;         // EMIT, photons: 1 = the pass removes the photons it stages (qed_step), 0 = it only stages
+    // EMIT, leptons: 1 = the pass also re-draws the optical depth of the leptons it stages (qed_step: tau = -ln U from the parent's
+    // Philox words), so that it leaves with the pass's own vector store and the event pass rewrites three scattered
+    // sectors per event instead of four; the evolved value stays in the record (capacity rule)
+    int redraw_tau;
+    unsigned long long seed, step, id_base;
     UnitScales units;           // the caller's unit system (picsarqed_set_units)
 };
 
@@ -48,8 +53,8 @@ constexpr int kStageCap = 24;               // records per chunk segment (mean a
 // records (segment overflow, or counted by count_chunks_kernel: generate_* calls and the ragged last tile)
 // bit 14 = the events of the chunk have been generated already (fused step, step.cuh): its segment holds StepResult
 // records -- the secondaries, waiting for their slots
-// bit 13 = the chunk's records are those of photons the evolve pass has removed already (p = 0, tau = +inf written with
-// its own stores, while the sectors were in L2): the event pass only creates the pairs
+// bit 13 = the evolve pass has done its part of the parents' rewrite already, with its own stores: photons are removed (p = 0,
+// tau = +inf: the event pass only creates the pairs), leptons have their new optical depth (the event pass rewrites the momentum only)
 constexpr unsigned short kStageCountMask = 0x1FFFu;
 constexpr unsigned short kStageNoRecords = 0x8000u;
 constexpr unsigned short kStageDone = 0x4000u;
@@ -294,6 +299,7 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ unsigned long long mbar;
     __shared__ unsigned int warp_counts[kEvolveThreads / 32];
+    __shared__ double tau_new_s[(EMIT && SPECIES == 0) ? kEvolveThreads / 32 : 1][(EMIT && SPECIES == 0) ? kStageCap : 1];
 
     const R* tab = a.tab.L;
     if (a.table_in_smem) {
@@ -365,8 +371,9 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                 }
                 const long long chunk = (base + (long long)warp * WCH) / kChunk;
                 if (lane == 0) {
+                    const bool part_done = SPECIES == 1 ? a.remove_photons != 0 : a.redraw_tau != 0;
                     a.stage_cnt[chunk] = (unsigned short)(total <= (unsigned)kStageCap
-                                                              ? (SPECIES == 1 && total > 0 && a.remove_photons ? (total | kStageParentDone) : total)
+                                                              ? (total > 0 && part_done ? (total | kStageParentDone) : total)
                                                               : (total | kStageNoRecords));
                     if (total > 0) atomicAdd(a.tile_sum + chunk / kEventTileChunks, total);
                 }
@@ -389,6 +396,25 @@ evolve_kernel(const EvolveArgs<R, TR> a) {
                                 rec.tau_ev = (double)t[u].v[v];
                                 ++r;
                             }
+                        }
+                    }
+                    if (SPECIES == 0 && a.redraw_tau) {
+                        // the new optical depths of the chunk's leptons in one pass: lane r serves record r (<= kStageCap < 32)
+                        __syncwarp();
+                        TR* tnew = reinterpret_cast<TR*>(tau_new_s[warp]);
+                        if (lane < (int)total) {
+                            const unsigned long long id =
+                                a.id_base + (unsigned long long)(base + (long long)warp * WCH + (long long)wbuf[lane].idx);
+                            const Words4 w = qed_words(a.seed, id, a.step, 1, 0);
+                            tnew[lane] = draw_tau<TR>(w.w[2], w.w[3]);
+                        }
+                        __syncwarp();
+#pragma unroll
+                        for (int u = 0; u < U; ++u) {
+                            unsigned int r = rank_u[u];
+#pragma unroll
+                            for (int v = 0; v < V; ++v)
+                                if ((fired_bits >> (u * V + v)) & 1u) t[u].v[v] = tnew[r++];
                         }
                     }
                     if (SPECIES == 1 && a.remove_photons) {

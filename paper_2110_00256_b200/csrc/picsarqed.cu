@@ -65,6 +65,7 @@ struct picsarqed_ctx {
     int step_spill = 0;          // fused kernel: 1 = a streaming warp whose queue is full hands the chunk to the record path
     int step_batch_wait = 0;     // fused kernel: polls (2 us each) an event warp waits for four chunks before it takes fewer
     int step_config = 0;         // fused kernel: see launch_fused_step
+    int evolve_redraw = 2;       // qed_step of leptons: see launch_step
     int time_kernels = 0;        // qed_step brackets its evolve pass and its event pass with CUDA events
     std::vector<cudaEvent_t> timing_events;  // triples (start, after evolve, after events), not yet read
     // per-chunk scratch of the event path: staged records, counts, output offsets (see events.cuh)
@@ -428,6 +429,8 @@ int picsarqed_set_option(picsarqed_ctx* c, const char* name, long long value) {
         c->fused_step = (int)value;
     else if (!std::strcmp(name, "stage_records") && (value == 0 || value == 1))
         c->stage_records = (int)value;
+    else if (!std::strcmp(name, "evolve_redraw") && value >= 0 && value <= 2)
+        c->evolve_redraw = (int)value;
     else if (!std::strcmp(name, "step_config") && value >= 0 && value <= 1)
         c->step_config = (int)value;
     else if (!std::strcmp(name, "step_spill") && (value == 0 || value == 1))
@@ -569,7 +572,8 @@ int launch_chi(picsarqed_ctx* c, long long n, const void* const* a, void* out) {
     return PICSARQED_OK;
 }
 
-struct StageView { unsigned char* rec; unsigned short* cnt; unsigned int* tile_sum; int chunks_per_tile; long long stride; int remove_photons; };
+struct StageView { unsigned char* rec; unsigned short* cnt; unsigned int* tile_sum; int chunks_per_tile; long long stride; int remove_photons;
+                   int redraw_tau = 0; unsigned long long seed = 0, step = 0, id_base = 0; };
 
 template <typename R, typename TR, int SPECIES, int U, bool EMIT>
 int launch_evolve_u(picsarqed_ctx* c, long long n, const void* const* a, double dt, void* tau,
@@ -596,6 +600,10 @@ int launch_evolve_u(picsarqed_ctx* c, long long n, const void* const* a, double 
     args.tile_sum = sv.tile_sum;
     args.chunks_per_tile = sv.chunks_per_tile;
     args.remove_photons = sv.remove_photons;
+    args.redraw_tau = sv.redraw_tau;
+    args.seed = sv.seed;
+    args.step = sv.step;
+    args.id_base = sv.id_base;
     size_t smem = ((size_t)args.tab.n * sizeof(R) + 127) & ~(size_t)127;
     args.table_in_smem = smem <= 96 * 1024;  // larger tables are read through L1/L2
     if (!args.table_in_smem) smem = 0;
@@ -830,6 +838,8 @@ int launch_fused_step_c(picsarqed_ctx* c, long long n, void* const* p, const voi
     args.tile_sum = cs.sum;
     args.chunks_per_tile = event_chunks_per_tile(c);
     args.remove_photons = 0;
+    args.redraw_tau = 0;
+    args.seed = args.step = args.id_base = 0;
     // shared memory: [1D table][sub-chunk stages][record queues]; a table that does not fit beside them is read through L1
     constexpr size_t kSmemMax = 227 * 1024 - 2048;   // (2 KB: the kernel's static shared memory)
     size_t smem = ((size_t)args.tab.n * sizeof(R) + 127) & ~(size_t)127;
@@ -924,6 +934,12 @@ int launch_step(picsarqed_ctx* c, long long n, void* const* p, const void* const
     sv.tile_sum = cs.sum;
     sv.chunks_per_tile = event_chunks_per_tile(c);
     sv.remove_photons = 1;
+    // "evolve_redraw": 0 = the event pass re-draws the parents' optical depth, 1 = the evolve pass does, for fp64 particles
+    // (whose evolve pass waits for HBM and has the issue slots), 2 = for every dtype
+    sv.redraw_tau = SPECIES == 0 && (c->evolve_redraw == 2 || (c->evolve_redraw == 1 && sizeof(R) == 8)) ? 1 : 0;
+    sv.seed = seed;
+    sv.step = step;
+    sv.id_base = id_base;
     const void* a9[9] = {p[0], p[1], p[2], eb[0], eb[1], eb[2], eb[3], eb[4], eb[5]};
     constexpr int U = kChunk / (32 * (16 / (int)sizeof(R)));  // fp64: 2, fp32: 1
     StepEvents se;
