@@ -62,10 +62,9 @@ constexpr unsigned short kStageParentDone = 0x2000u;
 
 // one staged record: what event generation needs of a particle that fired -- its momentum, chi^2 (computed by the
 // evolve pass anyway) and its index inside the chunk.  Sizes are multiples of 16 bytes so that records move as
-// 128-bit vectors.  (Also staging the fields, 80 B, and letting the evolve pass re-draw the parent's optical depth
-// -- in the owner lanes, or compacted into one warp pass per chunk with the evolved value kept in the record's spare
-// bytes for the capacity rule -- were measured: the first made the evolve pass slower by more than the event pass
-// gained; the last gave evolve +12 us, events -16 us: 1 % of the step for 5 points of the evolve pass's HBM fraction.)
+// 128-bit vectors.  (Also staging the fields, 80 B, was measured: it made the evolve pass slower by more than the event
+// pass gained.  Re-drawing the parent's optical depth in the evolve pass -- compacted into one warp pass per chunk, the
+// evolved value kept in the record for the capacity rule -- is what EvolveArgs::redraw_tau does.)
 template <typename R> struct StageRecord;
 // tau_ev: the evolved optical depth (what undoes a removed photon that falls beyond the capacity of the output)
 template <> struct alignas(16) StageRecord<double> {
