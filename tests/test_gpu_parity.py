@@ -490,6 +490,35 @@ def test_fused_kernel_matches_the_two_kernel_step(orc, qed, ctx, mid_tables, spe
                 assert ref["n_fired"] > 0.5 * target * n
 
 
+@pytest.mark.parametrize("dtype,tdtype", DTYPES, ids=IDS)
+def test_optical_depth_redrawn_by_either_pass(orc, qed, ctx, mid_tables, dtype, tdtype):
+    """option "evolve_redraw": whether the evolve pass (one Philox pass per chunk, the new value leaves with the pass's vector store)
+    or the event pass (a fourth scattered store) re-draws the optical depth of the leptons that emit, every output is the same bit
+    for bit -- all tiles, a ragged end, chunks with more than 24 events (which the event pass re-scans: their parents are re-drawn
+    there), and a capacity below the number of events: the parents beyond it keep their evolved, negative optical depth"""
+    for n, target in ((9 * 2048 + 777, 0.06), (2 * 2048 + 5, 0.5), (300, 0.06)):
+        p, e, b = qed.workloads.config1(seed=61, n=n, species=LEPTON, dtype=dtype)
+        tables = _tables_for(mid_tables, dtype)
+        dt = qed.workloads.choose_dt(orc.rate(tables, LEPTON, p, e, b), target)
+        tau0 = orc.init_optical_depth(LEPTON, code(tdtype), n, 9).astype(tdtype)
+        for cap in (n, max(1, n // 50)):
+            runs = []
+            for mode in (0, 1, 2):
+                ctx.set_option("evolve_redraw", mode)
+                try:
+                    runs.append(_run_fused(qed, ctx, LEPTON, dtype, tdtype, p, e, b, tau0, dt, 5, 3, 1 << 35, cap))
+                finally:
+                    ctx.set_option("evolve_redraw", 2)
+            ref = runs[0]
+            for got in runs[1:]:
+                assert got["n_fired"] == ref["n_fired"] and _same(got["parent"], ref["parent"])
+                assert _same(got["tau"], ref["tau"]) and all(_same(x, y) for x, y in zip(got["p"], ref["p"]))
+                assert all(_same(x, y) for x, y in zip(got["sec_p"][0], ref["sec_p"][0]))
+                assert _same(got["sec_tau"][0], ref["sec_tau"][0])
+            if cap < ref["n_fired"]:
+                assert int((ref["tau"] < 0).sum()) == ref["n_fired"] - cap     # the parents beyond the capacity wait, untouched
+
+
 def test_staged_records_are_dropped_when_not_consumed(orc, qed, ctx, mid_tables):
     """"stage_records": records staged by an evolve call that no generate call consumes (another evolve, another array,
     another size in between) must not leak into the next event pass"""
