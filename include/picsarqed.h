@@ -93,6 +93,8 @@ int picsarqed_version(void);
  * "event_config" 0..1 = shape of the event kernel; "time_kernels" 0/1; "stage_records" 0/1 (see
  * evolve_optical_depth); "fused_step" 0/1 = qed_step as one warp-specialised kernel (experimental, slower today: DESIGN.md 11),
  * with "step_config", "step_spill", "step_batch_wait" its tuning knobs;
+ * "event_pdl" 0/1 (default 1) = the event kernel is launched as a programmatic dependent of the offsets scan (its CTAs become
+ * resident while the scan runs and wait for it at griddepcontrol.wait);
  * "evolve_redraw" 0..2 = which pass of qed_step re-draws the optical depth of the leptons that emit (same Philox words, same
  * value either way): 0 = the event pass (a fourth scattered store per event), 1 = the evolve pass for fp64 particles, 2 (default)
  * = the evolve pass for every dtype (the new value leaves with the pass's own vector store);

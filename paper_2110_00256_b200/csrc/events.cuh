@@ -212,6 +212,7 @@ __global__ void __launch_bounds__(kScanThreads) tile_scan_kernel(const unsigned 
                                                                  const unsigned long long* d_entries,
                                                                  unsigned int* __restrict__ tile_sum) {
     __shared__ unsigned long long warp_sum[2][kScanThreads / 32];
+    asm volatile("griddepcontrol.launch_dependents;");   // (the event kernel may take its place on the SMs; it waits for this grid's end)
     if (d_entries) {
         const unsigned long long live = (*d_entries + kChunk - 1) / kChunk;
         if (live < (unsigned long long)n_chunks) n_chunks = (long long)live;
@@ -302,6 +303,9 @@ __global__ void __launch_bounds__(THREADS, MINB) event_kernel(const EventArgs<R,
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const long long n_chunks = (a.n + kChunk - 1) / kChunk;
     const long long n_tiles = (n_chunks + CHUNKS - 1) / CHUNKS;
+    // launched as a programmatic dependent of tile_scan_kernel: everything before this line overlaps the scan; the tile
+    // offsets (and everything the kernels before it wrote) are visible after it.  A no-op in an ordinary launch.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     // Persistent CTAs stride over the tiles.  The warps of a CTA walk the same tiles in the same order but do
     // not wait for one another (no barrier on the common path): a warp whose slice of a tile holds no event is
     // already loading the next tile.  The loads of the next tile are issued before the current one is processed.

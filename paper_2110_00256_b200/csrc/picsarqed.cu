@@ -66,6 +66,7 @@ struct picsarqed_ctx {
     int step_batch_wait = 0;     // fused kernel: polls (2 us each) an event warp waits for four chunks before it takes fewer
     int step_config = 0;         // fused kernel: see launch_fused_step
     int evolve_redraw = 2;       // qed_step of leptons: see launch_step
+    int event_pdl = 1;           // the event kernel is launched as a programmatic dependent of the offsets scan
     int time_kernels = 0;        // qed_step brackets its evolve pass and its event pass with CUDA events
     std::vector<cudaEvent_t> timing_events;  // triples (start, after evolve, after events), not yet read
     // per-chunk scratch of the event path: staged records, counts, output offsets (see events.cuh)
@@ -429,6 +430,8 @@ int picsarqed_set_option(picsarqed_ctx* c, const char* name, long long value) {
         c->fused_step = (int)value;
     else if (!std::strcmp(name, "stage_records") && (value == 0 || value == 1))
         c->stage_records = (int)value;
+    else if (!std::strcmp(name, "event_pdl") && (value == 0 || value == 1))
+        c->event_pdl = (int)value;
     else if (!std::strcmp(name, "evolve_redraw") && value >= 0 && value <= 2)
         c->evolve_redraw = (int)value;
     else if (!std::strcmp(name, "step_config") && value >= 0 && value <= 1)
@@ -745,7 +748,18 @@ int launch_event_pass(picsarqed_ctx* c, long long n, const ChunkScratch& cs, voi
         PXQ_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, T, 0));                     \
         const unsigned grid = (unsigned)std::max<long long>(                                                 \
             1, std::min<long long>(n_tiles, (long long)c->num_sms * std::max(per_sm, 1)));                   \
-        kern<<<grid, T, 0, c->stream>>>(ev);                                                                 \
+        /* programmatic dependent launch: the CTAs become resident while the offsets scan (one CTA) still runs and wait   \
+           for it at griddepcontrol.wait -- the launch latency of this kernel is off the step's critical path */        \
+        cudaLaunchConfig_t cfg{};                                                                            \
+        cfg.gridDim = dim3(grid);                                                                            \
+        cfg.blockDim = dim3(T);                                                                              \
+        cfg.stream = c->stream;                                                                              \
+        cudaLaunchAttribute at[1];                                                                           \
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;                                       \
+        at[0].val.programmaticStreamSerializationAllowed = c->event_pdl ? 1 : 0;                             \
+        cfg.attrs = at;                                                                                      \
+        cfg.numAttrs = 1;                                                                                    \
+        PXQ_CUDA(c, cudaLaunchKernelEx(&cfg, kern, ev));                                                     \
     } while (0)
     switch (c->event_config) {
         case 1: PXQ_LAUNCH_EVENTS(256, kEventTileChunks, 3); break;
